@@ -1,0 +1,120 @@
+"""ctypes binding to oracle/oracle_dedisp.c (plain C, OpenMP over trials).
+
+TEST INFRASTRUCTURE ONLY -- see oracle/__init__.py.  The arithmetic lives in the C file; this
+module only marshals numpy arrays and composes steps O5 (sizes) from the C results.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle_dedisp.c")
+_LIB = os.path.join(_HERE, "liboracle_dedisp.so")
+_lib = None
+
+_ERRORS = {-1: "invalid argument", -2: "window exceeds the valid span (too short)", -3: "out of memory"}
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (baseline x86-64, -O3, OpenMP).  Returns the .so path."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.run(
+            ["gcc", "-O3", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"],
+            check=True,
+        )
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        i32, i64, f64, vp = ctypes.c_int32, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_channel_freqs.argtypes = [f64, f64, i32, vp]
+        lib.oracle_delay_table.argtypes = [f64, f64, i32, f64, i32, f64, f64, i32, vp]
+        lib.oracle_decimate.argtypes = [vp, i32, i64, i64, i32, vp]
+        lib.oracle_dedisperse.argtypes = [vp, i64, i64, vp, i32, vp, i32, i64, i64, vp]
+        for fn in (lib.oracle_channel_freqs, lib.oracle_delay_table, lib.oracle_decimate, lib.oracle_dedisperse):
+            fn.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise ValueError("oracle %s: %s (code %d)" % (what, _ERRORS.get(rc, "error"), rc))
+
+
+def _ptr(a: np.ndarray) -> int:
+    return a.ctypes.data
+
+
+def num_threads() -> int:
+    """OpenMP threads the oracle will use (OMP_NUM_THREADS or the host core count)."""
+    return int(_load().oracle_num_threads())
+
+
+def channel_freqs(f_top_mhz: float, chan_width_mhz: float, nchans: int) -> np.ndarray:
+    """O2: f_c = f_top + c*width."""
+    f = np.empty(nchans, dtype=np.float64)
+    _check(_load().oracle_channel_freqs(f_top_mhz, chan_width_mhz, nchans, _ptr(f)), "channel_freqs")
+    return f
+
+
+def delay_table(f_top_mhz, chan_width_mhz, nchans, tsamp_s, decim, dm_lo, dm_step, ndm) -> np.ndarray:
+    """O3+O4 (Eq. 1.1): int64 delays [ndm][nchans] in samples of tsamp*decim."""
+    d = np.empty((ndm, nchans), dtype=np.int64)
+    rc = _load().oracle_delay_table(f_top_mhz, chan_width_mhz, nchans, tsamp_s, decim, dm_lo, dm_step, ndm, _ptr(d))
+    _check(rc, "delay_table")
+    return d
+
+
+def range_sizes(nsamps: int, decim: int, delays: np.ndarray):
+    """O5: ns_r = nsamps // decim, maxd_r = largest delay of the range, nout_r = ns_r - maxd_r."""
+    ns_r = int(nsamps) // int(decim)
+    maxd = int(delays.max())
+    return ns_r, maxd, ns_r - maxd
+
+
+def decimate(x: np.ndarray, decim: int) -> np.ndarray:
+    """O6: y[c][t'] = sum_{i<decim} x[c][decim*t'+i] as uint32; x is [nchans][nsamps] uint8/uint16."""
+    if x.ndim != 2 or x.dtype not in (np.uint8, np.uint16):
+        raise ValueError("oracle decimate: x must be a 2-D uint8/uint16 array")
+    x = np.ascontiguousarray(x)
+    nchans, nsamps = x.shape
+    y = np.empty((nchans, nsamps // decim), dtype=np.uint32)
+    _check(_load().oracle_decimate(_ptr(x), 8 * x.dtype.itemsize, nchans, nsamps, decim, _ptr(y)), "decimate")
+    return y
+
+
+def dedisperse(y: np.ndarray, delays: np.ndarray, sel=None, t0: int = 0, nt: int | None = None) -> np.ndarray:
+    """O7: S[j][t'] = sum_c y[c][t'+d(c,j)] for trials `sel` and t' in [t0, t0+nt).
+
+    y: uint32 [nchans][ns_r] (output of decimate); delays: int64 [ndm][nchans].
+    nt defaults to the range's valid span nout_r - t0.  Returns float32 [len(sel)][nt].
+    """
+    if y.ndim != 2 or y.dtype != np.uint32:
+        raise ValueError("oracle dedisperse: y must be a 2-D uint32 array")
+    y = np.ascontiguousarray(y)
+    delays = np.ascontiguousarray(delays, dtype=np.int64)
+    nchans, ns_r = y.shape
+    ndm = delays.shape[0]
+    if delays.shape[1] != nchans:
+        raise ValueError("oracle dedisperse: delay table does not match nchans")
+    if sel is None:
+        sel_arr = np.arange(ndm, dtype=np.int32)
+    else:
+        sel_arr = np.ascontiguousarray(sel, dtype=np.int32)
+    if nt is None:
+        nt = ns_r - int(delays.max()) - t0
+    out = np.empty((len(sel_arr), nt), dtype=np.float32)
+    rc = _load().oracle_dedisperse(_ptr(y), nchans, ns_r, _ptr(delays), ndm, _ptr(sel_arr), len(sel_arr), t0, nt, _ptr(out))
+    _check(rc, "dedisperse")
+    return out
