@@ -1,0 +1,154 @@
+/*
+ * dd.h -- C ABI of libdd: brute-force incoherent dedispersion on one NVIDIA B200 (sm_100a).
+ *
+ * The operation (PAPER.md = /root/reference/PAPER.md, arxiv/paper_2605_03531):
+ *   - cold-plasma dispersion delay, PAPER.md:256-263 (Eq. 1.1):
+ *         dt = 4.14881 ms * DM * (nu1^-2 - nu2^-2)   [nu in GHz, DM in pc cm^-3]
+ *     turned into integer sample delays per channel c and trial j of range r
+ *         d_r(c,j) = round( K * DM_{r,j} * (f_c^-2 - f_top^-2) / (tsamp * decim_r) ),
+ *         K = 4.148808e3 s MHz^2 cm^3/pc, f in MHz, DM_{r,j} = dm_lo_r + j*dm_step_r,
+ *     evaluated in IEEE double, rounded half away from zero (BASELINE.json north_star;
+ *     DESIGN.md readings A1, A4, A6);
+ *   - brute-force dedispersion, the O(m x N) direct sum per trial of PAPER.md:421 (section 3.2),
+ *     over a plan of many trial DMs, PAPER.md:317 (section 2.1):
+ *         y_r[b][c][t'] = sum_{i<decim_r} in[b][c][decim_r*t' + i]            (time decimation, a SUM)
+ *         S_r[b][j][t'] = sum_{c<nchans} y_r[b][c][t' + d_r(c,j)]              t' = 0 .. nout_r-1
+ *         out           = fl32(S)                                              (one rounding, RNE)
+ *     with ns_r = nsamps / decim_r (tail dropped), maxd_r = d_r(nchans-1, ndm_r-1),
+ *     nout_r = ns_r - maxd_r (valid samples only; no padding, no wrap-around);
+ *   - DM = 0 is the plain channel sum ("0 DM time series").
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  All functions return
+ * 0 on success or a negative dd_status code; nothing throws or aborts across this boundary.
+ * "dev" pointers are CUDA device pointers on the device that was current at dd_plan_create;
+ * "host" pointers are ordinary host memory (pinned memory makes the *_host call asynchronous).
+ */
+#ifndef DD_H_
+#define DD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DD_VERSION 100 /* major*100 + minor */
+
+typedef enum dd_status {
+  DD_OK = 0,
+  DD_ERR_INVALID = -1,   /* null pointer; nchans<1; chan_width>=0; tsamp<=0; nsamps<1; nbeams<1;
+                            in_bits not 8/16; nranges<1; decim not in {1,2,4,8}; ndm<1; dm_lo<0; dm_step<0;
+                            bad range index; unknown kernel variant */
+  DD_ERR_TOO_SHORT = -2, /* some range has nout_r < 1 (largest delay >= decimated length) */
+  DD_ERR_OVERFLOW = -3,  /* nchans * (2^in_bits - 1) * decim >= 2^32: exact integer sums impossible */
+  DD_ERR_ALIGN = -4,     /* in_dev / out_dev / workspace not 16-byte aligned */
+  DD_ERR_CUDA = -5,      /* a CUDA runtime call failed; text via dd_last_cuda_error() */
+  DD_ERR_NOMEM = -6      /* host or device allocation failed; workspace too small */
+} dd_status;
+
+/* One DM range: trials DM_j = dm_lo + j*dm_step, j = 0..ndm-1, dedispersed on the input summed
+ * over `decim` adjacent samples (decim in {1,2,4,8}; 2/4/8 are used for high-DM ranges). */
+typedef struct dd_range {
+  double dm_lo;    /* pc cm^-3, >= 0 */
+  double dm_step;  /* pc cm^-3, >= 0 */
+  int32_t ndm;     /* >= 1 */
+  int32_t decim;   /* 1, 2, 4 or 8 */
+} dd_range_t;
+
+/* The filterbank and the DM plan.  `ranges` is copied by dd_plan_create. */
+typedef struct dd_config {
+  double f_top_mhz;       /* frequency of channel 0, the highest (reference) channel, MHz */
+  double chan_width_mhz;  /* f_c = f_top + c*chan_width; must be negative */
+  int32_t nchans;
+  double tsamp_s;         /* sampling time of the input, seconds */
+  int64_t nsamps;         /* time samples per channel */
+  int32_t nbeams;         /* independent beams sharing the plan, batched in one call */
+  int32_t in_bits;        /* 8 (uint8) or 16 (uint16) unsigned samples */
+  int32_t nranges;
+  const dd_range_t* ranges;
+} dd_config_t;
+
+typedef struct dd_plan dd_plan_t; /* opaque */
+
+/* Kernel variants selectable for tests and measurements (dd_plan_set_kernel). */
+#define DD_KERNEL_AUTO 0   /* the tiled kernel below, tile shape chosen per range */
+#define DD_KERNEL_DIRECT 1 /* one thread per (trial, sample), delays from a global table: slow, simple */
+#define DD_KERNEL_TILED 2  /* shared-memory staged, register-blocked, packed-lane adder (the product path) */
+
+/*
+ * dd_plan_create: host work (delay tables, per-range sizes, tile shapes) plus device allocations and
+ * table uploads on the current CUDA device.  Allocates the plan-owned workspace for the packed /
+ * decimated copies of the input unless dd_plan_set_workspace is called before the first execute.
+ * On success *plan_out owns all of it; release with dd_plan_destroy.  Synchronises the device once.
+ */
+int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out);
+
+/*
+ * dd_execute: enqueue the whole hot path on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ * legacy default stream): pack/decimate kernels for every range, then the dedispersion kernels, which
+ * write fp32 results straight into out_dev.  No host synchronisation, no allocation.
+ *   in_dev : [nbeams][nchans][nsamps], time contiguous, uint8 or uint16 (in_bits), 16-byte aligned,
+ *            read only.  (PAPER.md:351 keeps spectra time-major; channel-major is BASELINE.json's layout.)
+ *   out_dev: dd_plan_out_elems() floats, 16-byte aligned.  Beam b, range r, trial j, sample t' lives at
+ *            out_dev[b*beam_stride + offset_r + j*pitch_r + t'],  t' < nout_r; the pitch_r - nout_r pad
+ *            floats of each row are left untouched.
+ * One execute per plan may be in flight at a time (the workspace is shared).  The caller owns both
+ * buffers and the stream.
+ */
+int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* cuda_stream);
+
+/*
+ * dd_execute_host: the same path from HOST buffers, end to end: copies in_host to a plan-owned device
+ * buffer, runs dd_execute, copies the result back to out_host, all enqueued on `cuda_stream`, then
+ * synchronises that stream before returning.  Layouts as in dd_execute, except that whole rows are
+ * copied back, so the pad floats of out_host are overwritten with unspecified values.  The staging buffers are
+ * allocated on first use (DD_ERR_NOMEM if that fails) and freed by dd_plan_destroy.
+ */
+int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream);
+
+/* dd_plan_destroy: frees host and device memory of the plan.  NULL is a no-op returning DD_OK.  The
+ * caller must make sure no execute of this plan is still running. */
+int dd_plan_destroy(dd_plan_t* plan);
+
+/* ---- queries: host only, no device work ---------------------------------------------------- */
+
+/* Total floats of the output buffer (all beams, all ranges, pitch padding included). */
+int dd_plan_out_elems(const dd_plan_t* plan, int64_t* total_floats);
+/* Floats between consecutive beams in the output. */
+int dd_plan_beam_stride(const dd_plan_t* plan, int64_t* floats);
+/* Per-range sizes (any pointer may be NULL): ns_r, maxd_r, nout_r as defined above; pitch_floats =
+ * nout_r rounded up to a multiple of 32; offset_floats = start of the range within one beam. */
+int dd_plan_range_info(const dd_plan_t* plan, int32_t r, int64_t* ns_r, int64_t* maxd_r, int64_t* nout_r,
+                       int64_t* pitch_floats, int64_t* offset_floats);
+/* Test hook: copies the delay table of range r, int32 [ndm_r][nchans], into host_buf. */
+int dd_plan_get_delays(const dd_plan_t* plan, int32_t r, int32_t* host_buf);
+/* Sum over beams and ranges of ndm_r * nout_r (the "DM-trial x samples" of one execute) and the
+ * brute-force add count, that number times nchans (O(m x N) per trial). */
+int dd_plan_work(const dd_plan_t* plan, int64_t* dm_samples, int64_t* adds);
+/* Kernel launches one dd_execute enqueues (pack + dedispersion) with the current kernel variant. */
+int dd_plan_launches(const dd_plan_t* plan, int32_t* n_launches);
+
+/* ---- workspace and variants ------------------------------------------------------------------ */
+
+/* Bytes of device scratch dd_execute needs for the packed / decimated input copies. */
+int dd_plan_workspace_bytes(const dd_plan_t* plan, int64_t* bytes);
+/* Use caller-owned device scratch (16-byte aligned, >= dd_plan_workspace_bytes) instead of the plan's
+ * own; frees the plan-owned one.  dev == NULL switches back to a plan-owned allocation. */
+int dd_plan_set_workspace(dd_plan_t* plan, void* dev, int64_t bytes);
+/* Choose the dedispersion kernel variant (DD_KERNEL_*).  All variants produce identical bits. */
+int dd_plan_set_kernel(dd_plan_t* plan, int32_t variant);
+/* Tile shape the tiled kernel uses for range r (any pointer may be NULL): trials per CTA, packed time
+ * words per CTA, time lanes per packed word (8 = 16-bit lanes, 4 = 32-bit lanes), channels between
+ * flushes of the packed accumulators, and whether neighbouring-trial reuse is enabled. */
+int dd_plan_tile_info(const dd_plan_t* plan, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta,
+                      int32_t* lanes, int32_t* flush_chans, int32_t* reuse);
+
+/* ---- errors ---------------------------------------------------------------------------------- */
+const char* dd_strerror(int code);       /* static string for a dd_status */
+const char* dd_last_cuda_error(void);    /* text of the last CUDA failure seen by this thread ("" if none) */
+int dd_version(void);                    /* DD_VERSION */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DD_H_ */

@@ -1,0 +1,223 @@
+"""Thin ctypes binding to libdd.so -- same names as include/dd.h, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; there is no CPU fallback.
+If the library is missing or cannot be loaded this module raises at import of the symbol, loudly.
+Device memory and streams come from PyTorch (`tensor.data_ptr()`, `torch.cuda.current_stream()`).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import List, Optional, Sequence, Tuple
+
+from .build import LIB, build
+
+DD_OK = 0
+DD_ERR_INVALID, DD_ERR_TOO_SHORT, DD_ERR_OVERFLOW, DD_ERR_ALIGN, DD_ERR_CUDA, DD_ERR_NOMEM = -1, -2, -3, -4, -5, -6
+DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED = 0, 1, 2
+
+# every symbol include/dd.h declares
+SYMBOLS = [
+    "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
+    "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
+    "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
+    "dd_strerror", "dd_last_cuda_error", "dd_version",
+]
+
+
+class dd_range_t(ctypes.Structure):
+    _fields_ = [("dm_lo", ctypes.c_double), ("dm_step", ctypes.c_double), ("ndm", ctypes.c_int32), ("decim", ctypes.c_int32)]
+
+
+class dd_config_t(ctypes.Structure):
+    _fields_ = [
+        ("f_top_mhz", ctypes.c_double), ("chan_width_mhz", ctypes.c_double), ("nchans", ctypes.c_int32),
+        ("tsamp_s", ctypes.c_double), ("nsamps", ctypes.c_int64), ("nbeams", ctypes.c_int32),
+        ("in_bits", ctypes.c_int32), ("nranges", ctypes.c_int32), ("ranges", ctypes.POINTER(dd_range_t)),
+    ]
+
+
+class DDError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        self.code = code
+        lib = _load()
+        msg = lib.dd_strerror(code).decode()
+        if code == DD_ERR_CUDA:
+            msg += " -- " + lib.dd_last_cuda_error().decode()
+        super().__init__("%s failed: %s (code %d)" % (what, msg, code))
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB):
+            build()
+        lib = ctypes.CDLL(LIB)  # raises OSError if the CUDA extension is missing: no fallback
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        P = ctypes.POINTER
+        lib.dd_plan_create.argtypes = [P(dd_config_t), P(vp)]
+        lib.dd_execute.argtypes = [vp, vp, vp, vp]
+        lib.dd_execute_host.argtypes = [vp, vp, vp, vp]
+        lib.dd_plan_destroy.argtypes = [vp]
+        lib.dd_plan_out_elems.argtypes = [vp, P(i64)]
+        lib.dd_plan_beam_stride.argtypes = [vp, P(i64)]
+        lib.dd_plan_range_info.argtypes = [vp, i32, P(i64), P(i64), P(i64), P(i64), P(i64)]
+        lib.dd_plan_get_delays.argtypes = [vp, i32, vp]
+        lib.dd_plan_work.argtypes = [vp, P(i64), P(i64)]
+        lib.dd_plan_launches.argtypes = [vp, P(i32)]
+        lib.dd_plan_workspace_bytes.argtypes = [vp, P(i64)]
+        lib.dd_plan_set_workspace.argtypes = [vp, vp, i64]
+        lib.dd_plan_set_kernel.argtypes = [vp, i32]
+        lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
+        lib.dd_strerror.argtypes = [ctypes.c_int]
+        lib.dd_strerror.restype = ctypes.c_char_p
+        lib.dd_last_cuda_error.restype = ctypes.c_char_p
+        for name in SYMBOLS:
+            getattr(lib, name)  # AttributeError if the library does not export it
+        _lib = lib
+    return _lib
+
+
+def library_path() -> str:
+    return LIB
+
+
+def dd_version() -> int:
+    return int(_load().dd_version())
+
+
+def dd_strerror(code: int) -> str:
+    return _load().dd_strerror(code).decode()
+
+
+def _chk(rc: int, what: str) -> None:
+    if rc != DD_OK:
+        raise DDError(rc, what)
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        return None
+    if isinstance(stream, int):
+        return stream or None
+    return int(stream.cuda_stream) or None  # torch.cuda.Stream
+
+
+class Plan:
+    """Owns a dd_plan_t*.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, f_top_mhz: float, chan_width_mhz: float, nchans: int, tsamp_s: float, nsamps: int,
+                 ranges: Sequence[Tuple[float, float, int, int]], nbeams: int = 1, in_bits: int = 8):
+        lib = _load()
+        arr = (dd_range_t * max(1, len(ranges)))()
+        for i, (lo, step, ndm, decim) in enumerate(ranges):
+            arr[i] = dd_range_t(float(lo), float(step), int(ndm), int(decim))
+        cfg = dd_config_t(float(f_top_mhz), float(chan_width_mhz), int(nchans), float(tsamp_s), int(nsamps),
+                          int(nbeams), int(in_bits), len(ranges), arr)
+        h = ctypes.c_void_p()
+        _chk(lib.dd_plan_create(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create")
+        self._h = h
+        self.nranges = len(ranges)
+        self.nchans, self.nbeams, self.in_bits, self.nsamps = int(nchans), int(nbeams), int(in_bits), int(nsamps)
+        self.ranges = [(float(a), float(b), int(c), int(d)) for a, b, c, d in ranges]
+
+    @classmethod
+    def from_workload(cls, w) -> "Plan":
+        return cls(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, w.nsamps,
+                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits)
+
+    # -- dd_plan_destroy
+    def destroy(self) -> None:
+        if getattr(self, "_h", None):
+            _load().dd_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # -- dd_execute / dd_execute_host
+    def execute(self, in_dev, out_dev, stream=None) -> None:
+        """in_dev / out_dev: torch CUDA tensors (or raw device pointers as int)."""
+        ip = in_dev if isinstance(in_dev, int) else in_dev.data_ptr()
+        op = out_dev if isinstance(out_dev, int) else out_dev.data_ptr()
+        _chk(_load().dd_execute(self._h, ip, op, _stream_ptr(stream)), "dd_execute")
+
+    def execute_host(self, in_host, out_host, stream=None) -> None:
+        """in_host / out_host: host buffers (numpy arrays, pinned torch tensors, or int addresses)."""
+        def addr(a):
+            if isinstance(a, int):
+                return a
+            if hasattr(a, "data_ptr"):
+                return a.data_ptr()
+            return a.ctypes.data
+        _chk(_load().dd_execute_host(self._h, addr(in_host), addr(out_host), _stream_ptr(stream)), "dd_execute_host")
+
+    # -- queries
+    def out_elems(self) -> int:
+        v = ctypes.c_int64()
+        _chk(_load().dd_plan_out_elems(self._h, ctypes.byref(v)), "dd_plan_out_elems")
+        return v.value
+
+    def beam_stride(self) -> int:
+        v = ctypes.c_int64()
+        _chk(_load().dd_plan_beam_stride(self._h, ctypes.byref(v)), "dd_plan_beam_stride")
+        return v.value
+
+    def range_info(self, r: int) -> dict:
+        vals = [ctypes.c_int64() for _ in range(5)]
+        _chk(_load().dd_plan_range_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_range_info")
+        keys = ["ns", "maxd", "nout", "pitch", "offset"]
+        d = {k: v.value for k, v in zip(keys, vals)}
+        d["ndm"] = self.ranges[r][2]
+        d["decim"] = self.ranges[r][3]
+        return d
+
+    def get_delays(self, r: int):
+        import numpy as np
+        buf = np.empty((self.ranges[r][2], self.nchans), dtype=np.int32)
+        _chk(_load().dd_plan_get_delays(self._h, r, buf.ctypes.data), "dd_plan_get_delays")
+        return buf
+
+    def work(self) -> Tuple[int, int]:
+        a, b = ctypes.c_int64(), ctypes.c_int64()
+        _chk(_load().dd_plan_work(self._h, ctypes.byref(a), ctypes.byref(b)), "dd_plan_work")
+        return a.value, b.value
+
+    def launches(self) -> int:
+        v = ctypes.c_int32()
+        _chk(_load().dd_plan_launches(self._h, ctypes.byref(v)), "dd_plan_launches")
+        return v.value
+
+    def workspace_bytes(self) -> int:
+        v = ctypes.c_int64()
+        _chk(_load().dd_plan_workspace_bytes(self._h, ctypes.byref(v)), "dd_plan_workspace_bytes")
+        return v.value
+
+    def set_workspace(self, dev, nbytes: int = 0) -> None:
+        ptr = None if dev is None else (dev if isinstance(dev, int) else dev.data_ptr())
+        if dev is not None and not isinstance(dev, int) and not nbytes:
+            nbytes = dev.numel() * dev.element_size()
+        _chk(_load().dd_plan_set_workspace(self._h, ptr, int(nbytes)), "dd_plan_set_workspace")
+        self._ws_ref = dev  # keep the tensor alive
+
+    def set_kernel(self, variant: int) -> None:
+        _chk(_load().dd_plan_set_kernel(self._h, int(variant)), "dd_plan_set_kernel")
+
+    def tile_info(self, r: int) -> dict:
+        vals = [ctypes.c_int32() for _ in range(5)]
+        _chk(_load().dd_plan_tile_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_tile_info")
+        return {k: v.value for k, v in zip(["dm_per_cta", "words_per_cta", "lanes", "flush_chans", "reuse"], vals)}
+
+    # -- convenience for callers holding torch tensors
+    def view_range(self, out, r: int, beam: int = 0):
+        """View of the valid [ndm_r][nout_r] block of range r, beam `beam`, inside the flat output."""
+        info = self.range_info(r)
+        base = beam * self.beam_stride() + info["offset"]
+        flat = out.reshape(-1)[base: base + info["ndm"] * info["pitch"]]
+        return flat.reshape(info["ndm"], info["pitch"])[:, : info["nout"]]

@@ -1,0 +1,86 @@
+// dd_internal.h -- private declarations shared by dd_plan.cu (host plan builder + C ABI) and
+// dd_kernels.cu (CUDA kernels + launchers).  Not part of the public boundary (include/dd.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "dd.h"
+
+namespace dd {
+
+// Packed time word ("superword"): 16 bytes holding NL time lanes of one channel.
+//   lane m of superword i is the decimated sample y[i + m*H]   (H = lane segment length)
+//   NL = 8: eight 16-bit lanes (word q holds lanes 2q (low half) and 2q+1 (high half))
+//   NL = 4: four 32-bit lanes
+// A delay of d samples is a shift of d superwords for every lane at once, so any delay is a
+// 16-byte aligned access.
+constexpr int kSuperwordBytes = 16;
+constexpr int kRD = 4;            // trials register-blocked per thread
+
+struct RangePlan {
+  // definition
+  double dm_lo = 0, dm_step = 0;
+  int ndm = 0, decim = 1;
+  int64_t ns = 0, maxd = 0, nout = 0, pitch = 0, offset = 0;
+  std::vector<int32_t> delays;  // host copy [ndm][nchans]
+  // tiled kernel shape
+  int NL = 8;        // lanes per superword
+  int flush = 0;     // channels between flushes of the 16-bit lanes (0: never, 32-bit lanes)
+  int G = 0;         // trial groups per CTA (kRD trials each)
+  int T = 0;         // superwords per CTA (multiple of 32)
+  int Dcta = 0;      // trials per CTA = G*kRD
+  int Cc = 0;        // channels per pipeline stage
+  int stages = 0;
+  int tiled_ok = 0;  // 0: the tile does not fit shared memory, this range runs the direct kernel
+  int reuse = 0;     // skip shared-memory reloads when neighbouring trials share a delay
+  int nblocks = 0;   // trial blocks = ceil(ndm/Dcta)
+  int Smax = 0;      // largest delay spread inside one trial block (superwords)
+  int Cpad = 0;      // nchans rounded up to a multiple of Cc (zero rows)
+  int64_t H = 0;     // lane segment length (superwords), multiple of 16
+  int64_t Wp = 0;    // row pitch of the packed array (superwords), multiple of 4
+  int64_t ntau = 0;  // time tiles = ceil(H/T)
+  int64_t ws_offset = 0;  // byte offset of this range's packed array in the workspace
+  int64_t ws_bytes = 0;
+  size_t smem_bytes = 0;
+  // device tables
+  uint32_t* d_meta = nullptr;   // [nblocks][Cpad][Dcta] byte offsets (delay - dmin) * 16
+  int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
+  int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
+  int32_t* d_delays = nullptr;  // [ndm][nchans], only for the direct kernel (lazy)
+};
+
+}  // namespace dd
+
+struct dd_plan {
+  // config
+  double f_top = 0, cw = 0, tsamp = 0;
+  int nchans = 0, nbeams = 0, in_bits = 8;
+  int64_t nsamps = 0;
+  std::vector<dd::RangePlan> ranges;
+  int64_t beam_stride = 0, out_elems = 0;
+  int64_t dm_samples = 0, adds = 0;
+  int device = 0;
+  int variant = DD_KERNEL_AUTO;
+  // workspace
+  int64_t ws_bytes = 0;
+  void* ws = nullptr;
+  bool ws_owned = false;
+  // host-path staging
+  void* h_in_dev = nullptr;
+  float* h_out_dev = nullptr;
+};
+
+namespace dd {
+
+// launchers (dd_kernels.cu); all enqueue on `stream` and return the CUDA error of the launch
+cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream);
+cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream);
+cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_dev, float* out_dev,
+                          cudaStream_t stream);
+cudaError_t configure_kernels(const dd_plan* p);  // opt in to the dynamic shared memory sizes
+size_t tiled_smem_bytes(const RangePlan& r);
+
+}  // namespace dd

@@ -1,0 +1,467 @@
+// dd_plan.cu -- host side of libdd: the C ABI of include/dd.h, the plan / delay-table builder
+// (step a1 of SURVEY.md 8(a)) and the execute sequencing.  No torch types, no exceptions across
+// the boundary.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "dd_internal.h"
+
+namespace {
+
+thread_local std::string g_last_cuda_error;
+
+int cuda_fail(cudaError_t e, const char* what) {
+  g_last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
+  return DD_ERR_CUDA;
+}
+#define DD_CUDA(call)                                      \
+  do {                                                     \
+    cudaError_t e__ = (call);                              \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call);  \
+  } while (0)
+
+// Dispersion constant of the north_star, s MHz^2 cm^3 / pc  (PAPER.md:258 prints 4.14881 ms GHz^2).
+constexpr double kDispersion = 4.148808e3;
+
+inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+// a1: d_r(c,j) = round(K * DM_j * (f_c^-2 - f_top^-2) / (tsamp*decim)), double precision, half away
+// from zero (the argument is never negative).  PAPER.md:258 Eq. 1.1; readings A1, A4, A6.
+bool build_delays(const dd_plan& p, dd::RangePlan& r) {
+  const double ts = p.tsamp * (double)r.decim;
+  const double inv_top = 1.0 / (p.f_top * p.f_top);
+  r.delays.resize((size_t)r.ndm * p.nchans);
+  for (int j = 0; j < r.ndm; ++j) {
+    const double dm = r.dm_lo + (double)j * r.dm_step;
+    for (int c = 0; c < p.nchans; ++c) {
+      const double f = p.f_top + (double)c * p.cw;
+      const double x = kDispersion * dm * (1.0 / (f * f) - inv_top) / ts;
+      const double d = floor(x + 0.5);
+      if (!(d >= 0.0) || d > 2.0e9) return false;
+      r.delays[(size_t)j * p.nchans + c] = (int32_t)d;
+    }
+  }
+  return true;
+}
+
+struct TileChoice {
+  int G, T, Cc, stages;
+};
+
+int env_int(const char* name, int dflt) {
+  const char* s = getenv(name);
+  return (s && *s) ? atoi(s) : dflt;
+}
+
+// Delay spread of one trial block: d(c, last) - d(c, first); delays are non-decreasing in j.
+inline int block_spread(const dd_plan& p, const dd::RangePlan& r, int blk, int Dcta, int c) {
+  const int j0 = blk * Dcta;
+  const int j1 = std::min(r.ndm - 1, j0 + Dcta - 1);
+  return r.delays[(size_t)j1 * p.nchans + c] - r.delays[(size_t)j0 * p.nchans + c];
+}
+
+// Pick the tile shape of the tiled kernel for one range: more trials per CTA amortise the
+// L2 -> shared-memory fill of a channel row over more adds, but widen the staged window by the delay
+// spread of the block.  Cost model: staged bytes per add; constraint: >= 3 stages in 200 KB.
+void choose_tile(const dd_plan& p, dd::RangePlan& r) {
+  const int maxval = ((1 << p.in_bits) - 1) * r.decim;
+  if (maxval <= 4095) {  // at least 16 channels between flushes
+    r.NL = 8;
+    r.flush = std::min(256, 65535 / maxval);
+  } else {
+    r.NL = 4;
+    r.flush = 0;
+  }
+  static const int cand[][2] = {{16, 32}, {8, 64}, {4, 128}, {2, 256}, {1, 512}, {8, 32}, {4, 64}, {2, 128}, {1, 256}};
+  const size_t budget = 200 * 1024;
+  double best = 1e300;
+  TileChoice bc = {1, 256, 2, 2};
+  bool found = false;
+  for (auto& gt : cand) {
+    const int G = gt[0], T = gt[1], D = G * dd::kRD;
+    const int nblocks = (r.ndm + D - 1) / D;
+    int smax = 0;
+    double ssum = 0;
+    const int cstep = std::max(1, p.nchans / 64);
+    int nsamp = 0;
+    for (int b = 0; b < nblocks; ++b) {
+      smax = std::max(smax, block_spread(p, r, b, D, p.nchans - 1));
+      for (int c = 0; c < p.nchans; c += cstep, ++nsamp) ssum += block_spread(p, r, b, D, c);
+    }
+    const double smean = ssum / std::max(1, nsamp);
+    for (int Cc : {16, 8, 4, 2}) {
+      if (r.NL == 8 && Cc > r.flush) continue;
+      const size_t stage = (size_t)Cc * ((size_t)(T + smax) * 16 + (size_t)D * 4);
+      const int stages = (int)std::min<size_t>(4, budget / stage);
+      if (stages < (Cc >= 8 ? 3 : 2)) continue;
+      // bytes staged per add: row (T + mean spread) superwords + the offsets row, over T*NL*D adds
+      double cost = ((T + smean) * 16.0 + D * 4.0) / ((double)T * r.NL * D);
+      if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
+      if (Cc < 16) cost *= 1.0 + 0.05 * (16 / Cc - 1);  // shorter stages synchronise more often
+      if (cost < best) {
+        best = cost;
+        bc = {G, T, Cc, stages};
+        found = true;
+      }
+    }
+  }
+  r.tiled_ok = found ? 1 : 0;  // otherwise the delay spread of 4 trials exceeds shared memory: direct kernel
+  // tuning hook (measurements only): DD_TILE="G,T,Cc,stages"
+  if (const char* s = getenv("DD_TILE")) {
+    int g, t, cc, st;
+    if (sscanf(s, "%d,%d,%d,%d", &g, &t, &cc, &st) == 4 && (g * t == 256 || g * t == 512) && t % 32 == 0 &&
+        cc >= 2 && cc <= 32 && cc % 2 == 0 && st >= 2 && st <= 8 && (r.NL != 8 || cc <= r.flush)) {
+      bc = {g, t, cc, st};
+      r.tiled_ok = 1;
+    }
+  }
+  r.G = bc.G;
+  r.T = bc.T;
+  r.Cc = bc.Cc;
+  r.stages = bc.stages;
+  r.Dcta = r.G * dd::kRD;
+  r.nblocks = (r.ndm + r.Dcta - 1) / r.Dcta;
+  r.Cpad = (int)round_up(p.nchans, r.Cc);
+  if (r.NL == 8) r.flush = r.flush / r.Cc * r.Cc;
+  r.Smax = 0;
+  int64_t same = 0, total = 0;
+  for (int b = 0; b < r.nblocks; ++b) r.Smax = std::max(r.Smax, block_spread(p, r, b, r.Dcta, p.nchans - 1));
+  // fraction of neighbouring-trial transitions (inside a register block) that keep the delay
+  const int cstep = std::max(1, p.nchans / 128);
+  for (int j = 0; j + 1 < r.ndm; ++j) {
+    if ((j + 1) % dd::kRD == 0) continue;
+    for (int c = 0; c < p.nchans; c += cstep) {
+      same += r.delays[(size_t)j * p.nchans + c] == r.delays[(size_t)(j + 1) * p.nchans + c];
+      ++total;
+    }
+  }
+  r.reuse = total > 0 && (double)same / (double)total >= 0.25;
+  r.reuse = env_int("DD_REUSE", r.reuse) ? 1 : 0;
+  while (r.stages > 2 && dd::tiled_smem_bytes(r) > (size_t)227 * 1024) --r.stages;
+  r.H = round_up((r.nout + r.NL - 1) / r.NL, 16);
+  r.ntau = (r.H + r.T - 1) / r.T;
+  r.Wp = round_up(r.ntau * r.T + r.maxd, 4);
+  r.ws_bytes = (int64_t)p.nbeams * r.Cpad * r.Wp * dd::kSuperwordBytes;
+  r.smem_bytes = dd::tiled_smem_bytes(r);
+  if (r.smem_bytes > (size_t)227 * 1024) r.tiled_ok = 0;
+  if (!r.tiled_ok) r.ws_bytes = 0;
+}
+
+// Device tables of the tiled kernel: per trial block and channel the first delay (start of the staged
+// row), the spread (length of the staged row beyond T) and per trial the byte offset into the row.
+int upload_tables(const dd_plan& p, dd::RangePlan& r) {
+  const size_t nbc = (size_t)r.nblocks * r.Cpad;
+  std::vector<int32_t> dmin(nbc, 0), span(nbc, 0);
+  std::vector<uint32_t> meta(nbc * r.Dcta, 0);
+  for (int b = 0; b < r.nblocks; ++b) {
+    for (int c = 0; c < p.nchans; ++c) {
+      const int j0 = b * r.Dcta;
+      const int32_t d0 = r.delays[(size_t)j0 * p.nchans + c];
+      int32_t dl = d0;
+      for (int jj = 0; jj < r.Dcta; ++jj) {
+        const int j = std::min(r.ndm - 1, j0 + jj);  // trials past the end repeat the last one
+        const int32_t d = r.delays[(size_t)j * p.nchans + c];
+        dl = std::max(dl, d);
+        meta[((size_t)b * r.Cpad + c) * r.Dcta + jj] = (uint32_t)(d - d0) * dd::kSuperwordBytes;
+      }
+      dmin[(size_t)b * r.Cpad + c] = d0;
+      span[(size_t)b * r.Cpad + c] = dl - d0;
+    }
+  }
+  DD_CUDA(cudaMalloc(&r.d_meta, meta.size() * sizeof(uint32_t)));
+  DD_CUDA(cudaMalloc(&r.d_dmin, nbc * sizeof(int32_t)));
+  DD_CUDA(cudaMalloc(&r.d_span, nbc * sizeof(int32_t)));
+  DD_CUDA(cudaMemcpy(r.d_meta, meta.data(), meta.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_dmin, dmin.data(), nbc * sizeof(int32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_span, span.data(), nbc * sizeof(int32_t), cudaMemcpyHostToDevice));
+  return DD_OK;
+}
+
+int ensure_direct_tables(dd_plan* p, bool only_untiled) {
+  for (auto& r : p->ranges) {
+    if (r.d_delays || (only_untiled && r.tiled_ok)) continue;
+    DD_CUDA(cudaMalloc(&r.d_delays, r.delays.size() * sizeof(int32_t)));
+    DD_CUDA(cudaMemcpy(r.d_delays, r.delays.data(), r.delays.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  }
+  return DD_OK;
+}
+
+int ensure_workspace(dd_plan* p) {
+  if (p->ws || p->ws_bytes == 0) return DD_OK;
+  cudaError_t e = cudaMalloc(&p->ws, (size_t)p->ws_bytes);
+  if (e != cudaSuccess) {
+    cuda_fail(e, "cudaMalloc(workspace)");
+    p->ws = nullptr;
+    return DD_ERR_NOMEM;
+  }
+  p->ws_owned = true;
+  return DD_OK;
+}
+
+inline bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+int dd_version(void) { return DD_VERSION; }
+
+const char* dd_strerror(int code) {
+  switch (code) {
+    case DD_OK: return "ok";
+    case DD_ERR_INVALID: return "invalid argument";
+    case DD_ERR_TOO_SHORT: return "input too short for the largest delay of a range";
+    case DD_ERR_OVERFLOW: return "channel sum does not fit 32 bits";
+    case DD_ERR_ALIGN: return "buffer not 16-byte aligned";
+    case DD_ERR_CUDA: return "CUDA error (see dd_last_cuda_error)";
+    case DD_ERR_NOMEM: return "out of memory or workspace too small";
+    default: return "unknown dd_status";
+  }
+}
+
+const char* dd_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
+  if (!cfg || !plan_out) return DD_ERR_INVALID;
+  *plan_out = nullptr;
+  if (cfg->nchans < 1 || !(cfg->chan_width_mhz < 0.0) || !(cfg->tsamp_s > 0.0) || cfg->nsamps < 1 ||
+      cfg->nbeams < 1 || !(cfg->in_bits == 8 || cfg->in_bits == 16) || cfg->nranges < 1 || !cfg->ranges ||
+      !(cfg->f_top_mhz > 0.0) || cfg->nchans > 65535 || cfg->nbeams > 65535)
+    return DD_ERR_INVALID;
+  if (!(cfg->f_top_mhz + (double)(cfg->nchans - 1) * cfg->chan_width_mhz > 0.0)) return DD_ERR_INVALID;
+  for (int r = 0; r < cfg->nranges; ++r) {
+    const dd_range_t& q = cfg->ranges[r];
+    if (!(q.decim == 1 || q.decim == 2 || q.decim == 4 || q.decim == 8) || q.ndm < 1 || q.ndm > 65535 ||
+        !(q.dm_lo >= 0.0) || !(q.dm_step >= 0.0))
+      return DD_ERR_INVALID;
+    const double bound = (double)cfg->nchans * (double)((1 << cfg->in_bits) - 1) * (double)q.decim;
+    if (bound >= 4294967296.0) return DD_ERR_OVERFLOW;
+  }
+  dd_plan* p = new (std::nothrow) dd_plan();
+  if (!p) return DD_ERR_NOMEM;
+  int rc = DD_OK;
+  try {
+    p->f_top = cfg->f_top_mhz;
+    p->cw = cfg->chan_width_mhz;
+    p->tsamp = cfg->tsamp_s;
+    p->nchans = cfg->nchans;
+    p->nbeams = cfg->nbeams;
+    p->in_bits = cfg->in_bits;
+    p->nsamps = cfg->nsamps;
+    p->ranges.resize(cfg->nranges);
+    int64_t offset = 0;
+    for (int i = 0; i < cfg->nranges && rc == DD_OK; ++i) {
+      dd::RangePlan& r = p->ranges[i];
+      r.dm_lo = cfg->ranges[i].dm_lo;
+      r.dm_step = cfg->ranges[i].dm_step;
+      r.ndm = cfg->ranges[i].ndm;
+      r.decim = cfg->ranges[i].decim;
+      r.ns = p->nsamps / r.decim;
+      if (!build_delays(*p, r)) { rc = DD_ERR_TOO_SHORT; break; }
+      r.maxd = r.delays[(size_t)(r.ndm - 1) * p->nchans + (p->nchans - 1)];
+      r.nout = r.ns - r.maxd;
+      if (r.nout < 1) { rc = DD_ERR_TOO_SHORT; break; }
+      r.pitch = round_up(r.nout, 32);
+      r.offset = offset;
+      offset += (int64_t)r.ndm * r.pitch;
+      p->dm_samples += (int64_t)p->nbeams * r.ndm * r.nout;
+      choose_tile(*p, r);
+      r.ws_offset = p->ws_bytes;
+      p->ws_bytes += round_up(r.ws_bytes, 256);
+    }
+    if (rc == DD_OK) {
+      p->beam_stride = offset;
+      p->out_elems = offset * p->nbeams;
+      p->adds = p->dm_samples * p->nchans;
+    }
+  } catch (const std::bad_alloc&) {
+    rc = DD_ERR_NOMEM;
+  }
+  if (rc != DD_OK) {
+    delete p;
+    return rc;
+  }
+  cudaError_t e = cudaGetDevice(&p->device);
+  if (e != cudaSuccess) {
+    delete p;
+    return cuda_fail(e, "cudaGetDevice");
+  }
+  e = dd::configure_kernels(p);
+  if (e != cudaSuccess) {
+    delete p;
+    return cuda_fail(e, "cudaFuncSetAttribute");
+  }
+  for (auto& r : p->ranges) {
+    rc = r.tiled_ok ? upload_tables(*p, r) : DD_OK;
+    if (rc != DD_OK) break;
+  }
+  if (rc == DD_OK) rc = ensure_direct_tables(p, /*only_untiled=*/true);
+  if (rc == DD_OK) rc = ensure_workspace(p);
+  if (rc == DD_OK) {
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) rc = cuda_fail(e, "cudaDeviceSynchronize");
+  }
+  if (rc != DD_OK) {
+    dd_plan_destroy(p);
+    return rc;
+  }
+  *plan_out = p;
+  return DD_OK;
+}
+
+int dd_plan_destroy(dd_plan_t* p) {
+  if (!p) return DD_OK;
+  for (auto& r : p->ranges) {
+    if (r.d_meta) cudaFree(r.d_meta);
+    if (r.d_dmin) cudaFree(r.d_dmin);
+    if (r.d_span) cudaFree(r.d_span);
+    if (r.d_delays) cudaFree(r.d_delays);
+  }
+  if (p->ws && p->ws_owned) cudaFree(p->ws);
+  if (p->h_in_dev) cudaFree(p->h_in_dev);
+  if (p->h_out_dev) cudaFree(p->h_out_dev);
+  delete p;
+  return DD_OK;
+}
+
+int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* cuda_stream) {
+  if (!plan || !in_dev || !out_dev) return DD_ERR_INVALID;
+  if (!aligned16(in_dev) || !aligned16(out_dev)) return DD_ERR_ALIGN;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
+  // a2 for every range first, then a3+a4: the dedispersion kernels of consecutive ranges follow each
+  // other on the stream without a pack kernel draining the machine in between.
+  for (const auto& r : plan->ranges) {
+    if (all_direct || !r.tiled_ok) continue;
+    if (!plan->ws) return DD_ERR_NOMEM;
+    DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
+  }
+  for (const auto& r : plan->ranges) {
+    if (all_direct || !r.tiled_ok) {
+      if (!r.d_delays) return DD_ERR_INVALID;  // uploaded by dd_plan_create / dd_plan_set_kernel
+      DD_CUDA(dd::launch_direct(plan, r, in_dev, out_dev, stream));
+    } else {
+      DD_CUDA(dd::launch_tiled(plan, r, out_dev, stream));
+    }
+  }
+  return DD_OK;
+}
+
+int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
+  if (!plan || !in_host || !out_host) return DD_ERR_INVALID;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const size_t in_bytes = (size_t)plan->nbeams * plan->nchans * plan->nsamps * (plan->in_bits / 8);
+  const size_t out_bytes = (size_t)plan->out_elems * sizeof(float);
+  if (!plan->h_in_dev) {
+    if (cudaMalloc(&plan->h_in_dev, in_bytes) != cudaSuccess) { plan->h_in_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
+  }
+  if (!plan->h_out_dev) {
+    if (cudaMalloc(&plan->h_out_dev, out_bytes) != cudaSuccess) { plan->h_out_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
+  }
+  DD_CUDA(cudaMemcpyAsync(plan->h_in_dev, in_host, in_bytes, cudaMemcpyHostToDevice, stream));
+  int rc = dd_execute(plan, plan->h_in_dev, plan->h_out_dev, cuda_stream);
+  if (rc != DD_OK) return rc;
+  DD_CUDA(cudaMemcpyAsync(out_host, plan->h_out_dev, out_bytes, cudaMemcpyDeviceToHost, stream));
+  DD_CUDA(cudaStreamSynchronize(stream));
+  return DD_OK;
+}
+
+int dd_plan_out_elems(const dd_plan_t* p, int64_t* total_floats) {
+  if (!p || !total_floats) return DD_ERR_INVALID;
+  *total_floats = p->out_elems;
+  return DD_OK;
+}
+
+int dd_plan_beam_stride(const dd_plan_t* p, int64_t* floats) {
+  if (!p || !floats) return DD_ERR_INVALID;
+  *floats = p->beam_stride;
+  return DD_OK;
+}
+
+int dd_plan_range_info(const dd_plan_t* p, int32_t r, int64_t* ns_r, int64_t* maxd_r, int64_t* nout_r,
+                       int64_t* pitch_floats, int64_t* offset_floats) {
+  if (!p || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  if (ns_r) *ns_r = q.ns;
+  if (maxd_r) *maxd_r = q.maxd;
+  if (nout_r) *nout_r = q.nout;
+  if (pitch_floats) *pitch_floats = q.pitch;
+  if (offset_floats) *offset_floats = q.offset;
+  return DD_OK;
+}
+
+int dd_plan_get_delays(const dd_plan_t* p, int32_t r, int32_t* host_buf) {
+  if (!p || !host_buf || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  memcpy(host_buf, q.delays.data(), q.delays.size() * sizeof(int32_t));
+  return DD_OK;
+}
+
+int dd_plan_work(const dd_plan_t* p, int64_t* dm_samples, int64_t* adds) {
+  if (!p) return DD_ERR_INVALID;
+  if (dm_samples) *dm_samples = p->dm_samples;
+  if (adds) *adds = p->adds;
+  return DD_OK;
+}
+
+int dd_plan_launches(const dd_plan_t* p, int32_t* n) {
+  if (!p || !n) return DD_ERR_INVALID;
+  int k = 0;
+  for (const auto& r : p->ranges) k += (p->variant == DD_KERNEL_DIRECT || !r.tiled_ok) ? 1 : 2;
+  *n = k;
+  return DD_OK;
+}
+
+int dd_plan_workspace_bytes(const dd_plan_t* p, int64_t* bytes) {
+  if (!p || !bytes) return DD_ERR_INVALID;
+  *bytes = p->ws_bytes;
+  return DD_OK;
+}
+
+int dd_plan_set_workspace(dd_plan_t* p, void* dev, int64_t bytes) {
+  if (!p) return DD_ERR_INVALID;
+  if (dev) {
+    if (!aligned16(dev)) return DD_ERR_ALIGN;
+    if (bytes < p->ws_bytes) return DD_ERR_NOMEM;
+    if (p->ws && p->ws_owned) cudaFree(p->ws);
+    p->ws = dev;
+    p->ws_owned = false;
+    return DD_OK;
+  }
+  if (p->ws && !p->ws_owned) p->ws = nullptr;
+  return ensure_workspace(p);
+}
+
+int dd_plan_set_kernel(dd_plan_t* p, int32_t variant) {
+  if (!p) return DD_ERR_INVALID;
+  if (variant != DD_KERNEL_AUTO && variant != DD_KERNEL_DIRECT && variant != DD_KERNEL_TILED) return DD_ERR_INVALID;
+  if (variant == DD_KERNEL_DIRECT) {
+    int rc = ensure_direct_tables(p, false);
+    if (rc != DD_OK) return rc;
+  }
+  p->variant = variant;
+  return DD_OK;
+}
+
+int dd_plan_tile_info(const dd_plan_t* p, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta, int32_t* lanes,
+                      int32_t* flush_chans, int32_t* reuse) {
+  if (!p || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  if (dm_per_cta) *dm_per_cta = q.Dcta;
+  if (words_per_cta) *words_per_cta = q.T;
+  if (lanes) *lanes = q.NL;
+  if (flush_chans) *flush_chans = q.flush;
+  if (reuse) *reuse = q.reuse;
+  return DD_OK;
+}
+
+}  // extern "C"

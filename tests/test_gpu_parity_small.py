@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, bit-exact.
+
+Sizes: small enough for the oracle to finish in seconds, large enough to span several time tiles,
+trial blocks and channel stages of the tiled kernel, with ragged tails in every dimension.
+"""
+import numpy as np
+import pytest
+
+from paper_2605_03531_b200 import workloads as W
+
+from _util import check_full, gpu_run, oracle_full
+
+pytestmark = pytest.mark.gpu
+
+DIRECT, TILED = 1, 2
+
+
+def _rng_filterbank(nbeams, nchans, nsamps, bits, seed):
+    rng = np.random.default_rng(seed)
+    return rng.integers(0, 2 ** bits, size=(nbeams, nchans, nsamps), dtype=np.uint8 if bits == 8 else np.uint16)
+
+
+@pytest.mark.parametrize("variant", [DIRECT, TILED])
+def test_cfg1_tiny_full(variant):
+    w = W.CONFIGS[1]
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, variant)
+    check_full(w, x, plan, flat)
+    # the injected pulse is recovered at DM 50 (PAPER.md:387-393 injection test)
+    out = plan.view_range(flat, 0)
+    j, t = np.unravel_index(np.argmax(out), out.shape)
+    assert abs(j - 50) <= 1 and 1024 <= t <= 1028
+
+
+@pytest.mark.parametrize("variant", [DIRECT, TILED])
+def test_cfg3_shaped_multirange_decimation(variant):
+    """config-3 shape scaled down: 3 ranges with x1/x2/x4 decimation, zeroed channels, uint8."""
+    w = W.scaled(W.CONFIGS[3], nchans=272, nsamps=2 ** 15 + 3,
+                 ranges=[W.DMRange(0.0, 0.1, 203, 1), W.DMRange(200.0, 0.2, 150, 2), W.DMRange(600.0, 0.5, 141, 4)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, variant)
+    check_full(w, x, plan, flat)
+    if variant == TILED:
+        assert plan.tile_info(0)["lanes"] == 8 and plan.tile_info(0)["reuse"] == 1
+
+
+@pytest.mark.parametrize("variant", [DIRECT, TILED])
+def test_cfg2_shaped_large_delay_steps(variant):
+    """config-2 shape scaled: delays change by several samples per trial (no reuse)."""
+    w = W.scaled(W.CONFIGS[2], nchans=200, nsamps=2 ** 15, ranges=[W.DMRange(0.0, 0.5, 301, 1)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, variant)
+    check_full(w, x, plan, flat)
+
+
+@pytest.mark.parametrize("variant", [DIRECT, TILED])
+def test_cfg4_shaped_uint16(variant):
+    """uint16 input, x1 and x8 ranges: sums exceed 2^24, result must be fl32(exact sum): 0 ulp."""
+    w = W.scaled(W.CONFIGS[4], nchans=520, nsamps=2 ** 16,
+                 ranges=[W.DMRange(0.0, 0.25, 130, 1), W.DMRange(1000.0, 1.0, 77, 8)])
+    x = W.generate(w)
+    assert x.dtype == np.uint16
+    want = oracle_full(w, x)
+    assert want[0][0].max() > 2 ** 24        # the inexact regime is exercised
+    plan, flat = gpu_run(w, x, variant)
+    check_full(w, x, plan, flat, want)
+    assert plan.tile_info(0)["lanes"] == 4
+
+
+def test_uint16_extreme_values_exact_rounding():
+    """All-65535 rows with a few odd values: sums near 2^32/8, every rounding case hit."""
+    rng = np.random.default_rng(4)
+    x = np.full((1, 300, 4096), 65535, dtype=np.uint16)
+    x[0, ::7, :] -= rng.integers(0, 3, size=x[0, ::7, :].shape, dtype=np.uint16)
+    w = W.Workload("u16_extreme", 500.0, -200.0 / 300, 300, 1.31072e-3, 4096, 1, 16,
+                   (W.DMRange(0.0, 3.0, 9, 1), W.DMRange(30.0, 5.0, 5, 8)), 1, 0, 0)
+    for variant in (DIRECT, TILED):
+        plan, flat = gpu_run(w, x, variant)
+        check_full(w, x, plan, flat)
+
+
+@pytest.mark.parametrize("variant", [DIRECT, TILED])
+def test_cfg5_shaped_multibeam(variant):
+    w = W.scaled(W.CONFIGS[5], nchans=144, nsamps=2 ** 14, nbeams=3, ranges=[W.DMRange(0.0, 0.5, 90, 1)])
+    x = W.generate(w)
+    assert not np.array_equal(x[0], x[1])
+    plan, flat = gpu_run(w, x, variant)
+    check_full(w, x, plan, flat)
+
+
+@pytest.mark.parametrize("decim", [1, 2, 4, 8])
+@pytest.mark.parametrize("bits", [8, 16])
+def test_all_decimations_saturated_input(decim, bits):
+    """Saturated samples (255 / 65535 everywhere but a few): the packed 16-bit lanes reach their bound
+    exactly at the flush interval; any missing flush or lane carry shows up."""
+    nch, ns = 530, 20000 + decim - 1
+    x = np.full((1, nch, ns), 2 ** bits - 1, dtype=np.uint8 if bits == 8 else np.uint16)
+    x[0, 3, 100:200] = 0
+    w = W.Workload("sat", 750.0, -200.0 / nch, nch, 1.31072e-3, ns, 1, bits, (W.DMRange(0.0, 1.0, 21, decim),), 1, 0, 0)
+    plan, flat = gpu_run(w, x, TILED)
+    check_full(w, x, plan, flat)
+    out = plan.view_range(flat, 0)
+    assert out.max() == np.float32(nch * decim * (2 ** bits - 1))
+
+
+@pytest.mark.parametrize("nchans,nsamps,ndm,step", [
+    (1, 700, 5, 10.0),       # single channel: identity (P8)
+    (2, 64, 1, 0.0),         # one trial, DM 0
+    (3, 5000, 7, 2.0),       # odd channel count: zero-padded channel rows
+    (33, 3000, 37, 0.7),     # trial count not a multiple of the register block or the CTA block
+    (64, 1211, 9, 3.0),
+])
+def test_edge_shapes(nchans, nsamps, ndm, step):
+    x = _rng_filterbank(1, nchans, nsamps, 8, 100 + nchans)
+    w = W.Workload("edge", 500.0, -200.0 / nchans, nchans, 1.024e-3, nsamps, 1, 8, (W.DMRange(0.0, step, ndm, 1),), 1, 0, 0)
+    for variant in (DIRECT, TILED):
+        plan, flat = gpu_run(w, x, variant)
+        check_full(w, x, plan, flat)
+
+
+def test_minimum_valid_span_nout_1():
+    """nout = 1: the largest delay leaves a single valid sample."""
+    nch = 16
+    import oracle
+    tab = oracle.delay_table(500.0, -200.0 / nch, nch, 1.024e-3, 1, 0.0, 1.0, 11)
+    ns = int(tab.max()) + 1
+    x = _rng_filterbank(1, nch, ns, 8, 5)
+    w = W.Workload("nout1", 500.0, -200.0 / nch, nch, 1.024e-3, ns, 1, 8, (W.DMRange(0.0, 1.0, 11, 1),), 1, 0, 0)
+    for variant in (DIRECT, TILED):
+        plan, flat = gpu_run(w, x, variant)
+        assert plan.range_info(0)["nout"] == 1
+        check_full(w, x, plan, flat)
+
+
+def test_too_short_and_overflow_are_rejected():
+    from paper_2605_03531_b200 import binding as B
+    with pytest.raises(B.DDError) as e:
+        B.Plan(500.0, -200.0 / 16, 16, 1.024e-3, 100, [(0.0, 1.0, 11, 1)])
+    assert e.value.code == B.DD_ERR_TOO_SHORT
+    with pytest.raises(B.DDError) as e:
+        B.Plan(500.0, -0.001, 65535, 1.024e-3, 100000, [(0.0, 0.0, 1, 8)], in_bits=16)
+    assert e.value.code == B.DD_ERR_OVERFLOW
+
+
+def test_delay_table_matches_oracle_all_configs():
+    """dd_plan_get_delays == oracle table for the five BASELINE configs (plan builder parity)."""
+    import oracle
+    from paper_2605_03531_b200 import binding as B
+    for k, w in W.CONFIGS.items():
+        if k == 5:
+            w = W.scaled(w, nbeams=1)
+        plan = B.Plan.from_workload(w)
+        for r, rg in enumerate(w.ranges):
+            want = oracle.delay_table(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, rg.decim, rg.dm_lo, rg.dm_step, rg.ndm)
+            got = plan.get_delays(r)
+            assert np.array_equal(got.astype(np.int64), want), (k, r)
+        plan.destroy()
+
+
+def test_host_path_and_caller_workspace():
+    import torch
+    w = W.scaled(W.CONFIGS[3], nchans=96, nsamps=2 ** 14,
+                 ranges=[W.DMRange(0.0, 0.1, 40, 1), W.DMRange(200.0, 0.2, 24, 2)])
+    x = W.generate(w)
+    want = oracle_full(w, x)
+    plan, flat = gpu_run(w, x, TILED, host_path=True)
+    check_full(w, x, plan, flat, want, check_pad=False)   # the host path copies whole rows back
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device="cuda")
+    plan.set_workspace(ws)
+    xin = torch.from_numpy(x).cuda()
+    out = torch.full((plan.out_elems(),), -1.0, dtype=torch.float32, device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        plan.execute(xin, out, s)
+    s.synchronize()
+    check_full(w, x, plan, out.cpu().numpy(), want)
+    assert plan.launches() == 4
