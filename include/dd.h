@@ -143,6 +143,18 @@ int dd_plan_set_kernel(dd_plan_t* plan, int32_t variant);
 int dd_plan_tile_info(const dd_plan_t* plan, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta,
                       int32_t* lanes, int32_t* flush_chans, int32_t* reuse);
 
+/* ---- per-kernel timing (measurement hook) ------------------------------------------------------- */
+
+/* Record a CUDA event before and after every kernel launch of the next `max_executes` calls of
+ * dd_execute (slot = call index modulo max_executes).  max_executes = 0 switches it off and frees the
+ * events.  The events are recorded on the caller's stream; nothing synchronises. */
+int dd_plan_set_profiling(dd_plan_t* plan, int32_t max_executes);
+/* After the caller has synchronised the stream: device time of each launch of execute slot `slot`, in
+ * launch order.  ms[i] = milliseconds, kind[i] = 0 pack/decimate, 1 tiled dedispersion, 2 direct
+ * dedispersion, range[i] = range index.  Arrays hold `cap` entries; *n = launches written. */
+int dd_plan_kernel_times(const dd_plan_t* plan, int32_t slot, int32_t cap, float* ms, int32_t* kind,
+                         int32_t* range, int32_t* n);
+
 /* ---- errors ---------------------------------------------------------------------------------- */
 const char* dd_strerror(int code);       /* static string for a dd_status */
 const char* dd_last_cuda_error(void);    /* text of the last CUDA failure seen by this thread ("" if none) */

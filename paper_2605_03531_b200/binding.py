@@ -21,7 +21,7 @@ SYMBOLS = [
     "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
-    "dd_strerror", "dd_last_cuda_error", "dd_version",
+    "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
 ]
 
 
@@ -72,6 +72,8 @@ def _load():
         lib.dd_plan_set_workspace.argtypes = [vp, vp, i64]
         lib.dd_plan_set_kernel.argtypes = [vp, i32]
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
+        lib.dd_plan_set_profiling.argtypes = [vp, i32]
+        lib.dd_plan_kernel_times.argtypes = [vp, i32, i32, P(ctypes.c_float), P(i32), P(i32), P(i32)]
         lib.dd_strerror.argtypes = [ctypes.c_int]
         lib.dd_strerror.restype = ctypes.c_char_p
         lib.dd_last_cuda_error.restype = ctypes.c_char_p
@@ -213,6 +215,19 @@ class Plan:
         vals = [ctypes.c_int32() for _ in range(5)]
         _chk(_load().dd_plan_tile_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_tile_info")
         return {k: v.value for k, v in zip(["dm_per_cta", "words_per_cta", "lanes", "flush_chans", "reuse"], vals)}
+
+    def set_profiling(self, max_executes: int) -> None:
+        _chk(_load().dd_plan_set_profiling(self._h, int(max_executes)), "dd_plan_set_profiling")
+
+    def kernel_times(self, slot: int) -> List[dict]:
+        cap = 2 * self.nranges
+        ms = (ctypes.c_float * cap)()
+        kind = (ctypes.c_int32 * cap)()
+        rng = (ctypes.c_int32 * cap)()
+        n = ctypes.c_int32()
+        _chk(_load().dd_plan_kernel_times(self._h, slot, cap, ms, kind, rng, ctypes.byref(n)), "dd_plan_kernel_times")
+        names = {0: "pack", 1: "tiled", 2: "direct"}
+        return [{"ms": float(ms[i]), "kind": names[kind[i]], "range": int(rng[i])} for i in range(n.value)]
 
     # -- convenience for callers holding torch tensors
     def view_range(self, out, r: int, beam: int = 0):

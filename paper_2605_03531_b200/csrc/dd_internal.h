@@ -68,6 +68,11 @@ struct dd_plan {
   int64_t ws_bytes = 0;
   void* ws = nullptr;
   bool ws_owned = false;
+  // per-kernel timing hook (dd_plan_set_profiling): events[slot][2*launch + {0,1}]
+  int prof_slots = 0;
+  mutable long long prof_calls = 0;
+  std::vector<cudaEvent_t> prof_events;
+  mutable std::vector<int> prof_kind, prof_range, prof_count;  // per slot*max_launches
   // host-path staging
   void* h_in_dev = nullptr;
   float* h_out_dev = nullptr;

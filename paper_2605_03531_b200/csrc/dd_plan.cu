@@ -326,6 +326,7 @@ int dd_plan_destroy(dd_plan_t* p) {
     if (r.d_span) cudaFree(r.d_span);
     if (r.d_delays) cudaFree(r.d_delays);
   }
+  for (cudaEvent_t e : p->prof_events) cudaEventDestroy(e);
   if (p->ws && p->ws_owned) cudaFree(p->ws);
   if (p->h_in_dev) cudaFree(p->h_in_dev);
   if (p->h_out_dev) cudaFree(p->h_out_dev);
@@ -338,19 +339,41 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
   if (!aligned16(in_dev) || !aligned16(out_dev)) return DD_ERR_ALIGN;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
+  // optional per-launch events (measurement hook)
+  const int max_launch = 2 * (int)plan->ranges.size();
+  const int slot = plan->prof_slots > 0 ? (int)(plan->prof_calls++ % plan->prof_slots) : -1;
+  int nl = 0;
+  auto ev_before = [&](int kind, int range) -> cudaError_t {
+    if (slot < 0) return cudaSuccess;
+    plan->prof_kind[(size_t)slot * max_launch + nl] = kind;
+    plan->prof_range[(size_t)slot * max_launch + nl] = range;
+    return cudaEventRecord(plan->prof_events[((size_t)slot * max_launch + nl) * 2], stream);
+  };
+  auto ev_after = [&]() -> cudaError_t {
+    if (slot < 0) return cudaSuccess;
+    cudaError_t e = cudaEventRecord(plan->prof_events[((size_t)slot * max_launch + nl) * 2 + 1], stream);
+    plan->prof_count[slot] = ++nl;
+    return e;
+  };
   // a2 for every range first, then a3+a4: the dedispersion kernels of consecutive ranges follow each
   // other on the stream without a pack kernel draining the machine in between.
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) continue;
     if (!plan->ws) return DD_ERR_NOMEM;
+    DD_CUDA(ev_before(0, (int)(&r - plan->ranges.data())));
     DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
+    DD_CUDA(ev_after());
   }
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) {
       if (!r.d_delays) return DD_ERR_INVALID;  // uploaded by dd_plan_create / dd_plan_set_kernel
+      DD_CUDA(ev_before(2, (int)(&r - plan->ranges.data())));
       DD_CUDA(dd::launch_direct(plan, r, in_dev, out_dev, stream));
+      DD_CUDA(ev_after());
     } else {
+      DD_CUDA(ev_before(1, (int)(&r - plan->ranges.data())));
       DD_CUDA(dd::launch_tiled(plan, r, out_dev, stream));
+      DD_CUDA(ev_after());
     }
   }
   return DD_OK;
@@ -449,6 +472,45 @@ int dd_plan_set_kernel(dd_plan_t* p, int32_t variant) {
     if (rc != DD_OK) return rc;
   }
   p->variant = variant;
+  return DD_OK;
+}
+
+int dd_plan_set_profiling(dd_plan_t* p, int32_t max_executes) {
+  if (!p || max_executes < 0 || max_executes > 4096) return DD_ERR_INVALID;
+  for (cudaEvent_t e : p->prof_events) cudaEventDestroy(e);
+  p->prof_events.clear();
+  p->prof_slots = 0;
+  p->prof_calls = 0;
+  const size_t max_launch = 2 * p->ranges.size();
+  try {
+    p->prof_kind.assign(max_launch * max_executes, 0);
+    p->prof_range.assign(max_launch * max_executes, 0);
+    p->prof_count.assign(max_executes, 0);
+    p->prof_events.reserve(max_launch * max_executes * 2);
+  } catch (const std::bad_alloc&) {
+    return DD_ERR_NOMEM;
+  }
+  for (size_t i = 0; i < max_launch * max_executes * 2; ++i) {
+    cudaEvent_t e;
+    DD_CUDA(cudaEventCreate(&e));
+    p->prof_events.push_back(e);
+  }
+  p->prof_slots = max_executes;
+  return DD_OK;
+}
+
+int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* ms, int32_t* kind, int32_t* range,
+                         int32_t* n) {
+  if (!p || !ms || !n || slot < 0 || slot >= p->prof_slots || cap < 0) return DD_ERR_INVALID;
+  const size_t max_launch = 2 * p->ranges.size();
+  const int cnt = std::min<int>(cap, p->prof_count[slot]);
+  for (int i = 0; i < cnt; ++i) {
+    const size_t k = (size_t)slot * max_launch + i;
+    DD_CUDA(cudaEventElapsedTime(&ms[i], p->prof_events[2 * k], p->prof_events[2 * k + 1]));
+    if (kind) kind[i] = p->prof_kind[k];
+    if (range) range[i] = p->prof_range[k];
+  }
+  *n = cnt;
   return DD_OK;
 }
 
