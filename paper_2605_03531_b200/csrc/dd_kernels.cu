@@ -197,6 +197,26 @@ __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4
   acc.w = acc.w + a.w + b.w;
 }
 
+// Shared-memory superword loads of the inner loop, written in PTX so that the conditional reload
+// overwrites the four registers IN PLACE (the C++ form made ptxas copy them on every trial).
+__device__ __forceinline__ void lds_first(uint4& w, uint32_t base, uint32_t off) {
+  asm volatile("{\n .reg .u32 a;\n add.u32 a, %4, %5;\n ld.shared.v4.u32 {%0,%1,%2,%3}, [a];\n}"
+               : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
+               : "r"(base), "r"(off));
+}
+template <bool REUSE>
+__device__ __forceinline__ void lds_if_changed(uint4& w, uint32_t base, uint32_t off, uint32_t prev) {
+  if constexpr (REUSE) {
+    asm volatile(
+        "{\n .reg .pred p;\n .reg .u32 a;\n setp.ne.u32 p, %5, %6;\n add.u32 a, %4, %5;\n"
+        " @p ld.shared.v4.u32 {%0,%1,%2,%3}, [a];\n}"
+        : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w)
+        : "r"(base), "r"(off), "r"(prev));
+  } else {
+    lds_first(w, base, off);
+  }
+}
+
 template <int NL, bool REUSE, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParams p) {
   extern __shared__ __align__(128) unsigned char smem[];
@@ -225,36 +245,53 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   }
   __syncthreads();
 
-  // ---------------- producer role (warp 0, in addition to its consumer work) ------------------------
-  // One bulk copy per channel row + one for the offsets of the chunk; chunk `it` lands in stage
-  // it % nstages and signals full[stage] with its byte count.
+  // ---------------- producer role, rotated over the warps ---------------------------------------------
+  // Chunk k (channels k*Cc .. k*Cc+Cc-1) is issued by warp k % nwarps: one bulk copy per channel row plus
+  // one for the offsets, landing in stage k % nstages and signalling full[stage] with the byte count.
+  // A warp issues chunk k when it starts iteration k - ahead (ahead = nstages - 2): the stage it refills
+  // was consumed two iterations ago, so the wait on its empty barrier is normally already satisfied.
+  // Row start and length of the warp's NEXT chunk are fetched one turn early (pf_d0 / pf_bytes).
   const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T;
   const long long tab = (long long)blk * p.Cpad;
-  auto produce = [&](int it) {
-    const int lane = tid;  // warp 0 only
-    const int s = it % nstages;
-    if (it >= nstages) mbar_wait(bar_base + 8u * (nstages + s), ((uint32_t)(it / nstages) & 1u) ^ 1u);
+  const int lane = tid & 31;
+  const int warp = tid >> 5;
+  constexpr int kWarps = NT / 32;
+  const int ahead = nstages - 2;
+  int pf_d0 = 0;
+  uint32_t pf_bytes = 0;
+  auto prefetch = [&](int k) {
+    pf_bytes = 0;
+    if (k < nchunks && lane < p.Cc) {
+      const int c = k * p.Cc + lane;
+      pf_d0 = __ldg(p.dmin + tab + c);
+      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
+    }
+  };
+  auto produce = [&](int k) {
+    const int s = k % nstages;
+    if (k >= nstages) mbar_wait(bar_base + 8u * (nstages + s), ((uint32_t)(k / nstages) & 1u) ^ 1u);
     const uint32_t sbase = smem_u32(smem + kBarRegion + (size_t)s * stage_bytes);
     const uint32_t full = bar_base + 8u * s;
-    const int c = it * p.Cc + lane;
-    uint32_t bytes = 0;
-    int d0 = 0;
-    if (lane < p.Cc) {
-      d0 = __ldg(p.dmin + tab + c);
-      bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
-    }
-    uint32_t total = bytes;
+    uint32_t total = pf_bytes;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
     if (lane == 0) {
       mbar_arrive_expect_tx(full, total + meta_bytes);
-      bulk_copy_g2s(sbase + data_bytes, p.meta + (tab + (long long)it * p.Cc) * p.Dcta, meta_bytes, full);
+      bulk_copy_g2s(sbase + data_bytes, p.meta + (tab + (long long)k * p.Cc) * p.Dcta, meta_bytes, full);
     }
     __syncwarp();
-    if (lane < p.Cc) bulk_copy_g2s(sbase + lane * row_bytes, Pbeam + (long long)c * p.Wp + d0, bytes, full);
+    if (lane < p.Cc)
+      bulk_copy_g2s(sbase + lane * row_bytes, Pbeam + (long long)(k * p.Cc + lane) * p.Wp + pf_d0, pf_bytes, full);
   };
-  if (tid < 32) {
-    for (int it = 0; it < nstages - 1 && it < nchunks; ++it) produce(it);
+  // prologue: chunks 0 .. ahead-1
+  for (int k = warp; k < ahead && k < nchunks; k += kWarps) {
+    prefetch(k);
+    produce(k);
+  }
+  {  // first chunk this warp issues inside the loop
+    int k = warp;
+    while (k < ahead) k += kWarps;
+    prefetch(k);
   }
 
   // ---------------- consumers: kRD trials x one superword (NL time lanes) per thread --------------
@@ -276,8 +313,13 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   for (int it = 0; it < nchunks; ++it) {
     const int s = it % nstages;
     const uint32_t ph = (uint32_t)(it / nstages) & 1u;
-    // refill the stage freed one iteration ago while this one is consumed
-    if (tid < 32 && it + nstages - 1 < nchunks) produce(it + nstages - 1);
+    {  // producer turn: chunk it + ahead belongs to warp (it + ahead) % kWarps
+      const int k = it + ahead;
+      if (k < nchunks && (k % kWarps) == warp) {
+        produce(k);
+        prefetch(k + kWarps);
+      }
+    }
     mbar_wait(bar_base + 8u * s, ph);
     const unsigned char* sdata = smem + kBarRegion + (size_t)s * stage_bytes + thread_off;
     const unsigned char* smeta = smem + kBarRegion + (size_t)s * stage_bytes + data_bytes + group_off;
@@ -287,17 +329,19 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
       const uint4 ob = *reinterpret_cast<const uint4*>(smeta + (uint32_t)(cc + 1) * meta_row);
       const unsigned char* ra = sdata + (uint32_t)cc * row_bytes;
       const unsigned char* rb = ra + row_bytes;
-      uint4 wa = *reinterpret_cast<const uint4*>(ra + oa.x);
-      uint4 wb = *reinterpret_cast<const uint4*>(rb + ob.x);
+      const uint32_t aa = smem_u32(ra), ab = smem_u32(rb);
+      uint4 wa, wb;
+      lds_first(wa, aa, oa.x);
+      lds_first(wb, ab, ob.x);
       add_pair(acc[0], wa, wb);
-      if (!REUSE || oa.y != oa.x) wa = *reinterpret_cast<const uint4*>(ra + oa.y);
-      if (!REUSE || ob.y != ob.x) wb = *reinterpret_cast<const uint4*>(rb + ob.y);
+      lds_if_changed<REUSE>(wa, aa, oa.y, oa.x);
+      lds_if_changed<REUSE>(wb, ab, ob.y, ob.x);
       add_pair(acc[1], wa, wb);
-      if (!REUSE || oa.z != oa.y) wa = *reinterpret_cast<const uint4*>(ra + oa.z);
-      if (!REUSE || ob.z != ob.y) wb = *reinterpret_cast<const uint4*>(rb + ob.z);
+      lds_if_changed<REUSE>(wa, aa, oa.z, oa.y);
+      lds_if_changed<REUSE>(wb, ab, ob.z, ob.y);
       add_pair(acc[2], wa, wb);
-      if (!REUSE || oa.w != oa.z) wa = *reinterpret_cast<const uint4*>(ra + oa.w);
-      if (!REUSE || ob.w != ob.z) wb = *reinterpret_cast<const uint4*>(rb + ob.w);
+      lds_if_changed<REUSE>(wa, aa, oa.w, oa.z);
+      lds_if_changed<REUSE>(wb, ab, ob.w, ob.z);
       add_pair(acc[3], wa, wb);
     }
     __syncwarp();

@@ -101,7 +101,7 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
     for (int Cc : {16, 8, 4, 2}) {
       if (r.NL == 8 && Cc > r.flush) continue;
       const size_t stage = (size_t)Cc * ((size_t)(T + smax) * 16 + (size_t)D * 4);
-      const int stages = (int)std::min<size_t>(4, budget / stage);
+      const int stages = (int)std::min<size_t>(6, budget / stage);
       if (stages < (Cc >= 8 ? 3 : 2)) continue;
       // bytes staged per add: row (T + mean spread) superwords + the offsets row, over T*NL*D adds
       double cost = ((T + smean) * 16.0 + D * 4.0) / ((double)T * r.NL * D);
