@@ -1,0 +1,94 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (tiled kernel,
+tile shape chosen by the plan).  The oracle cannot produce 1e9 outputs in test time, so per config:
+
+  * sampled trials (first, second, middle, last two, three seeded random ones per range; for the
+    32-beam config on beams 0, 13 and 31) are computed by the oracle over the FULL valid span and
+    compared bit for bit;
+  * a property that holds at any size covers EVERY trial of every beam: the sum over time of row j,
+        sum_t S[j][t] = sum_c ( Y[c][d(c,j) + nout] - Y[c][d(c,j)] ),   Y = prefix sum of y over time,
+    evaluated in exact integer arithmetic from the oracle's decimated input and delay table and compared
+    with the float64 sum of the GPU row (exact for the uint8 configs: every term < 2^24, totals < 2^53;
+    1e-7 relative for the uint16 config whose outputs are rounded once);
+  * DM = 0 (trial 0 of range 0) equals the plain channel sum.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_03531_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _sample_trials(ndm, seed):
+    rng = np.random.default_rng(seed)
+    base = {0, 1, ndm // 2, ndm - 2, ndm - 1}
+    base |= set(int(v) for v in rng.integers(0, ndm, size=3))
+    return np.array(sorted(v for v in base if 0 <= v < ndm), dtype=np.int32)
+
+
+def _run_full(key, beams_to_check):
+    import torch
+    from paper_2605_03531_b200 import binding as B
+
+    w = W.CONFIGS[key]
+    x = W.generate(w)
+    plan = B.Plan.from_workload(w)
+    xin = torch.from_numpy(x.view(np.int16) if x.dtype == np.uint16 else x).cuda()
+    out = torch.full((plan.out_elems(),), -1.0, dtype=torch.float32, device="cuda")
+    plan.execute(xin, out, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    del xin
+    exact = w.in_bits == 8
+    for beam in beams_to_check:
+        for r, rg in enumerate(w.ranges):
+            tab = oracle.delay_table(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, rg.decim, rg.dm_lo, rg.dm_step, rg.ndm)
+            ns_r, maxd, nout = oracle.range_sizes(w.nsamps, rg.decim, tab)
+            info = plan.range_info(r)
+            assert (info["ns"], info["maxd"], info["nout"]) == (ns_r, maxd, nout)
+            y = oracle.decimate(x[beam], rg.decim)
+            view = plan.view_range(out, r, beam)                      # torch view [ndm][nout] on the GPU
+            # (1) sampled trials, full span, bit-exact
+            sel = _sample_trials(rg.ndm, 1000 * key + 10 * r + beam)
+            want = oracle.dedisperse(y, tab, sel=sel, t0=0, nt=nout)
+            got = view[torch.from_numpy(sel.astype(np.int64)).cuda()].cpu().numpy()
+            assert np.array_equal(got.view(np.uint32), want.view(np.uint32)), (key, beam, r)
+            # (2) every trial: row sums from prefix sums (exact integers)
+            Y = np.zeros((w.nchans, ns_r + 1), dtype=np.uint64)
+            np.cumsum(y, axis=1, dtype=np.uint64, out=Y[:, 1:])
+            rows = np.arange(w.nchans)
+            want_sum = np.empty(rg.ndm, dtype=np.float64)
+            for j in range(rg.ndm):
+                d = tab[j]
+                want_sum[j] = float((Y[rows, d + nout] - Y[rows, d]).sum())
+            got_sum = view.sum(dim=1, dtype=torch.float64).cpu().numpy()
+            if exact:
+                assert np.array_equal(got_sum, want_sum), (key, beam, r, int(np.argmax(got_sum != want_sum)))
+            else:
+                assert np.allclose(got_sum, want_sum, rtol=1e-7, atol=0), (key, beam, r)
+            # (3) DM = 0
+            if r == 0 and rg.dm_lo == 0.0:
+                plain = y.sum(axis=0, dtype=np.uint64)[:nout]
+                assert np.array_equal(view[0].cpu().numpy(), plain.astype(np.float64).astype(np.float32))
+            # row padding untouched
+            flat = out[beam * plan.beam_stride() + info["offset"]: beam * plan.beam_stride() + info["offset"] + info["ndm"] * info["pitch"]]
+            pad = flat.reshape(info["ndm"], info["pitch"])[:, info["nout"]:]
+            assert bool((pad == -1.0).all())
+            del y, Y
+    plan.destroy()
+
+
+def test_full_cfg2_1024ch():
+    _run_full(2, [0])
+
+
+def test_full_cfg3_spotlight_4096ch():
+    _run_full(3, [0])
+
+
+def test_full_cfg4_uint16():
+    _run_full(4, [0])
+
+
+def test_full_cfg5_32beams():
+    _run_full(5, [0, 13, 31])
