@@ -39,7 +39,7 @@ WORKLOAD_KEY = 3  # BASELINE.json configs[2]
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum per dd_tiled_kernel launch (mean of the 3 ranges) from the
 # committed `ncu --set full` capture (profiles/); None until one exists for the current kernel.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 10.1e9  # profiles/r1_dd_tiled_kernel_ncu_full.md: (12.27 GB range 0 + 7.98 GB range 2) / 2
 
 
 def _measured_peaks():
@@ -305,7 +305,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=WORKLOAD_KEY, help="BASELINE config number (1-5); default 3")
-    ap.add_argument("--ref-trials", type=int, default=12, help="oracle sample: trials per range")
+    ap.add_argument("--ref-trials", type=int, default=48, help="oracle sample: trials per range")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
