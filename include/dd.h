@@ -139,9 +139,11 @@ int dd_plan_set_workspace(dd_plan_t* plan, void* dev, int64_t bytes);
 int dd_plan_set_kernel(dd_plan_t* plan, int32_t variant);
 /* Tile shape the tiled kernel uses for range r (any pointer may be NULL): trials per CTA, packed time
  * words per CTA, time lanes per packed word (8 = 16-bit lanes, 4 = 32-bit lanes), channels between
- * flushes of the packed accumulators, and whether neighbouring-trial reuse is enabled. */
+ * flushes of the packed accumulators, and the table mode: 0 = one shared-memory load per (channel, trial),
+ * 1 = load skipped when the delay equals the previous trial's, 2 = delta form (all delay steps inside a
+ * group of 8 trials are 0 or 1; one changed bit per trial). */
 int dd_plan_tile_info(const dd_plan_t* plan, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta,
-                      int32_t* lanes, int32_t* flush_chans, int32_t* reuse);
+                      int32_t* lanes, int32_t* flush_chans, int32_t* mode);
 
 /* ---- per-kernel timing (measurement hook) ------------------------------------------------------- */
 

@@ -214,7 +214,7 @@ class Plan:
     def tile_info(self, r: int) -> dict:
         vals = [ctypes.c_int32() for _ in range(5)]
         _chk(_load().dd_plan_tile_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_tile_info")
-        return {k: v.value for k, v in zip(["dm_per_cta", "words_per_cta", "lanes", "flush_chans", "reuse"], vals)}
+        return {k: v.value for k, v in zip(["dm_per_cta", "words_per_cta", "lanes", "flush_chans", "mode"], vals)}
 
     def set_profiling(self, max_executes: int) -> None:
         _chk(_load().dd_plan_set_profiling(self._h, int(max_executes)), "dd_plan_set_profiling")

@@ -18,7 +18,25 @@ namespace dd {
 // A delay of d samples is a shift of d superwords for every lane at once, so any delay is a
 // 16-byte aligned access.
 constexpr int kSuperwordBytes = 16;
-constexpr int kRD = 4;            // trials register-blocked per thread
+constexpr int kRD = 8;            // trials register-blocked per thread (one "trial group")
+
+// How the tiled kernel finds the staged superword of (channel, trial):
+//   kModeGeneral       per channel and trial group: kRD 16-bit superword offsets, one shared-memory load per trial
+//   kModeGeneralReuse  same table; the load is skipped when the offset equals the previous trial's
+//   kModeDelta         every delay step inside a trial group is 0 or 1 (fine DM grids): per channel the
+//                      offset of the group's first trial plus one "changed" bit per later trial; a changed
+//                      bit advances the address by one superword and reloads, otherwise the registers are reused
+enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2 };
+
+// kModeDelta processes channels in quads A,B,C,D.  The changed bits of a quad share one 32-bit word laid
+// out so that each byte feeds one R2P (register -> 7 predicates): bit n%7 of byte n/7, n = (j-1)*4 + q
+// for trial step j = 1..kRD-1 of channel q = 0..3.
+__host__ __device__ constexpr int delta_bit(int j, int q) { return (((j - 1) * 4 + q) / 7) * 8 + ((j - 1) * 4 + q) % 7; }
+
+// Meta bytes per pipeline stage of Cc channels and G trial groups.
+__host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int Cc, int G) {
+  return (size_t)(mode == kModeDelta ? Cc / 4 : Cc) * (size_t)G * 16;
+}
 
 struct RangePlan {
   // definition
@@ -29,13 +47,13 @@ struct RangePlan {
   // tiled kernel shape
   int NL = 8;        // lanes per superword
   int flush = 0;     // channels between flushes of the 16-bit lanes (0: never, 32-bit lanes)
+  int mode = 0;      // TiledMode
   int G = 0;         // trial groups per CTA (kRD trials each)
   int T = 0;         // superwords per CTA (multiple of 32)
   int Dcta = 0;      // trials per CTA = G*kRD
   int Cc = 0;        // channels per pipeline stage
   int stages = 0;
   int tiled_ok = 0;  // 0: the tile does not fit shared memory, this range runs the direct kernel
-  int reuse = 0;     // skip shared-memory reloads when neighbouring trials share a delay
   int nblocks = 0;   // trial blocks = ceil(ndm/Dcta)
   int Smax = 0;      // largest delay spread inside one trial block (superwords)
   int Cpad = 0;      // nchans rounded up to a multiple of Cc (zero rows)
@@ -46,7 +64,8 @@ struct RangePlan {
   int64_t ws_bytes = 0;
   size_t smem_bytes = 0;
   // device tables
-  uint32_t* d_meta = nullptr;   // [nblocks][Cpad][Dcta] byte offsets (delay - dmin) * 16
+  uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] kRD 16-bit offsets (delay - dmin, superwords);
+                                // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, 0}
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
   int32_t* d_delays = nullptr;  // [ndm][nchans], only for the direct kernel (lazy)

@@ -19,43 +19,6 @@
 namespace dd {
 
 // ------------------------------------------------------------------------------------------------
-// PTX helpers: mbarrier + 1-D bulk async copy (TMA), shared::cta addresses are 32-bit.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra WAIT_DONE;\n"
-      "bra WAIT_LOOP;\n"
-      "WAIT_DONE:\n"
-      "}\n" ::"r"(bar),
-      "r"(parity)
-      : "memory");
-}
-__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-               "l"(src), "r"(bytes), "r"(bar)
-               : "memory");
-}
-__device__ __forceinline__ void fence_barrier_init() {
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-
-// ------------------------------------------------------------------------------------------------
 // a2: pack + time decimation
 // ------------------------------------------------------------------------------------------------
 // Thread = 4 consecutive superwords i0..i0+3 of one (beam, channel) row.
@@ -163,298 +126,6 @@ cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev
     return r.NL == 8 ? launch_pack_t<uint8_t, 8>(p, r, in_dev, stream) : launch_pack_t<uint8_t, 4>(p, r, in_dev, stream);
   }
   return r.NL == 8 ? launch_pack_t<uint16_t, 8>(p, r, in_dev, stream) : launch_pack_t<uint16_t, 4>(p, r, in_dev, stream);
-}
-
-// ------------------------------------------------------------------------------------------------
-// a3 + a4: tiled dedispersion
-// ------------------------------------------------------------------------------------------------
-struct TiledParams {
-  const uint4* P;        // packed input of this range [nbeams][Cpad][Wp]
-  const uint32_t* meta;  // [nblocks][Cpad][Dcta] byte offsets (d - dmin)*16
-  const int32_t* dmin;   // [nblocks][Cpad]
-  const int32_t* span;   // [nblocks][Cpad]
-  float* out;            // beam 0, this range
-  long long out_beam_stride, pitch, Wp, H, nout, ntau;
-  int ndm, Cpad, Dcta, T, Cc, nstages, nblocks;
-  int rowpitch;      // superwords per staged row = T + Smax
-  int flush_stages;  // flush the 16-bit lanes every this many stages (NL == 8)
-};
-
-__host__ __device__ inline size_t tiled_stage_bytes(int Cc, int rowpitch, int Dcta) {
-  return (size_t)Cc * ((size_t)rowpitch * kSuperwordBytes + (size_t)Dcta * 4);
-}
-constexpr int kBarRegion = 128;  // bytes reserved for the mbarriers at the start of dynamic smem
-
-size_t tiled_smem_bytes(const RangePlan& r) {
-  return kBarRegion + (size_t)r.stages * tiled_stage_bytes(r.Cc, r.T + r.Smax, r.Dcta);
-}
-
-__device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4& b) {
-  // one IADD3 per 32-bit word: two channels, and (NL == 8) two 16-bit time lanes, per instruction
-  acc.x = acc.x + a.x + b.x;
-  acc.y = acc.y + a.y + b.y;
-  acc.z = acc.z + a.z + b.z;
-  acc.w = acc.w + a.w + b.w;
-}
-
-// Shared-memory superword loads of the inner loop, written in PTX so that the conditional reload
-// overwrites the four registers IN PLACE (the C++ form made ptxas copy them on every trial).
-__device__ __forceinline__ void lds_first(uint4& w, uint32_t base, uint32_t off) {
-  asm volatile("{\n .reg .u32 a;\n add.u32 a, %4, %5;\n ld.shared.v4.u32 {%0,%1,%2,%3}, [a];\n}"
-               : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
-               : "r"(base), "r"(off));
-}
-template <bool REUSE>
-__device__ __forceinline__ void lds_if_changed(uint4& w, uint32_t base, uint32_t off, uint32_t prev) {
-  if constexpr (REUSE) {
-    asm volatile(
-        "{\n .reg .pred p;\n .reg .u32 a;\n setp.ne.u32 p, %5, %6;\n add.u32 a, %4, %5;\n"
-        " @p ld.shared.v4.u32 {%0,%1,%2,%3}, [a];\n}"
-        : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w)
-        : "r"(base), "r"(off), "r"(prev));
-  } else {
-    lds_first(w, base, off);
-  }
-}
-
-template <int NL, bool REUSE, int NT>
-__global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParams p) {
-  extern __shared__ __align__(128) unsigned char smem[];
-  const int tid = threadIdx.x;
-  // CTA -> (trial block fastest, time tile, beam): CTAs resident together share a time tile in L2
-  const long long lin = blockIdx.x;
-  const int blk = (int)(lin % p.nblocks);
-  const long long rest = lin / p.nblocks;
-  const long long tau = rest % p.ntau;
-  const int beam = (int)(rest / p.ntau);
-
-  const uint32_t bar_base = smem_u32(smem);  // full[s] at +8*s, empty[s] at +8*(nstages+s)
-  const int nstages = p.nstages;
-  const size_t stage_bytes = tiled_stage_bytes(p.Cc, p.rowpitch, p.Dcta);
-  const uint32_t row_bytes = (uint32_t)p.rowpitch * kSuperwordBytes;
-  const uint32_t data_bytes = (uint32_t)p.Cc * row_bytes;
-  const uint32_t meta_bytes = (uint32_t)p.Cc * (uint32_t)p.Dcta * 4u;
-  const int nchunks = p.Cpad / p.Cc;
-
-  if (tid == 0) {
-    for (int s = 0; s < nstages; ++s) {
-      mbar_init(bar_base + 8u * s, 1);                    // full: one arrive.expect_tx by the producer
-      mbar_init(bar_base + 8u * (nstages + s), NT / 32);  // empty: one arrive per consumer warp
-    }
-    fence_barrier_init();
-  }
-  __syncthreads();
-
-  // ---------------- producer role, rotated over the warps ---------------------------------------------
-  // Chunk k (channels k*Cc .. k*Cc+Cc-1) is issued by warp k % nwarps: one bulk copy per channel row plus
-  // one for the offsets, landing in stage k % nstages and signalling full[stage] with the byte count.
-  // A warp issues chunk k when it starts iteration k - ahead (ahead = nstages - 2): the stage it refills
-  // was consumed two iterations ago, so the wait on its empty barrier is normally already satisfied.
-  // Row start and length of the warp's NEXT chunk are fetched one turn early (pf_d0 / pf_bytes).
-  const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T;
-  const long long tab = (long long)blk * p.Cpad;
-  const int lane = tid & 31;
-  const int warp = tid >> 5;
-  constexpr int kWarps = NT / 32;
-  const int ahead = nstages - 2;
-  int pf_d0 = 0;
-  uint32_t pf_bytes = 0;
-  auto prefetch = [&](int k) {
-    pf_bytes = 0;
-    if (k < nchunks && lane < p.Cc) {
-      const int c = k * p.Cc + lane;
-      pf_d0 = __ldg(p.dmin + tab + c);
-      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
-    }
-  };
-  auto produce = [&](int k) {
-    const int s = k % nstages;
-    if (k >= nstages) mbar_wait(bar_base + 8u * (nstages + s), ((uint32_t)(k / nstages) & 1u) ^ 1u);
-    const uint32_t sbase = smem_u32(smem + kBarRegion + (size_t)s * stage_bytes);
-    const uint32_t full = bar_base + 8u * s;
-    uint32_t total = pf_bytes;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
-    if (lane == 0) {
-      mbar_arrive_expect_tx(full, total + meta_bytes);
-      bulk_copy_g2s(sbase + data_bytes, p.meta + (tab + (long long)k * p.Cc) * p.Dcta, meta_bytes, full);
-    }
-    __syncwarp();
-    if (lane < p.Cc)
-      bulk_copy_g2s(sbase + lane * row_bytes, Pbeam + (long long)(k * p.Cc + lane) * p.Wp + pf_d0, pf_bytes, full);
-  };
-  // prologue: chunks 0 .. ahead-1
-  for (int k = warp; k < ahead && k < nchunks; k += kWarps) {
-    prefetch(k);
-    produce(k);
-  }
-  {  // first chunk this warp issues inside the loop
-    int k = warp;
-    while (k < ahead) k += kWarps;
-    prefetch(k);
-  }
-
-  // ---------------- consumers: kRD trials x one superword (NL time lanes) per thread --------------
-  const int g = tid / p.T;       // trial group inside the CTA (warp-uniform: T is a multiple of 32)
-  const int ti = tid - g * p.T;  // superword inside the time tile
-  uint4 acc[kRD];
-  uint32_t wide[kRD][NL == 8 ? 8 : 1];
-#pragma unroll
-  for (int j = 0; j < kRD; ++j) {
-    acc[j] = make_uint4(0, 0, 0, 0);
-#pragma unroll
-    for (int m = 0; m < (NL == 8 ? 8 : 1); ++m) wide[j][m] = 0;
-  }
-  const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
-  const uint32_t group_off = (uint32_t)g * kRD * 4u;
-  const uint32_t meta_row = (uint32_t)p.Dcta * 4u;
-  int since_flush = 0;
-
-  for (int it = 0; it < nchunks; ++it) {
-    const int s = it % nstages;
-    const uint32_t ph = (uint32_t)(it / nstages) & 1u;
-    {  // producer turn: chunk it + ahead belongs to warp (it + ahead) % kWarps
-      const int k = it + ahead;
-      if (k < nchunks && (k % kWarps) == warp) {
-        produce(k);
-        prefetch(k + kWarps);
-      }
-    }
-    mbar_wait(bar_base + 8u * s, ph);
-    const unsigned char* sdata = smem + kBarRegion + (size_t)s * stage_bytes + thread_off;
-    const unsigned char* smeta = smem + kBarRegion + (size_t)s * stage_bytes + data_bytes + group_off;
-#pragma unroll 2
-    for (int cc = 0; cc < p.Cc; cc += 2) {
-      const uint4 oa = *reinterpret_cast<const uint4*>(smeta + (uint32_t)cc * meta_row);
-      const uint4 ob = *reinterpret_cast<const uint4*>(smeta + (uint32_t)(cc + 1) * meta_row);
-      const unsigned char* ra = sdata + (uint32_t)cc * row_bytes;
-      const unsigned char* rb = ra + row_bytes;
-      const uint32_t aa = smem_u32(ra), ab = smem_u32(rb);
-      uint4 wa, wb;
-      lds_first(wa, aa, oa.x);
-      lds_first(wb, ab, ob.x);
-      add_pair(acc[0], wa, wb);
-      lds_if_changed<REUSE>(wa, aa, oa.y, oa.x);
-      lds_if_changed<REUSE>(wb, ab, ob.y, ob.x);
-      add_pair(acc[1], wa, wb);
-      lds_if_changed<REUSE>(wa, aa, oa.z, oa.y);
-      lds_if_changed<REUSE>(wb, ab, ob.z, ob.y);
-      add_pair(acc[2], wa, wb);
-      lds_if_changed<REUSE>(wa, aa, oa.w, oa.z);
-      lds_if_changed<REUSE>(wb, ab, ob.w, ob.z);
-      add_pair(acc[3], wa, wb);
-    }
-    __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive(bar_base + 8u * (nstages + s));  // stage may be refilled
-    if constexpr (NL == 8) {
-      if (++since_flush == p.flush_stages) {  // 16-bit lanes would overflow next: widen to 32 bits
-        since_flush = 0;
-#pragma unroll
-        for (int j = 0; j < kRD; ++j) {
-          wide[j][0] += acc[j].x & 0xffffu;
-          wide[j][1] += acc[j].x >> 16;
-          wide[j][2] += acc[j].y & 0xffffu;
-          wide[j][3] += acc[j].y >> 16;
-          wide[j][4] += acc[j].z & 0xffffu;
-          wide[j][5] += acc[j].z >> 16;
-          wide[j][6] += acc[j].w & 0xffffu;
-          wide[j][7] += acc[j].w >> 16;
-          acc[j] = make_uint4(0, 0, 0, 0);
-        }
-      }
-    }
-  }
-
-  // ---------------- a4: DM-time writer, fp32 (I2F rounds to nearest even) -------------------------
-  const long long i = tau * p.T + ti;
-  if (i >= p.H) return;
-  float* obase = p.out + (long long)beam * p.out_beam_stride;
-#pragma unroll
-  for (int j = 0; j < kRD; ++j) {
-    const int jj = blk * p.Dcta + g * kRD + j;
-    if (jj >= p.ndm) break;
-    float* orow = obase + (long long)jj * p.pitch;
-    uint32_t v[NL];
-    if constexpr (NL == 8) {
-      v[0] = wide[j][0] + (acc[j].x & 0xffffu);
-      v[1] = wide[j][1] + (acc[j].x >> 16);
-      v[2] = wide[j][2] + (acc[j].y & 0xffffu);
-      v[3] = wide[j][3] + (acc[j].y >> 16);
-      v[4] = wide[j][4] + (acc[j].z & 0xffffu);
-      v[5] = wide[j][5] + (acc[j].z >> 16);
-      v[6] = wide[j][6] + (acc[j].w & 0xffffu);
-      v[7] = wide[j][7] + (acc[j].w >> 16);
-    } else {
-      v[0] = acc[j].x;
-      v[1] = acc[j].y;
-      v[2] = acc[j].z;
-      v[3] = acc[j].w;
-    }
-#pragma unroll
-    for (int m = 0; m < NL; ++m) {
-      const long long t = i + (long long)m * p.H;
-      if (t < p.nout) orow[t] = __uint2float_rn(v[m]);  // consecutive threads -> consecutive floats
-    }
-  }
-}
-
-template <int NL, bool REUSE, int NT>
-static cudaError_t launch_tiled_t(const TiledParams& tp, long long nctas, size_t smem, cudaStream_t stream) {
-  dd_tiled_kernel<NL, REUSE, NT><<<(unsigned)nctas, NT, smem, stream>>>(tp);
-  return cudaGetLastError();
-}
-
-template <int NL, bool REUSE, int NT>
-static cudaError_t set_smem_t() {
-  return cudaFuncSetAttribute(dd_tiled_kernel<NL, REUSE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-}
-
-cudaError_t configure_kernels(const dd_plan*) {
-  cudaError_t e;
-#define DD_CFG(NL, RE, NT) \
-  if ((e = set_smem_t<NL, RE, NT>()) != cudaSuccess) return e;
-  DD_CFG(8, false, 256) DD_CFG(8, true, 256) DD_CFG(8, false, 512) DD_CFG(8, true, 512)
-  DD_CFG(4, false, 256) DD_CFG(4, true, 256) DD_CFG(4, false, 512) DD_CFG(4, true, 512)
-#undef DD_CFG
-  return cudaSuccess;
-}
-
-cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream) {
-  TiledParams tp;
-  tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset);
-  tp.meta = r.d_meta;
-  tp.dmin = r.d_dmin;
-  tp.span = r.d_span;
-  tp.out = out_dev + r.offset;
-  tp.out_beam_stride = p->beam_stride;
-  tp.pitch = r.pitch;
-  tp.Wp = r.Wp;
-  tp.H = r.H;
-  tp.nout = r.nout;
-  tp.ntau = r.ntau;
-  tp.ndm = r.ndm;
-  tp.Cpad = r.Cpad;
-  tp.Dcta = r.Dcta;
-  tp.T = r.T;
-  tp.Cc = r.Cc;
-  tp.nstages = r.stages;
-  tp.nblocks = r.nblocks;
-  tp.rowpitch = r.T + r.Smax;
-  tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;
-  const long long nctas = (long long)r.nblocks * r.ntau * p->nbeams;
-  if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  const size_t smem = tiled_smem_bytes(r);
-  const int nt = r.G * r.T;
-#define DD_GO(NL, RE, NT) return launch_tiled_t<NL, RE, NT>(tp, nctas, smem, stream)
-  if (r.NL == 8) {
-    if (nt == 512) { if (r.reuse) DD_GO(8, true, 512); else DD_GO(8, false, 512); }
-    if (nt == 256) { if (r.reuse) DD_GO(8, true, 256); else DD_GO(8, false, 256); }
-  } else {
-    if (nt == 512) { if (r.reuse) DD_GO(4, true, 512); else DD_GO(4, false, 512); }
-    if (nt == 256) { if (r.reuse) DD_GO(4, true, 256); else DD_GO(4, false, 256); }
-  }
-#undef DD_GO
-  return cudaErrorInvalidConfiguration;
 }
 
 // ------------------------------------------------------------------------------------------------

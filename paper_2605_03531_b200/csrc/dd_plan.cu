@@ -69,22 +69,49 @@ inline int block_spread(const dd_plan& p, const dd::RangePlan& r, int blk, int D
   return r.delays[(size_t)j1 * p.nchans + c] - r.delays[(size_t)j0 * p.nchans + c];
 }
 
+// Which table form the tiled kernel uses for this range (dd_internal.h TiledMode).  Trial groups are the
+// kRD-aligned runs of trials counted from the start of the range.
+int choose_mode(const dd_plan& p, const dd::RangePlan& r) {
+  bool delta = true;
+  int64_t same = 0, total = 0;
+  for (int j = 0; j + 1 < r.ndm; ++j) {
+    if ((j + 1) % dd::kRD == 0) continue;  // first trial of a group always loads
+    const int32_t* d0 = &r.delays[(size_t)j * p.nchans];
+    const int32_t* d1 = d0 + p.nchans;
+    for (int c = 0; c < p.nchans; ++c) {
+      const int32_t inc = d1[c] - d0[c];
+      same += inc == 0;
+      delta = delta && inc <= 1;
+    }
+    total += p.nchans;
+  }
+  int mode = delta ? dd::kModeDelta : (total > 0 && (double)same / (double)total >= 0.25) ? dd::kModeGeneralReuse
+                                                                                         : dd::kModeGeneral;
+  mode = env_int("DD_MODE", mode);  // tuning hook (measurements only); delta is refused when it does not apply
+  if (mode < 0 || mode > 2 || (mode == dd::kModeDelta && !delta)) mode = dd::kModeGeneral;
+  return mode;
+}
+
 // Pick the tile shape of the tiled kernel for one range: more trials per CTA amortise the
 // L2 -> shared-memory fill of a channel row over more adds, but widen the staged window by the delay
 // spread of the block.  Cost model: staged bytes per add; constraint: >= 3 stages in 200 KB.
 void choose_tile(const dd_plan& p, dd::RangePlan& r) {
+  // 16-bit lanes hold lo + 256*hi exactly when (a) 255 + flush*maxval <= 65535 between flushes and (b) the
+  // hi lanes, which gain at most 255 per flush, stay below 65536: at most 256 flushes.
   const int maxval = ((1 << p.in_bits) - 1) * r.decim;
-  if (maxval <= 4095) {  // at least 16 channels between flushes
+  const int flush0 = 65280 / maxval;
+  if (maxval <= 4095 && (int64_t)p.nchans <= (int64_t)120 * flush0) {
     r.NL = 8;
-    r.flush = std::min(256, 65535 / maxval);
+    r.flush = flush0;
   } else {
     r.NL = 4;
     r.flush = 0;
   }
+  r.mode = choose_mode(p, r);
   static const int cand[][2] = {{16, 32}, {8, 64}, {4, 128}, {2, 256}, {1, 512}, {8, 32}, {4, 64}, {2, 128}, {1, 256}};
   const size_t budget = 200 * 1024;
   double best = 1e300;
-  TileChoice bc = {1, 256, 2, 2};
+  TileChoice bc = {1, 256, 4, 2};
   bool found = false;
   for (auto& gt : cand) {
     const int G = gt[0], T = gt[1], D = G * dd::kRD;
@@ -97,14 +124,17 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
       smax = std::max(smax, block_spread(p, r, b, D, p.nchans - 1));
       for (int c = 0; c < p.nchans; c += cstep, ++nsamp) ssum += block_spread(p, r, b, D, c);
     }
+    if (T + smax > 65535) continue;  // 16-bit offsets
     const double smean = ssum / std::max(1, nsamp);
-    for (int Cc : {16, 8, 4, 2}) {
+    for (int Cc : {32, 16, 8, 4}) {
       if (r.NL == 8 && Cc > r.flush) continue;
-      const size_t stage = (size_t)Cc * ((size_t)(T + smax) * 16 + (size_t)D * 4);
+      const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, Cc, G);
       const int stages = (int)std::min<size_t>(6, budget / stage);
       if (stages < (Cc >= 8 ? 3 : 2)) continue;
-      // bytes staged per add: row (T + mean spread) superwords + the offsets row, over T*NL*D adds
-      double cost = ((T + smean) * 16.0 + D * 4.0) / ((double)T * r.NL * D);
+      // bytes staged per add: row (T + mean spread) superwords + the table row, over T*NL*D adds
+      double cost = ((T + smean) * 16.0 + dd::tiled_meta_bytes(r.mode, 4, G) / 4.0) / ((double)T * r.NL * D);
+      // trials past the end of the last block are computed and dropped
+      cost *= (double)nblocks * D / (double)r.ndm;
       if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
       if (Cc < 16) cost *= 1.0 + 0.05 * (16 / Cc - 1);  // shorter stages synchronise more often
       if (cost < best) {
@@ -114,12 +144,12 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
       }
     }
   }
-  r.tiled_ok = found ? 1 : 0;  // otherwise the delay spread of 4 trials exceeds shared memory: direct kernel
+  r.tiled_ok = found ? 1 : 0;  // otherwise the delay spread of one trial group exceeds shared memory: direct kernel
   // tuning hook (measurements only): DD_TILE="G,T,Cc,stages"
   if (const char* s = getenv("DD_TILE")) {
     int g, t, cc, st;
     if (sscanf(s, "%d,%d,%d,%d", &g, &t, &cc, &st) == 4 && (g * t == 256 || g * t == 512) && t % 32 == 0 &&
-        cc >= 2 && cc <= 32 && cc % 2 == 0 && st >= 2 && st <= 8 && (r.NL != 8 || cc <= r.flush)) {
+        cc >= 4 && cc <= 32 && cc % 4 == 0 && st >= 2 && st <= 8 && (r.NL != 8 || cc <= r.flush)) {
       bc = {g, t, cc, st};
       r.tiled_ok = 1;
     }
@@ -133,19 +163,8 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   r.Cpad = (int)round_up(p.nchans, r.Cc);
   if (r.NL == 8) r.flush = r.flush / r.Cc * r.Cc;
   r.Smax = 0;
-  int64_t same = 0, total = 0;
   for (int b = 0; b < r.nblocks; ++b) r.Smax = std::max(r.Smax, block_spread(p, r, b, r.Dcta, p.nchans - 1));
-  // fraction of neighbouring-trial transitions (inside a register block) that keep the delay
-  const int cstep = std::max(1, p.nchans / 128);
-  for (int j = 0; j + 1 < r.ndm; ++j) {
-    if ((j + 1) % dd::kRD == 0) continue;
-    for (int c = 0; c < p.nchans; c += cstep) {
-      same += r.delays[(size_t)j * p.nchans + c] == r.delays[(size_t)(j + 1) * p.nchans + c];
-      ++total;
-    }
-  }
-  r.reuse = total > 0 && (double)same / (double)total >= 0.25;
-  r.reuse = env_int("DD_REUSE", r.reuse) ? 1 : 0;
+  if (r.T + r.Smax > 65535) r.tiled_ok = 0;
   while (r.stages > 2 && dd::tiled_smem_bytes(r) > (size_t)227 * 1024) --r.stages;
   r.H = round_up((r.nout + r.NL - 1) / r.NL, 16);
   r.ntau = (r.H + r.T - 1) / r.T;
@@ -157,24 +176,35 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
 }
 
 // Device tables of the tiled kernel: per trial block and channel the first delay (start of the staged
-// row), the spread (length of the staged row beyond T) and per trial the byte offset into the row.
+// row) and the spread (length of the staged row beyond T); per trial group the offsets into the row in
+// the form the range's mode wants (dd_internal.h).  Trials past the end of the range repeat the last one;
+// rows past nchans (zero rows of the packed input) keep offset 0.
 int upload_tables(const dd_plan& p, dd::RangePlan& r) {
   const size_t nbc = (size_t)r.nblocks * r.Cpad;
   std::vector<int32_t> dmin(nbc, 0), span(nbc, 0);
-  std::vector<uint32_t> meta(nbc * r.Dcta, 0);
+  const bool delta = r.mode == dd::kModeDelta;
+  const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
+  std::vector<uint32_t> meta(nentries * 4, 0);
+  auto delay = [&](int j, int c) { return r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c]; };
   for (int b = 0; b < r.nblocks; ++b) {
+    const int j0 = b * r.Dcta;
     for (int c = 0; c < p.nchans; ++c) {
-      const int j0 = b * r.Dcta;
-      const int32_t d0 = r.delays[(size_t)j0 * p.nchans + c];
-      int32_t dl = d0;
-      for (int jj = 0; jj < r.Dcta; ++jj) {
-        const int j = std::min(r.ndm - 1, j0 + jj);  // trials past the end repeat the last one
-        const int32_t d = r.delays[(size_t)j * p.nchans + c];
-        dl = std::max(dl, d);
-        meta[((size_t)b * r.Cpad + c) * r.Dcta + jj] = (uint32_t)(d - d0) * dd::kSuperwordBytes;
-      }
+      const int32_t d0 = delay(j0, c);
       dmin[(size_t)b * r.Cpad + c] = d0;
-      span[(size_t)b * r.Cpad + c] = dl - d0;
+      span[(size_t)b * r.Cpad + c] = delay(j0 + r.Dcta - 1, c) - d0;  // delays are non-decreasing in j
+      for (int g = 0; g < r.G; ++g) {
+        const int jg = j0 + g * dd::kRD;
+        if (delta) {
+          uint32_t* e = &meta[(((size_t)b * (r.Cpad / 4) + c / 4) * r.G + g) * 4];
+          const int q = c % 4;
+          e[1 + q / 2] |= (uint32_t)(delay(jg, c) - d0) << (16 * (q % 2));
+          for (int j = 1; j < dd::kRD; ++j)
+            if (delay(jg + j, c) != delay(jg + j - 1, c)) e[0] |= 1u << dd::delta_bit(j, q);
+        } else {
+          uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * 4];
+          for (int j = 0; j < dd::kRD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));
+        }
+      }
     }
   }
   DD_CUDA(cudaMalloc(&r.d_meta, meta.size() * sizeof(uint32_t)));
@@ -515,14 +545,14 @@ int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* m
 }
 
 int dd_plan_tile_info(const dd_plan_t* p, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta, int32_t* lanes,
-                      int32_t* flush_chans, int32_t* reuse) {
+                      int32_t* flush_chans, int32_t* mode) {
   if (!p || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
   const auto& q = p->ranges[r];
   if (dm_per_cta) *dm_per_cta = q.Dcta;
   if (words_per_cta) *words_per_cta = q.T;
   if (lanes) *lanes = q.NL;
   if (flush_chans) *flush_chans = q.flush;
-  if (reuse) *reuse = q.reuse;
+  if (mode) *mode = q.mode;
   return DD_OK;
 }
 

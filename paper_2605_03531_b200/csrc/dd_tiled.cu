@@ -1,0 +1,432 @@
+// dd_tiled.cu -- steps a3 + a4 of the hot path: the tiled dedispersion kernel and its
+// launcher.
+//
+//   S[j][t] = sum_c y[c][t + d(c,j)]      (PAPER.md:421 brute-force O(m x N) sum; delays of Eq. 1.1)
+//
+// CTA tile = Dcta trials x T superwords x all channels.  Thread = kRD (8) neighbouring trials x one
+// superword (NL time lanes, dd_internal.h).  Channel rows are staged into a shared-memory ring by 1-D TMA
+// bulk copies (cp.async.bulk + mbarrier).  The adder is integer and packed: one IADD3 adds two channels
+// into two 16-bit time lanes (NL == 8), i.e. four algorithmic adds per instruction.  Packed lanes are kept
+// exact by a two-level carry-save scheme: every `flush` channels the upper bytes of the 16-bit lanes are
+// moved into a second packed accumulator (sum = lo + 256*hi), so the accumulators of a trial are 8
+// registers and never overflow.  Neighbouring trials that share a delay reuse the superword held in
+// registers (kModeDelta / kModeGeneralReuse).  The DM-time writer converts once (I2F.RN) and stores fp32.
+//
+// Integer sums are exact, so the result has the same bits as the definition whatever the order.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dd_internal.h"
+
+namespace dd {
+
+// ------------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + 1-D bulk async copy (TMA); shared::cta addresses are 32-bit.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+// Shared-memory superword loads of the inner loop, written in PTX so that a conditional reload overwrites
+// the four registers IN PLACE (the C++ form makes ptxas copy them on every trial).
+__device__ __forceinline__ void lds_sw(uint4& w, uint32_t addr) {
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(addr));
+}
+// general modes: reload iff this trial's offset differs from the previous trial's
+__device__ __forceinline__ void lds_if_ne(uint4& w, uint32_t addr, uint32_t off, uint32_t prev) {
+  asm volatile(
+      "{\n .reg .pred p;\n setp.ne.u32 p, %5, %6;\n"
+      " @p ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n}"
+      : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w)
+      : "r"(addr), "r"(off), "r"(prev));
+}
+// delta mode: if bit BIT of m is set, step one superword forward and reload
+template <int BIT>
+__device__ __forceinline__ void lds_if_bit(uint4& w, uint32_t& addr, uint32_t m) {
+  asm volatile(
+      "{\n .reg .pred p;\n .reg .b32 t;\n and.b32 t, %5, %6;\n setp.ne.u32 p, t, 0;\n"
+      " @p add.u32 %4, %4, 16;\n"
+      " @p ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n}"
+      : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w), "+r"(addr)
+      : "r"(m), "n"(1u << BIT));
+}
+
+__device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4& b) {
+  // one IADD3 per 32-bit word: two channels, and (NL == 8) two 16-bit time lanes, per instruction
+  acc.x = acc.x + a.x + b.x;
+  acc.y = acc.y + a.y + b.y;
+  acc.z = acc.z + a.z + b.z;
+  acc.w = acc.w + a.w + b.w;
+}
+
+struct TiledParams {
+  const uint4* P;       // packed input of this range [nbeams][Cpad][Wp]
+  const uint4* meta;    // per trial block: offsets / changed bits (dd_internal.h RangePlan::d_meta)
+  const int32_t* dmin;  // [nblocks][Cpad] first delay of the block = start of the staged row
+  const int32_t* span;  // [nblocks][Cpad] delay spread of the block = staged row length beyond T
+  float* out;           // beam 0, this range
+  long long out_beam_stride, pitch, Wp, H, nout, ntau;
+  int ndm, Cpad, G, T, Cc, nstages, nblocks;
+  int rowpitch;      // superwords per staged row = T + Smax
+  int flush_stages;  // move the upper bytes of the 16-bit lanes away every this many stages (NL == 8)
+};
+
+__host__ __device__ inline size_t tiled_stage_bytes(int mode, int Cc, int rowpitch, int G) {
+  return (size_t)Cc * (size_t)rowpitch * kSuperwordBytes + tiled_meta_bytes(mode, Cc, G);
+}
+constexpr int kBarRegion = 128;  // bytes reserved for the mbarriers at the start of dynamic smem
+
+size_t tiled_smem_bytes(const RangePlan& r) {
+  return kBarRegion + (size_t)r.stages * tiled_stage_bytes(r.mode, r.Cc, r.T + r.Smax, r.G);
+}
+
+// ------------------------------------------------------------------------------------------------
+// consumer bodies: one pipeline stage (Cc channels) accumulated into the kRD trials of this thread
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t off16(const uint4& m, int j) {  // j-th 16-bit field of a meta entry
+  const uint32_t w = (j >> 1) == 0 ? m.x : (j >> 1) == 1 ? m.y : (j >> 1) == 2 ? m.z : m.w;
+  return (j & 1) ? (w >> 16) : (w & 0xffffu);
+}
+
+// general modes: channels in pairs, one table entry (kRD 16-bit superword offsets) per channel
+template <bool REUSE>
+__device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
+                                              uint32_t row_bytes, uint32_t meta_row) {
+#pragma unroll 1
+  for (int cc = 0; cc < Cc; cc += 2) {
+    uint4 ma, mb;
+    lds_sw(ma, smeta);
+    lds_sw(mb, smeta + meta_row);
+    smeta += 2 * meta_row;
+    const uint32_t ra = sdata, rb = sdata + row_bytes;
+    sdata += 2 * row_bytes;
+    uint4 wa, wb;
+    uint32_t pa = off16(ma, 0), pb = off16(mb, 0);
+    lds_sw(wa, ra + pa * kSuperwordBytes);
+    lds_sw(wb, rb + pb * kSuperwordBytes);
+    add_pair(acc[0], wa, wb);
+#pragma unroll
+    for (int j = 1; j < kRD; ++j) {
+      const uint32_t oa = off16(ma, j), ob = off16(mb, j);
+      if constexpr (REUSE) {
+        lds_if_ne(wa, ra + oa * kSuperwordBytes, oa, pa);
+        lds_if_ne(wb, rb + ob * kSuperwordBytes, ob, pb);
+        pa = oa;
+        pb = ob;
+      } else {
+        lds_sw(wa, ra + oa * kSuperwordBytes);
+        lds_sw(wb, rb + ob * kSuperwordBytes);
+      }
+      add_pair(acc[j], wa, wb);
+    }
+  }
+}
+
+// delta mode: channels in quads A..D; one table entry per quad = {changed bits, offA|offB<<16, offC|offD<<16, -}
+template <int J>
+__device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t& aa,
+                                            uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits) {
+  if constexpr (J < kRD) {
+    lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
+    lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
+    lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
+    lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
+    add_pair(acc[J], wa, wb);
+    add_pair(acc[J], wc, wd);
+    delta_steps<J + 1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bits);
+  }
+}
+
+__device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes,
+                                            uint32_t meta_row) {
+#pragma unroll 1
+  for (int cc = 0; cc < Cc; cc += 4) {
+    uint4 m;
+    lds_sw(m, smeta);
+    smeta += meta_row;
+    uint32_t aa = sdata + (m.y & 0xffffu) * kSuperwordBytes;
+    uint32_t ab = sdata + row_bytes + (m.y >> 16) * kSuperwordBytes;
+    uint32_t ac = sdata + 2 * row_bytes + (m.z & 0xffffu) * kSuperwordBytes;
+    uint32_t ad = sdata + 3 * row_bytes + (m.z >> 16) * kSuperwordBytes;
+    sdata += 4 * row_bytes;
+    uint4 wa, wb, wc, wd;
+    lds_sw(wa, aa);
+    lds_sw(wb, ab);
+    lds_sw(wc, ac);
+    lds_sw(wd, ad);
+    add_pair(acc[0], wa, wb);
+    add_pair(acc[0], wc, wd);
+    delta_steps<1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, m.x);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// the kernel
+// ------------------------------------------------------------------------------------------------
+template <int NL, int MODE, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParams p) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int tid = threadIdx.x;
+  // CTA -> (trial block fastest, time tile, beam): CTAs resident together share a time tile in L2
+  const long long lin = blockIdx.x;
+  const int blk = (int)(lin % p.nblocks);
+  const long long rest = lin / p.nblocks;
+  const long long tau = rest % p.ntau;
+  const int beam = (int)(rest / p.ntau);
+
+  const uint32_t bar_base = smem_u32(smem);  // full[s] at +8*s, empty[s] at +8*(nstages+s)
+  const int nstages = p.nstages;
+  const uint32_t row_bytes = (uint32_t)p.rowpitch * kSuperwordBytes;
+  const uint32_t data_bytes = (uint32_t)p.Cc * row_bytes;
+  const uint32_t meta_bytes = (uint32_t)tiled_meta_bytes(MODE, p.Cc, p.G);
+  const uint32_t stage_bytes = data_bytes + meta_bytes;
+  const uint32_t stage0 = bar_base + kBarRegion;
+  const int nchunks = p.Cpad / p.Cc;
+
+  if (tid == 0) {
+    for (int s = 0; s < nstages; ++s) {
+      mbar_init(bar_base + 8u * s, 1);                    // full: one arrive.expect_tx by the producer
+      mbar_init(bar_base + 8u * (nstages + s), NT / 32);  // empty: one arrive per consumer warp
+    }
+    fence_barrier_init();
+  }
+  __syncthreads();
+
+  // ---------------- producer role, rotated over the warps ---------------------------------------------
+  // Chunk k (channels k*Cc .. k*Cc+Cc-1) is issued by warp k % nwarps: one bulk copy per channel row plus
+  // one for the chunk's table slice, landing in stage k % nstages and signalling full[stage] with the
+  // byte count.  A warp issues chunk k when it starts iteration k - ahead (ahead = nstages - 2): the
+  // stage it refills was consumed two iterations ago, so the wait on its empty barrier is normally
+  // already satisfied.  Row start and length of the warp's NEXT chunk are fetched one turn early.
+  const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T;
+  const long long tab = (long long)blk * p.Cpad;
+  const char* meta_blk = reinterpret_cast<const char*>(p.meta) + (size_t)blk * (size_t)nchunks * meta_bytes;
+  const int lane = tid & 31;
+  const int warp = tid >> 5;
+  constexpr int kWarps = NT / 32;
+  const int ahead = nstages - 2;
+  int pf_d0 = 0;
+  uint32_t pf_bytes = 0;
+  auto prefetch = [&](int k) {
+    pf_bytes = 0;
+    if (k < nchunks && lane < p.Cc) {
+      const int c = k * p.Cc + lane;
+      pf_d0 = __ldg(p.dmin + tab + c);
+      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
+    }
+  };
+  // stage and wrap count of a chunk index are tracked incrementally (no divisions in the main loop)
+  auto produce = [&](int k, int s, uint32_t wraps) {  // s = k % nstages, wraps = k / nstages
+    if (wraps > 0) mbar_wait(bar_base + 8u * (nstages + s), (wraps & 1u) ^ 1u);
+    const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
+    const uint32_t full = bar_base + 8u * s;
+    uint32_t total = pf_bytes;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
+    if (lane == 0) {
+      mbar_arrive_expect_tx(full, total + meta_bytes);
+      bulk_copy_g2s(sbase + data_bytes, meta_blk + (size_t)k * meta_bytes, meta_bytes, full);
+    }
+    __syncwarp();
+    if (lane < p.Cc)
+      bulk_copy_g2s(sbase + lane * row_bytes, Pbeam + (long long)(k * p.Cc + lane) * p.Wp + pf_d0, pf_bytes, full);
+  };
+  // this warp's chunks are warp, warp + kWarps, ...; (my_k, my_s, my_w) is the next one it has to issue
+  int my_k = warp, my_s = warp % nstages;
+  uint32_t my_w = (uint32_t)(warp / nstages);
+  const int s_step = kWarps % nstages;
+  const uint32_t w_step = (uint32_t)(kWarps / nstages);
+  auto advance = [&]() {
+    my_k += kWarps;
+    my_s += s_step;
+    my_w += w_step;
+    if (my_s >= nstages) {
+      my_s -= nstages;
+      ++my_w;
+    }
+  };
+  // prologue: chunks 0 .. ahead-1
+  while (my_k < ahead && my_k < nchunks) {
+    prefetch(my_k);
+    produce(my_k, my_s, my_w);
+    advance();
+  }
+  prefetch(my_k);  // first chunk this warp issues inside the loop
+
+  // ---------------- consumers: kRD trials x one superword (NL time lanes) per thread --------------
+  const int g = tid / p.T;       // trial group inside the CTA (warp-uniform: T is a multiple of 32)
+  const int ti = tid - g * p.T;  // superword inside the time tile
+  uint4 acc[kRD], hi[NL == 8 ? kRD : 1];
+#pragma unroll
+  for (int j = 0; j < kRD; ++j) acc[j] = make_uint4(0, 0, 0, 0);
+#pragma unroll
+  for (int j = 0; j < (NL == 8 ? kRD : 1); ++j) hi[j] = make_uint4(0, 0, 0, 0);
+  const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
+  const uint32_t meta_row = (uint32_t)p.G * 16u;  // bytes between consecutive channels (quads) of the table
+  const uint32_t meta_off = data_bytes + (uint32_t)g * 16u;
+  int since_flush = 0;
+
+  int s = 0;        // stage of the chunk being consumed
+  uint32_t ph = 0;  // its full-barrier parity
+  for (int it = 0; it < nchunks; ++it) {
+    if (it + ahead == my_k && my_k < nchunks) {  // producer turn of this warp
+      produce(my_k, my_s, my_w);
+      advance();
+      prefetch(my_k);
+    }
+    mbar_wait(bar_base + 8u * s, ph);
+    const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
+    if constexpr (MODE == kModeDelta)
+      stage_delta(acc, sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row);
+    else
+      stage_general<MODE == kModeGeneralReuse>(acc, sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_base + 8u * (nstages + s));  // stage may be refilled
+    if (++s == nstages) {
+      s = 0;
+      ph ^= 1u;
+    }
+    if constexpr (NL == 8) {
+      if (++since_flush == p.flush_stages) {  // the 16-bit lanes could overflow next: move their upper bytes
+        since_flush = 0;
+#pragma unroll
+        for (int j = 0; j < kRD; ++j) {
+          hi[j].x += (acc[j].x >> 8) & 0x00ff00ffu;
+          hi[j].y += (acc[j].y >> 8) & 0x00ff00ffu;
+          hi[j].z += (acc[j].z >> 8) & 0x00ff00ffu;
+          hi[j].w += (acc[j].w >> 8) & 0x00ff00ffu;
+          acc[j].x &= 0x00ff00ffu;
+          acc[j].y &= 0x00ff00ffu;
+          acc[j].z &= 0x00ff00ffu;
+          acc[j].w &= 0x00ff00ffu;
+        }
+      }
+    }
+  }
+
+  // ---------------- a4: DM-time writer, fp32 (I2F rounds to nearest even) -------------------------
+  const long long i = tau * p.T + ti;
+  if (i >= p.H) return;
+  float* obase = p.out + (long long)beam * p.out_beam_stride;
+#pragma unroll
+  for (int j = 0; j < kRD; ++j) {
+    const int jj = (blk * p.G + g) * kRD + j;
+    if (jj >= p.ndm) break;
+    float* orow = obase + (long long)jj * p.pitch;
+    uint32_t v[NL];
+    if constexpr (NL == 8) {  // lane = lo + 256*hi
+      v[0] = (acc[j].x & 0xffffu) + ((hi[j].x & 0xffffu) << 8);
+      v[1] = (acc[j].x >> 16) + ((hi[j].x >> 16) << 8);
+      v[2] = (acc[j].y & 0xffffu) + ((hi[j].y & 0xffffu) << 8);
+      v[3] = (acc[j].y >> 16) + ((hi[j].y >> 16) << 8);
+      v[4] = (acc[j].z & 0xffffu) + ((hi[j].z & 0xffffu) << 8);
+      v[5] = (acc[j].z >> 16) + ((hi[j].z >> 16) << 8);
+      v[6] = (acc[j].w & 0xffffu) + ((hi[j].w & 0xffffu) << 8);
+      v[7] = (acc[j].w >> 16) + ((hi[j].w >> 16) << 8);
+    } else {
+      v[0] = acc[j].x;
+      v[1] = acc[j].y;
+      v[2] = acc[j].z;
+      v[3] = acc[j].w;
+    }
+#pragma unroll
+    for (int m = 0; m < NL; ++m) {
+      const long long t = i + (long long)m * p.H;
+      if (t < p.nout) orow[t] = __uint2float_rn(v[m]);  // consecutive threads -> consecutive floats
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// launcher
+// ------------------------------------------------------------------------------------------------
+template <int NL, int MODE, int NT>
+static cudaError_t launch_tiled_t(const TiledParams& tp, long long nctas, size_t smem, cudaStream_t stream) {
+  dd_tiled_kernel<NL, MODE, NT><<<(unsigned)nctas, NT, smem, stream>>>(tp);
+  return cudaGetLastError();
+}
+
+template <int NL, int MODE, int NT>
+static cudaError_t set_smem_t() {
+  return cudaFuncSetAttribute(dd_tiled_kernel<NL, MODE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+}
+
+#define DD_FOR_ALL_TILED(X)                                                                    \
+  X(8, kModeGeneral, 256) X(8, kModeGeneralReuse, 256) X(8, kModeDelta, 256)                   \
+  X(8, kModeGeneral, 512) X(8, kModeGeneralReuse, 512) X(8, kModeDelta, 512)                   \
+  X(4, kModeGeneral, 256) X(4, kModeGeneralReuse, 256) X(4, kModeDelta, 256)                   \
+  X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)
+
+cudaError_t configure_kernels(const dd_plan*) {
+  cudaError_t e;
+#define DD_CFG(NL, MODE, NT) \
+  if ((e = set_smem_t<NL, MODE, NT>()) != cudaSuccess) return e;
+  DD_FOR_ALL_TILED(DD_CFG)
+#undef DD_CFG
+  return cudaSuccess;
+}
+
+cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream) {
+  TiledParams tp;
+  tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset);
+  tp.meta = r.d_meta;
+  tp.dmin = r.d_dmin;
+  tp.span = r.d_span;
+  tp.out = out_dev + r.offset;
+  tp.out_beam_stride = p->beam_stride;
+  tp.pitch = r.pitch;
+  tp.Wp = r.Wp;
+  tp.H = r.H;
+  tp.nout = r.nout;
+  tp.ntau = r.ntau;
+  tp.ndm = r.ndm;
+  tp.Cpad = r.Cpad;
+  tp.G = r.G;
+  tp.T = r.T;
+  tp.Cc = r.Cc;
+  tp.nstages = r.stages;
+  tp.nblocks = r.nblocks;
+  tp.rowpitch = r.T + r.Smax;
+  tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;
+  const long long nctas = (long long)r.nblocks * r.ntau * p->nbeams;
+  if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+  const size_t smem = tiled_smem_bytes(r);
+  const int nt = r.G * r.T;
+#define DD_GO(NL_, MODE_, NT_) \
+  if (r.NL == NL_ && r.mode == MODE_ && nt == NT_) return launch_tiled_t<NL_, MODE_, NT_>(tp, nctas, smem, stream);
+  DD_FOR_ALL_TILED(DD_GO)
+#undef DD_GO
+  return cudaErrorInvalidConfiguration;
+}
+
+}  // namespace dd

@@ -41,7 +41,7 @@ def test_cfg3_shaped_multirange_decimation(variant):
     plan, flat = gpu_run(w, x, variant)
     check_full(w, x, plan, flat)
     if variant == TILED:
-        assert plan.tile_info(0)["lanes"] == 8 and plan.tile_info(0)["reuse"] == 1
+        assert plan.tile_info(0)["lanes"] == 8 and plan.tile_info(0)["mode"] == 2
 
 
 @pytest.mark.parametrize("variant", [DIRECT, TILED])
