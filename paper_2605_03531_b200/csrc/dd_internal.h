@@ -33,6 +33,10 @@ enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2 };
 // for trial step j = 1..kRD-1 of channel q = 0..3.
 __host__ __device__ constexpr int delta_bit(int j, int q) { return (((j - 1) * 4 + q) / 7) * 8 + ((j - 1) * 4 + q) % 7; }
 
+// Staged rows start and end on 128-byte lines (8 superwords): upper bound of the staged length beyond T
+// for a block whose delays spread over `spread` superwords.
+__host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 + 7) / 8 * 8; }
+
 // Meta bytes per pipeline stage of Cc channels and G trial groups.
 __host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int Cc, int G) {
   return (size_t)(mode == kModeDelta ? Cc / 4 : Cc) * (size_t)G * 16;
@@ -65,7 +69,7 @@ struct RangePlan {
   size_t smem_bytes = 0;
   // device tables
   uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] kRD 16-bit offsets (delay - dmin, superwords);
-                                // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, 0}
+                                // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits}
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
   int32_t* d_delays = nullptr;  // [ndm][nchans], only for the direct kernel (lazy)

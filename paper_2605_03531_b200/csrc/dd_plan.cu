@@ -124,8 +124,9 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
       smax = std::max(smax, block_spread(p, r, b, D, p.nchans - 1));
       for (int c = 0; c < p.nchans; c += cstep, ++nsamp) ssum += block_spread(p, r, b, D, c);
     }
+    smax = dd::aligned_span(smax);
     if (T + smax > 65535) continue;  // 16-bit offsets
-    const double smean = ssum / std::max(1, nsamp);
+    const double smean = ssum / std::max(1, nsamp) + 7.0;  // rows start and end on 128-byte lines
     for (int Cc : {32, 16, 8, 4}) {
       if (r.NL == 8 && Cc > r.flush) continue;
       const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, Cc, G);
@@ -164,19 +165,22 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   if (r.NL == 8) r.flush = r.flush / r.Cc * r.Cc;
   r.Smax = 0;
   for (int b = 0; b < r.nblocks; ++b) r.Smax = std::max(r.Smax, block_spread(p, r, b, r.Dcta, p.nchans - 1));
+  r.Smax = dd::aligned_span(r.Smax);
   if (r.T + r.Smax > 65535) r.tiled_ok = 0;
   while (r.stages > 2 && dd::tiled_smem_bytes(r) > (size_t)227 * 1024) --r.stages;
   r.H = round_up((r.nout + r.NL - 1) / r.NL, 16);
   r.ntau = (r.H + r.T - 1) / r.T;
-  r.Wp = round_up(r.ntau * r.T + r.maxd, 4);
+  r.Wp = round_up(r.ntau * r.T + r.maxd + 8, 8);  // rows are 128-byte multiples; +8: staged rows end on a line
   r.ws_bytes = (int64_t)p.nbeams * r.Cpad * r.Wp * dd::kSuperwordBytes;
   r.smem_bytes = dd::tiled_smem_bytes(r);
   if (r.smem_bytes > (size_t)227 * 1024) r.tiled_ok = 0;
   if (!r.tiled_ok) r.ws_bytes = 0;
 }
 
-// Device tables of the tiled kernel: per trial block and channel the first delay (start of the staged
-// row) and the spread (length of the staged row beyond T); per trial group the offsets into the row in
+// Device tables of the tiled kernel: per trial block and channel the start of the staged row (the first
+// delay of the block rounded down to a 128-byte line: bulk copies whose source and destination are both
+// line-aligned fill shared memory a line per wavefront, misaligned ones 16 bytes at a time -- ncu,
+// profiles/) and its length beyond T (rounded up likewise); per trial group the offsets into the row in
 // the form the range's mode wants (dd_internal.h).  Trials past the end of the range repeat the last one;
 // rows past nchans (zero rows of the packed input) keep offset 0.
 int upload_tables(const dd_plan& p, dd::RangePlan& r) {
@@ -189,9 +193,9 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
   for (int b = 0; b < r.nblocks; ++b) {
     const int j0 = b * r.Dcta;
     for (int c = 0; c < p.nchans; ++c) {
-      const int32_t d0 = delay(j0, c);
+      const int32_t d0 = delay(j0, c) & ~7;  // delays are non-decreasing in j
       dmin[(size_t)b * r.Cpad + c] = d0;
-      span[(size_t)b * r.Cpad + c] = delay(j0 + r.Dcta - 1, c) - d0;  // delays are non-decreasing in j
+      span[(size_t)b * r.Cpad + c] = (int32_t)round_up(delay(j0 + r.Dcta - 1, c) - d0, 8);
       for (int g = 0; g < r.G; ++g) {
         const int jg = j0 + g * dd::kRD;
         if (delta) {
@@ -199,7 +203,10 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
           const int q = c % 4;
           e[1 + q / 2] |= (uint32_t)(delay(jg, c) - d0) << (16 * (q % 2));
           for (int j = 1; j < dd::kRD; ++j)
-            if (delay(jg + j, c) != delay(jg + j - 1, c)) e[0] |= 1u << dd::delta_bit(j, q);
+            if (delay(jg + j, c) != delay(jg + j - 1, c)) {
+              e[0] |= 1u << dd::delta_bit(j, q);
+              e[3] |= 1u << j;  // some channel of the quad changes at this trial step
+            }
         } else {
           uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * 4];
           for (int j = 0; j < dd::kRD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));

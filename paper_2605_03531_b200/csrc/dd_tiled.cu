@@ -70,7 +70,7 @@ __device__ __forceinline__ void lds_if_ne(uint4& w, uint32_t addr, uint32_t off,
       : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w)
       : "r"(addr), "r"(off), "r"(prev));
 }
-// delta mode: if bit BIT of m is set, step one superword forward and reload
+// delta mode: if bit BIT of m is set, step one superword forward and reload in place
 template <int BIT>
 __device__ __forceinline__ void lds_if_bit(uint4& w, uint32_t& addr, uint32_t m) {
   asm volatile(
@@ -88,7 +88,6 @@ __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4
   acc.z = acc.z + a.z + b.z;
   acc.w = acc.w + a.w + b.w;
 }
-
 struct TiledParams {
   const uint4* P;       // packed input of this range [nbeams][Cpad][Wp]
   const uint4* meta;    // per trial block: offsets / changed bits (dd_internal.h RangePlan::d_meta)
@@ -102,7 +101,7 @@ struct TiledParams {
 };
 
 __host__ __device__ inline size_t tiled_stage_bytes(int mode, int Cc, int rowpitch, int G) {
-  return (size_t)Cc * (size_t)rowpitch * kSuperwordBytes + tiled_meta_bytes(mode, Cc, G);
+  return ((size_t)Cc * (size_t)rowpitch * kSuperwordBytes + tiled_meta_bytes(mode, Cc, G) + 127) / 128 * 128;
 }
 constexpr int kBarRegion = 128;  // bytes reserved for the mbarriers at the start of dynamic smem
 
@@ -152,18 +151,26 @@ __device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint32_t sdata,
   }
 }
 
-// delta mode: channels in quads A..D; one table entry per quad = {changed bits, offA|offB<<16, offC|offD<<16, -}
+// delta mode: channels in quads A..D; one table entry per quad =
+//   {changed bits (delta_bit), offA | offB<<16, offC | offD<<16, bit j: some channel of the quad changes at trial step j}
 template <int J>
 __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t& aa,
-                                            uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits) {
+                                            uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits, uint32_t any) {
   if constexpr (J < kRD) {
-    lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
-    lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
-    lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
-    lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
+    // A predicated-off LDS still occupies a slot of the shared-memory data pipe (ncu: one wavefront per
+    // skipped load, 36 % of the pipe in the first version), so the whole trial step of the quad is skipped
+    // by ONE branch on its "any channel changed" bit: neighbouring channels have nearly the same delay
+    // curve and almost always change at the same trial.  `any` sits in a uniform register (stage_delta),
+    // which makes this a BRA.U without reconvergence bookkeeping.
+    if (any & (1u << J)) {
+      lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
+      lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
+      lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
+      lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
+    }
     add_pair(acc[J], wa, wb);
     add_pair(acc[J], wc, wd);
-    delta_steps<J + 1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bits);
+    delta_steps<J + 1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bits, any);
   }
 }
 
@@ -186,7 +193,8 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
     lds_sw(wd, ad);
     add_pair(acc[0], wa, wb);
     add_pair(acc[0], wc, wd);
-    delta_steps<1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, m.x);
+    // the table entry is the same for the whole warp: a warp reduction hands it over in a uniform register
+    delta_steps<1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, m.x, __reduce_or_sync(0xffffffffu, m.w));
   }
 }
 
@@ -209,7 +217,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const uint32_t row_bytes = (uint32_t)p.rowpitch * kSuperwordBytes;
   const uint32_t data_bytes = (uint32_t)p.Cc * row_bytes;
   const uint32_t meta_bytes = (uint32_t)tiled_meta_bytes(MODE, p.Cc, p.G);
-  const uint32_t stage_bytes = data_bytes + meta_bytes;
+  const uint32_t stage_bytes = (uint32_t)tiled_stage_bytes(MODE, p.Cc, p.rowpitch, p.G);
   const uint32_t stage0 = bar_base + kBarRegion;
   const int nchunks = p.Cpad / p.Cc;
 
