@@ -129,6 +129,7 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
     const double smean = ssum / std::max(1, nsamp) + 7.0;  // rows start and end on 128-byte lines
     for (int Cc : {32, 16, 8, 4}) {
       if (r.NL == 8 && Cc > r.flush) continue;
+      if (r.mode == dd::kModeDelta && (size_t)Cc * (size_t)(T + smax) * 16 > 65536) continue;  // 16-bit byte offsets
       const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, Cc, G);
       const int stages = (int)std::min<size_t>(6, budget / stage);
       if (stages < (Cc >= 8 ? 3 : 2)) continue;
@@ -150,7 +151,8 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   if (const char* s = getenv("DD_TILE")) {
     int g, t, cc, st;
     if (sscanf(s, "%d,%d,%d,%d", &g, &t, &cc, &st) == 4 && (g * t == 256 || g * t == 512) && t % 32 == 0 &&
-        cc >= 4 && cc <= 32 && cc % 4 == 0 && st >= 2 && st <= 8 && (r.NL != 8 || cc <= r.flush)) {
+        cc >= 4 && cc <= 32 && cc % 4 == 0 && st >= 2 && st <= 8 && (r.NL != 8 || cc <= r.flush) &&
+        (r.mode != dd::kModeDelta || (size_t)cc * (size_t)(t + 8 * g + 14) * 16 <= 65536)) {
       bc = {g, t, cc, st};
       r.tiled_ok = 1;
     }
@@ -181,18 +183,18 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
 // delay of the block rounded down to a 128-byte line: bulk copies whose source and destination are both
 // line-aligned fill shared memory a line per wavefront, misaligned ones 16 bytes at a time -- ncu,
 // profiles/) and its length beyond T (rounded up likewise); per trial group the offsets into the row in
-// the form the range's mode wants (dd_internal.h).  Trials past the end of the range repeat the last one;
-// rows past nchans (zero rows of the packed input) keep offset 0.
+// the form the range's mode wants (dd_internal.h).  Trials past the end of the range repeat the last one.
 int upload_tables(const dd_plan& p, dd::RangePlan& r) {
   const size_t nbc = (size_t)r.nblocks * r.Cpad;
   std::vector<int32_t> dmin(nbc, 0), span(nbc, 0);
   const bool delta = r.mode == dd::kModeDelta;
   const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
   std::vector<uint32_t> meta(nentries * 4, 0);
-  auto delay = [&](int j, int c) { return r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c]; };
+  // rows past nchans are the zero rows of the packed input: delay 0 for every trial
+  auto delay = [&](int j, int c) { return c < p.nchans ? r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c] : 0; };
   for (int b = 0; b < r.nblocks; ++b) {
     const int j0 = b * r.Dcta;
-    for (int c = 0; c < p.nchans; ++c) {
+    for (int c = 0; c < r.Cpad; ++c) {
       const int32_t d0 = delay(j0, c) & ~7;  // delays are non-decreasing in j
       dmin[(size_t)b * r.Cpad + c] = d0;
       span[(size_t)b * r.Cpad + c] = (int32_t)round_up(delay(j0 + r.Dcta - 1, c) - d0, 8);
@@ -201,7 +203,8 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
         if (delta) {
           uint32_t* e = &meta[(((size_t)b * (r.Cpad / 4) + c / 4) * r.G + g) * 4];
           const int q = c % 4;
-          e[1 + q / 2] |= (uint32_t)(delay(jg, c) - d0) << (16 * (q % 2));
+          const uint32_t off = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg, c) - d0)) * 16u;
+          e[1 + q / 2] |= off << (16 * (q % 2));  // byte offset inside the stage, < 64 KB (choose_tile)
           for (int j = 1; j < dd::kRD; ++j)
             if (delay(jg + j, c) != delay(jg + j - 1, c)) {
               e[0] |= 1u << dd::delta_bit(j, q);

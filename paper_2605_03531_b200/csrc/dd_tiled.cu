@@ -153,6 +153,7 @@ __device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint32_t sdata,
 
 // delta mode: channels in quads A..D; one table entry per quad =
 //   {changed bits (delta_bit), offA | offB<<16, offC | offD<<16, bit j: some channel of the quad changes at trial step j}
+// off = byte offset of the superword of the group's first trial, counted from the start of the stage
 template <int J>
 __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t& aa,
                                             uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits, uint32_t any) {
@@ -181,11 +182,12 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
     uint4 m;
     lds_sw(m, smeta);
     smeta += meta_row;
-    uint32_t aa = sdata + (m.y & 0xffffu) * kSuperwordBytes;
-    uint32_t ab = sdata + row_bytes + (m.y >> 16) * kSuperwordBytes;
-    uint32_t ac = sdata + 2 * row_bytes + (m.z & 0xffffu) * kSuperwordBytes;
-    uint32_t ad = sdata + 3 * row_bytes + (m.z >> 16) * kSuperwordBytes;
-    sdata += 4 * row_bytes;
+    // byte offsets inside the stage, row of the channel included (16 bits each: choose_tile keeps the data
+    // of a delta-mode stage below 64 KB)
+    uint32_t aa = sdata + (m.y & 0xffffu);
+    uint32_t ab = sdata + (m.y >> 16);
+    uint32_t ac = sdata + (m.z & 0xffffu);
+    uint32_t ad = sdata + (m.z >> 16);
     uint4 wa, wb, wc, wd;
     lds_sw(wa, aa);
     lds_sw(wb, ab);
