@@ -175,3 +175,71 @@ def test_host_path_and_caller_workspace():
     s.synchronize()
     check_full(w, x, plan, out.cpu().numpy(), want)
     assert plan.launches() == 4
+
+
+# ---- kernel v2: table modes, tile shapes, two-level packed accumulators ---------------------------------
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_table_modes_agree_on_fine_dm_grid(mode, monkeypatch):
+    """A fine DM grid (every delay step 0 or 1) run through each table form of the tiled kernel:
+    0 = one load per trial, 1 = load skipped on equal offsets, 2 = delta bits + uniform skip branch."""
+    monkeypatch.setenv("DD_MODE", str(mode))
+    w = W.scaled(W.CONFIGS[3], nchans=260, nsamps=2 ** 14 + 5,
+                 ranges=[W.DMRange(0.0, 0.1, 150, 1), W.DMRange(600.0, 0.5, 75, 4)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, TILED)
+    assert plan.tile_info(0)["mode"] == mode
+    check_full(w, x, plan, flat)
+
+
+def test_delta_mode_is_refused_for_coarse_dm_grid(monkeypatch):
+    """Delay steps above 1 cannot be delta coded: the plan falls back to the offsets table."""
+    monkeypatch.setenv("DD_MODE", "2")
+    w = W.scaled(W.CONFIGS[2], nchans=64, nsamps=2 ** 14, ranges=[W.DMRange(0.0, 2.0, 40, 1)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, TILED)
+    assert plan.tile_info(0)["mode"] == 0
+    check_full(w, x, plan, flat)
+
+
+@pytest.mark.parametrize("tile", ["16,32,32,3", "16,32,4,6", "8,64,16,4", "4,128,8,3", "2,256,8,2", "1,512,4,2",
+                                  "8,32,16,4", "4,64,8,5", "1,256,8,2"])
+def test_tile_shapes(tile, monkeypatch):
+    """Every CTA shape (trial groups x superwords, channels per stage, ring depth) gives the same bits."""
+    monkeypatch.setenv("DD_TILE", tile)
+    w = W.scaled(W.CONFIGS[3], nchans=100, nsamps=2 ** 15 + 77,
+                 ranges=[W.DMRange(0.0, 0.1, 77, 1), W.DMRange(50.0, 1.5, 19, 2)])   # delta + offsets tables
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, TILED)
+    g, t = (int(v) for v in tile.split(",")[:2])
+    assert plan.tile_info(0)["dm_per_cta"] == 8 * g and plan.tile_info(0)["words_per_cta"] == t
+    check_full(w, x, plan, flat)
+
+
+def test_packed_lane_residual_plus_saturated_interval():
+    """Two-level accumulators: lanes keep their low byte at a flush, so the next interval starts from up to
+    255.  First 256 channels sum to 255 (mod 256 = 255), the next 256 are saturated: 255 + 256*255 = 65535
+    is the exact lane bound."""
+    nch, ns = 768, 6000
+    x = np.zeros((1, nch, ns), dtype=np.uint8)
+    x[0, 0, :] = 255
+    x[0, 256:512, :] = 255
+    x[0, 512:, :] = 7
+    x[0, 300, 1000:1100] = 3
+    w = W.Workload("resid", 750.0, -200.0 / nch, nch, 1.31072e-3, ns, 1, 8, (W.DMRange(0.0, 0.2, 19, 1),), 1, 0, 0)
+    plan, flat = gpu_run(w, x, TILED)
+    assert plan.tile_info(0)["lanes"] == 8 and plan.tile_info(0)["flush_chans"] == 256
+    check_full(w, x, plan, flat)
+
+
+def test_many_flushes_and_wide_fallback():
+    """uint8 x8 decimation: lanes hold at most 32 saturated channels between flushes.  3840 channels = 120
+    flushes of the upper bytes (the 16-bit lane bound allows 256); 3872 channels go to 32-bit lanes."""
+    for nch, lanes in ((3840, 8), (3872, 4)):
+        ns = 8 * 700
+        x = np.full((1, nch, ns), 255, dtype=np.uint8)
+        x[0, 5::97, :] = 254
+        w = W.Workload("flushes", 750.0, -200.0 / nch, nch, 1.31072e-3, ns, 1, 8, (W.DMRange(0.0, 10.0, 9, 8),), 1, 0, 0)
+        plan, flat = gpu_run(w, x, TILED)
+        assert plan.tile_info(0)["lanes"] == lanes
+        check_full(w, x, plan, flat)
