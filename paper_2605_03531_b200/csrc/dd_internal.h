@@ -13,12 +13,17 @@ namespace dd {
 
 // Packed time word ("superword"): 16 bytes holding NL time lanes of one channel.
 //   lane m of superword i is the decimated sample y[i + m*H]   (H = lane segment length)
+//   NL = 16: sixteen 8-bit lanes (byte k of word q holds lane 4q+k); undecimated ranges whose delay steps
+//            are too coarse for the delta table.  uint16 input is split into two such byte planes (low and
+//            high byte) that are dedispersed one after the other: S = S_lo + 256*S_hi.
 //   NL = 8: eight 16-bit lanes (word q holds lanes 2q (low half) and 2q+1 (high half))
 //   NL = 4: four 32-bit lanes
 // A delay of d samples is a shift of d superwords for every lane at once, so any delay is a
 // 16-byte aligned access.
 constexpr int kSuperwordBytes = 16;
-constexpr int kRD = 8;            // trials register-blocked per thread (one "trial group")
+constexpr int kRD = 8;            // trials register-blocked per thread (one "trial group"), NL = 8 and 4
+constexpr int kRD16 = 4;          // the same for NL = 16 (twice the accumulator registers per trial)
+__host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? kRD16 : kRD; }
 
 // How the tiled kernel finds the staged superword of (channel, trial):
 //   kModeGeneral       per channel and trial group: kRD 16-bit superword offsets, one shared-memory load per trial
@@ -37,9 +42,10 @@ __host__ __device__ constexpr int delta_bit(int j, int q) { return (((j - 1) * 4
 // for a block whose delays spread over `spread` superwords.
 __host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 + 7) / 8 * 8; }
 
-// Meta bytes per pipeline stage of Cc channels and G trial groups.
-__host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int Cc, int G) {
-  return (size_t)(mode == kModeDelta ? Cc / 4 : Cc) * (size_t)G * 16;
+// Meta bytes per pipeline stage of Cc channels and G trial groups: one 16-bit superword offset per
+// (channel, trial), or one 16-byte entry per channel quad in delta mode.
+__host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int NL, int Cc, int G) {
+  return mode == kModeDelta ? (size_t)(Cc / 4) * (size_t)G * 16 : (size_t)Cc * (size_t)G * 2 * trials_per_thread(NL);
 }
 
 struct RangePlan {
@@ -50,6 +56,9 @@ struct RangePlan {
   std::vector<int32_t> delays;  // host copy [ndm][nchans]
   // tiled kernel shape
   int NL = 8;        // lanes per superword
+  int RD = 8;        // trials per thread = trials_per_thread(NL)
+  int planes = 1;    // 2: uint16 input as low-byte and high-byte planes (NL = 16)
+  int64_t plane_bytes = 0;  // bytes of one packed plane in the workspace
   int flush = 0;     // channels between flushes of the 16-bit lanes (0: never, 32-bit lanes)
   int mode = 0;      // TiledMode
   int G = 0;         // trial groups per CTA (kRD trials each)
@@ -68,7 +77,7 @@ struct RangePlan {
   int64_t ws_bytes = 0;
   size_t smem_bytes = 0;
   // device tables
-  uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] kRD 16-bit offsets (delay - dmin, superwords);
+  uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] RD 16-bit offsets (delay - dmin, superwords);
                                 // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits}
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
@@ -105,7 +114,7 @@ namespace dd {
 
 // launchers (dd_kernels.cu); all enqueue on `stream` and return the CUDA error of the launch
 cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream);
-cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream);
+cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream);  // all planes
 cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_dev, float* out_dev,
                           cudaStream_t stream);
 cudaError_t configure_kernels(const dd_plan* p);  // opt in to the dynamic shared memory sizes

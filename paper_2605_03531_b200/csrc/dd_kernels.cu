@@ -121,7 +121,74 @@ static cudaError_t launch_pack_t(const dd_plan* p, const RangePlan& r, const voi
   return cudaGetLastError();
 }
 
+// a2 for 8-bit lanes (NL = 16), undecimated input.  Thread = 4 consecutive superwords i0..i0+3 of one
+// (beam, channel) row; byte k of word q of superword i is x[i + (4q+k)*H] (0 past the end of the row).  uint16
+// samples go to two planes of this form: plane 0 their low bytes, plane 1 their high bytes.
+template <typename Tin>
+__global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restrict__ in, uint4* __restrict__ P0,
+                                                            uint4* __restrict__ P1, int nchans, int Cpad, int64_t nsamps,
+                                                            int64_t H, int64_t Wp) {
+  const int64_t i0 = 4 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+  if (i0 >= Wp) return;
+  const int c = blockIdx.y;
+  const int beam = blockIdx.z;
+  const int64_t o = ((int64_t)beam * Cpad + c) * Wp + i0;
+  constexpr bool kTwo = sizeof(Tin) == 2;
+  if (c >= nchans) {  // zero rows that pad the channel count to a multiple of the stage size
+    const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      P0[o + e] = z;
+      if (kTwo) P1[o + e] = z;
+    }
+    return;
+  }
+  const Tin* row = in + ((int64_t)beam * nchans + c) * nsamps;
+  uint32_t lo[4][4] = {}, hi[4][4] = {};  // [superword e][word q]
+#pragma unroll
+  for (int m = 0; m < 16; ++m) {
+    const int64_t s = i0 + (int64_t)m * H;
+    uint32_t v[4];
+    const Tin* src = row + s;
+    if (s + 4 <= nsamps && (reinterpret_cast<uintptr_t>(src) & (4 * sizeof(Tin) - 1)) == 0) {
+      if constexpr (kTwo) {
+        const uint2 t = __ldg(reinterpret_cast<const uint2*>(src));
+        v[0] = t.x & 0xffffu, v[1] = t.x >> 16, v[2] = t.y & 0xffffu, v[3] = t.y >> 16;
+      } else {
+        const uint32_t t = __ldg(reinterpret_cast<const uint32_t*>(src));
+        v[0] = t & 0xffu, v[1] = (t >> 8) & 0xffu, v[2] = (t >> 16) & 0xffu, v[3] = t >> 24;
+      }
+    } else {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) v[e] = s + e < nsamps ? (uint32_t)row[s + e] : 0u;
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      lo[e][m / 4] |= (v[e] & 0xffu) << (8 * (m % 4));
+      if (kTwo) hi[e][m / 4] |= (v[e] >> 8) << (8 * (m % 4));
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < 4; ++e) {
+    P0[o + e] = make_uint4(lo[e][0], lo[e][1], lo[e][2], lo[e][3]);
+    if (kTwo) P1[o + e] = make_uint4(hi[e][0], hi[e][1], hi[e][2], hi[e][3]);
+  }
+}
+
 cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream) {
+  if (r.NL == 16) {
+    uint4* P0 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset);
+    uint4* P1 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset + r.plane_bytes);
+    dim3 block(256);
+    dim3 grid((unsigned)((r.Wp / 4 + 255) / 256), (unsigned)r.Cpad, (unsigned)p->nbeams);
+    if (p->in_bits == 8)
+      dd_pack_bytes_kernel<uint8_t><<<grid, block, 0, stream>>>(static_cast<const uint8_t*>(in_dev), P0, nullptr, p->nchans,
+                                                                r.Cpad, p->nsamps, r.H, r.Wp);
+    else
+      dd_pack_bytes_kernel<uint16_t><<<grid, block, 0, stream>>>(static_cast<const uint16_t*>(in_dev), P0, P1, p->nchans,
+                                                                 r.Cpad, p->nsamps, r.H, r.Wp);
+    return cudaGetLastError();
+  }
   if (p->in_bits == 8) {
     return r.NL == 8 ? launch_pack_t<uint8_t, 8>(p, r, in_dev, stream) : launch_pack_t<uint8_t, 4>(p, r, in_dev, stream);
   }

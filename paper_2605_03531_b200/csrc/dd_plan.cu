@@ -108,13 +108,24 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
     r.flush = 0;
   }
   r.mode = choose_mode(p, r);
+  // Undecimated ranges that cannot use the delta table run on 8-bit lanes: half the shared-memory traffic per
+  // sample (the bound of the offsets-table modes), uint16 input as two byte planes.  DD_BYTES=0 switches it off
+  // (measurements only).
+  const int flush16 = 65280 / 255;
+  if (r.decim == 1 && r.mode != dd::kModeDelta && (int64_t)p.nchans <= (int64_t)120 * flush16 && env_int("DD_BYTES", 1)) {
+    r.NL = 16;
+    r.flush = flush16;
+    r.mode = dd::kModeGeneral;
+    r.planes = p.in_bits / 8;
+  }
+  r.RD = dd::trials_per_thread(r.NL);
   static const int cand[][2] = {{16, 32}, {8, 64}, {4, 128}, {2, 256}, {1, 512}, {8, 32}, {4, 64}, {2, 128}, {1, 256}};
   const size_t budget = 200 * 1024;
   double best = 1e300;
   TileChoice bc = {1, 256, 4, 2};
   bool found = false;
   for (auto& gt : cand) {
-    const int G = gt[0], T = gt[1], D = G * dd::kRD;
+    const int G = gt[0], T = gt[1], D = G * r.RD;
     const int nblocks = (r.ndm + D - 1) / D;
     int smax = 0;
     double ssum = 0;
@@ -128,13 +139,13 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
     if (T + smax > 65535) continue;  // 16-bit offsets
     const double smean = ssum / std::max(1, nsamp) + 7.0;  // rows start and end on 128-byte lines
     for (int Cc : {32, 16, 8, 4}) {
-      if (r.NL == 8 && Cc > r.flush) continue;
+      if (r.flush > 0 && Cc > r.flush) continue;
       if (r.mode == dd::kModeDelta && (size_t)Cc * (size_t)(T + smax) * 16 > 65536) continue;  // 16-bit byte offsets
-      const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, Cc, G);
+      const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, r.NL, Cc, G);
       const int stages = (int)std::min<size_t>(6, budget / stage);
       if (stages < (Cc >= 8 ? 3 : 2)) continue;
       // bytes staged per add: row (T + mean spread) superwords + the table row, over T*NL*D adds
-      double cost = ((T + smean) * 16.0 + dd::tiled_meta_bytes(r.mode, 4, G) / 4.0) / ((double)T * r.NL * D);
+      double cost = ((T + smean) * 16.0 + dd::tiled_meta_bytes(r.mode, r.NL, 4, G) / 4.0) / ((double)T * r.NL * D);
       // trials past the end of the last block are computed and dropped
       cost *= (double)nblocks * D / (double)r.ndm;
       if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
@@ -151,7 +162,7 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   if (const char* s = getenv("DD_TILE")) {
     int g, t, cc, st;
     if (sscanf(s, "%d,%d,%d,%d", &g, &t, &cc, &st) == 4 && (g * t == 256 || g * t == 512) && t % 32 == 0 &&
-        cc >= 4 && cc <= 32 && cc % 4 == 0 && st >= 2 && st <= 8 && (r.NL != 8 || cc <= r.flush) &&
+        cc >= 4 && cc <= 32 && cc % 4 == 0 && st >= 2 && st <= 8 && (r.flush == 0 || cc <= r.flush) &&
         (r.mode != dd::kModeDelta || (size_t)cc * (size_t)(t + 8 * g + 14) * 16 <= 65536)) {
       bc = {g, t, cc, st};
       r.tiled_ok = 1;
@@ -161,10 +172,10 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   r.T = bc.T;
   r.Cc = bc.Cc;
   r.stages = bc.stages;
-  r.Dcta = r.G * dd::kRD;
+  r.Dcta = r.G * r.RD;
   r.nblocks = (r.ndm + r.Dcta - 1) / r.Dcta;
   r.Cpad = (int)round_up(p.nchans, r.Cc);
-  if (r.NL == 8) r.flush = r.flush / r.Cc * r.Cc;
+  if (r.flush > 0) r.flush = r.flush / r.Cc * r.Cc;
   r.Smax = 0;
   for (int b = 0; b < r.nblocks; ++b) r.Smax = std::max(r.Smax, block_spread(p, r, b, r.Dcta, p.nchans - 1));
   r.Smax = dd::aligned_span(r.Smax);
@@ -173,7 +184,8 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   r.H = round_up((r.nout + r.NL - 1) / r.NL, 16);
   r.ntau = (r.H + r.T - 1) / r.T;
   r.Wp = round_up(r.ntau * r.T + r.maxd + 8, 8);  // rows are 128-byte multiples; +8: staged rows end on a line
-  r.ws_bytes = (int64_t)p.nbeams * r.Cpad * r.Wp * dd::kSuperwordBytes;
+  r.plane_bytes = round_up((int64_t)p.nbeams * r.Cpad * r.Wp * dd::kSuperwordBytes, 256);
+  r.ws_bytes = r.plane_bytes * r.planes;
   r.smem_bytes = dd::tiled_smem_bytes(r);
   if (r.smem_bytes > (size_t)227 * 1024) r.tiled_ok = 0;
   if (!r.tiled_ok) r.ws_bytes = 0;
@@ -188,8 +200,9 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
   const size_t nbc = (size_t)r.nblocks * r.Cpad;
   std::vector<int32_t> dmin(nbc, 0), span(nbc, 0);
   const bool delta = r.mode == dd::kModeDelta;
+  const size_t words_per_entry = delta ? 4 : r.RD / 2;  // 16-bit offsets, two per word
   const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
-  std::vector<uint32_t> meta(nentries * 4, 0);
+  std::vector<uint32_t> meta(nentries * words_per_entry, 0);
   // rows past nchans are the zero rows of the packed input: delay 0 for every trial
   auto delay = [&](int j, int c) { return c < p.nchans ? r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c] : 0; };
   for (int b = 0; b < r.nblocks; ++b) {
@@ -199,20 +212,20 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
       dmin[(size_t)b * r.Cpad + c] = d0;
       span[(size_t)b * r.Cpad + c] = (int32_t)round_up(delay(j0 + r.Dcta - 1, c) - d0, 8);
       for (int g = 0; g < r.G; ++g) {
-        const int jg = j0 + g * dd::kRD;
+        const int jg = j0 + g * r.RD;
         if (delta) {
           uint32_t* e = &meta[(((size_t)b * (r.Cpad / 4) + c / 4) * r.G + g) * 4];
           const int q = c % 4;
           const uint32_t off = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg, c) - d0)) * 16u;
           e[1 + q / 2] |= off << (16 * (q % 2));  // byte offset inside the stage, < 64 KB (choose_tile)
-          for (int j = 1; j < dd::kRD; ++j)
+          for (int j = 1; j < r.RD; ++j)
             if (delay(jg + j, c) != delay(jg + j - 1, c)) {
               e[0] |= 1u << dd::delta_bit(j, q);
               e[3] |= 1u << j;  // some channel of the quad changes at this trial step
             }
         } else {
-          uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * 4];
-          for (int j = 0; j < dd::kRD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));
+          uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * words_per_entry];
+          for (int j = 0; j < r.RD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));
         }
       }
     }
@@ -479,7 +492,7 @@ int dd_plan_work(const dd_plan_t* p, int64_t* dm_samples, int64_t* adds) {
 int dd_plan_launches(const dd_plan_t* p, int32_t* n) {
   if (!p || !n) return DD_ERR_INVALID;
   int k = 0;
-  for (const auto& r : p->ranges) k += (p->variant == DD_KERNEL_DIRECT || !r.tiled_ok) ? 1 : 2;
+  for (const auto& r : p->ranges) k += (p->variant == DD_KERNEL_DIRECT || !r.tiled_ok) ? 1 : 1 + r.planes;
   *n = k;
   return DD_OK;
 }

@@ -97,16 +97,17 @@ struct TiledParams {
   long long out_beam_stride, pitch, Wp, H, nout, ntau;
   int ndm, Cpad, G, T, Cc, nstages, nblocks;
   int rowpitch;      // superwords per staged row = T + Smax
-  int flush_stages;  // move the upper bytes of the 16-bit lanes away every this many stages (NL == 8)
+  int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
+  float accum_scale;  // 0: store; else out = value * accum_scale + out (high byte plane of uint16 input)
 };
 
-__host__ __device__ inline size_t tiled_stage_bytes(int mode, int Cc, int rowpitch, int G) {
-  return ((size_t)Cc * (size_t)rowpitch * kSuperwordBytes + tiled_meta_bytes(mode, Cc, G) + 127) / 128 * 128;
+__host__ __device__ inline size_t tiled_stage_bytes(int mode, int NL, int Cc, int rowpitch, int G) {
+  return ((size_t)Cc * (size_t)rowpitch * kSuperwordBytes + tiled_meta_bytes(mode, NL, Cc, G) + 127) / 128 * 128;
 }
 constexpr int kBarRegion = 128;  // bytes reserved for the mbarriers at the start of dynamic smem
 
 size_t tiled_smem_bytes(const RangePlan& r) {
-  return kBarRegion + (size_t)r.stages * tiled_stage_bytes(r.mode, r.Cc, r.T + r.Smax, r.G);
+  return kBarRegion + (size_t)r.stages * tiled_stage_bytes(r.mode, r.NL, r.Cc, r.T + r.Smax, r.G);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -200,6 +201,153 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
   }
 }
 
+// 8-bit lanes (NL = 16): channels in pairs, one table entry (kRD16 16-bit superword offsets) per channel.
+// A loaded word w holds the bytes b0..b3 of four time lanes.  Two accumulators per word:
+//   e += w & 0x00ff00ff            two 16-bit lanes: A0 | A2 << 16 (sums of b0 and b2)   LOP3 + half an IADD3 per channel
+//   r += w >> 8                    = A1 + 2^8 A2 + 2^16 A3  (mod 2^32)                    one LEA.HI per channel
+// A2 is known from e, so r - (A2 << 8) = A1 + 2^16 A3 separates exactly as long as every lane sum stays below
+// 2^16 (upper bytes moved out every 256 channels, as for the 16-bit lanes); wrap-around of r is harmless.
+// (Measured alternatives: the shift-add as IMAD.HI or IMAD.WIDE on the idle FMA pipe is slower -- ptxas adds
+// register moves or splits it into a multiply plus 64-bit adds.)
+__device__ __forceinline__ void add_bytes(uint4& e, uint4& r, const uint4& a, const uint4& b) {
+  e.x = e.x + (a.x & 0x00ff00ffu) + (b.x & 0x00ff00ffu);
+  e.y = e.y + (a.y & 0x00ff00ffu) + (b.y & 0x00ff00ffu);
+  e.z = e.z + (a.z & 0x00ff00ffu) + (b.z & 0x00ff00ffu);
+  e.w = e.w + (a.w & 0x00ff00ffu) + (b.w & 0x00ff00ffu);
+  r.x = r.x + (a.x >> 8) + (b.x >> 8);
+  r.y = r.y + (a.y >> 8) + (b.y >> 8);
+  r.z = r.z + (a.z >> 8) + (b.z >> 8);
+  r.w = r.w + (a.w >> 8) + (b.w >> 8);
+}
+
+__device__ __forceinline__ void stage_bytes(uint4 (&e)[kRD16], uint4 (&r)[kRD16], uint32_t sdata, uint32_t smeta, int Cc,
+                                            uint32_t row_bytes, uint32_t meta_row) {
+#pragma unroll 1
+  for (int cc = 0; cc < Cc; cc += 2) {
+    uint32_t ma0, ma1, mb0, mb1;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(ma0), "=r"(ma1) : "r"(smeta));
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(mb0), "=r"(mb1) : "r"(smeta + meta_row));
+    smeta += 2 * meta_row;
+    const uint32_t ra = sdata, rb = sdata + row_bytes;
+    sdata += 2 * row_bytes;
+#pragma unroll
+    for (int j = 0; j < kRD16; ++j) {
+      const uint32_t wa = j < 2 ? ma0 : ma1, wb = j < 2 ? mb0 : mb1;
+      const uint32_t oa = (j & 1) ? (wa >> 16) : (wa & 0xffffu), ob = (j & 1) ? (wb >> 16) : (wb & 0xffffu);
+      uint4 xa, xb;
+      lds_sw(xa, ra + oa * kSuperwordBytes);
+      lds_sw(xb, rb + ob * kSuperwordBytes);
+      add_bytes(e[j], r[j], xa, xb);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// per-thread accumulators of the three lane widths
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void carry_save(uint32_t& lo, uint32_t& hi) {  // 16-bit lanes: hi += lo >> 8, lo &= 0xff
+  hi += (lo >> 8) & 0x00ff00ffu;
+  lo &= 0x00ff00ffu;
+}
+__device__ __forceinline__ void carry_save(uint4& lo, uint4& hi) {
+  carry_save(lo.x, hi.x);
+  carry_save(lo.y, hi.y);
+  carry_save(lo.z, hi.z);
+  carry_save(lo.w, hi.w);
+}
+
+template <int NL>
+struct Lanes;
+
+template <>
+struct Lanes<4> {  // four 32-bit lanes: plain sums
+  uint4 acc[kRD];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int j = 0; j < kRD; ++j) acc[j] = make_uint4(0, 0, 0, 0);
+  }
+  template <int MODE>
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
+    if constexpr (MODE == kModeDelta)
+      stage_delta(acc, sdata, smeta, Cc, row_bytes, meta_row);
+    else
+      stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
+  }
+  __device__ __forceinline__ void flush() {}
+  __device__ __forceinline__ void values(int j, uint32_t (&v)[4]) const {
+    v[0] = acc[j].x, v[1] = acc[j].y, v[2] = acc[j].z, v[3] = acc[j].w;
+  }
+};
+
+template <>
+struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
+  uint4 acc[kRD], hi[kRD];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int j = 0; j < kRD; ++j) acc[j] = hi[j] = make_uint4(0, 0, 0, 0);
+  }
+  template <int MODE>
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
+    if constexpr (MODE == kModeDelta)
+      stage_delta(acc, sdata, smeta, Cc, row_bytes, meta_row);
+    else
+      stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
+  }
+  __device__ __forceinline__ void flush() {
+#pragma unroll
+    for (int j = 0; j < kRD; ++j) carry_save(acc[j], hi[j]);
+  }
+  __device__ __forceinline__ void values(int j, uint32_t (&v)[8]) const {
+    const uint32_t lo[4] = {acc[j].x, acc[j].y, acc[j].z, acc[j].w}, up[4] = {hi[j].x, hi[j].y, hi[j].z, hi[j].w};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      v[2 * q] = (lo[q] & 0xffffu) + ((up[q] & 0xffffu) << 8);
+      v[2 * q + 1] = (lo[q] >> 16) + ((up[q] >> 16) << 8);
+    }
+  }
+};
+
+template <>
+struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upper bytes moved out at each flush
+  uint4 e[kRD16], r[kRD16], he[kRD16], hq[kRD16];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int j = 0; j < kRD16; ++j) e[j] = r[j] = he[j] = hq[j] = make_uint4(0, 0, 0, 0);
+  }
+  template <int MODE>
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
+    stage_bytes(e, r, sdata, smeta, Cc, row_bytes, meta_row);
+  }
+  // invariant: e = A0 | A2 << 16,  r = A1 + 2^8 A2 + 2^16 A3 (mod 2^32),  lane sum = A + 256 * (he | hq lane)
+  static __device__ __forceinline__ void flush_word(uint32_t& e, uint32_t& r, uint32_t& he, uint32_t& hq) {
+    uint32_t q = r - ((e >> 16) << 8);  // A1 | A3 << 16
+    carry_save(e, he);
+    carry_save(q, hq);
+    r = q + ((e >> 16) << 8);
+  }
+  __device__ __forceinline__ void flush() {
+#pragma unroll
+    for (int j = 0; j < kRD16; ++j) {
+      flush_word(e[j].x, r[j].x, he[j].x, hq[j].x);
+      flush_word(e[j].y, r[j].y, he[j].y, hq[j].y);
+      flush_word(e[j].z, r[j].z, he[j].z, hq[j].z);
+      flush_word(e[j].w, r[j].w, he[j].w, hq[j].w);
+    }
+  }
+  __device__ __forceinline__ void values(int j, uint32_t (&v)[16]) const {
+    const uint32_t ew[4] = {e[j].x, e[j].y, e[j].z, e[j].w}, rw[4] = {r[j].x, r[j].y, r[j].z, r[j].w};
+    const uint32_t hew[4] = {he[j].x, he[j].y, he[j].z, he[j].w}, hqw[4] = {hq[j].x, hq[j].y, hq[j].z, hq[j].w};
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t q = rw[w] - ((ew[w] >> 16) << 8);
+      v[4 * w + 0] = (ew[w] & 0xffffu) + ((hew[w] & 0xffffu) << 8);
+      v[4 * w + 1] = (q & 0xffffu) + ((hqw[w] & 0xffffu) << 8);
+      v[4 * w + 2] = (ew[w] >> 16) + ((hew[w] >> 16) << 8);
+      v[4 * w + 3] = (q >> 16) + ((hqw[w] >> 16) << 8);
+    }
+  }
+};
+
 // ------------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------------
@@ -218,8 +366,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const int nstages = p.nstages;
   const uint32_t row_bytes = (uint32_t)p.rowpitch * kSuperwordBytes;
   const uint32_t data_bytes = (uint32_t)p.Cc * row_bytes;
-  const uint32_t meta_bytes = (uint32_t)tiled_meta_bytes(MODE, p.Cc, p.G);
-  const uint32_t stage_bytes = (uint32_t)tiled_stage_bytes(MODE, p.Cc, p.rowpitch, p.G);
+  const uint32_t meta_bytes = (uint32_t)tiled_meta_bytes(MODE, NL, p.Cc, p.G);
+  const uint32_t stage_bytes = (uint32_t)tiled_stage_bytes(MODE, NL, p.Cc, p.rowpitch, p.G);
   const uint32_t stage0 = bar_base + kBarRegion;
   const int nchunks = p.Cpad / p.Cc;
 
@@ -293,17 +441,16 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   }
   prefetch(my_k);  // first chunk this warp issues inside the loop
 
-  // ---------------- consumers: kRD trials x one superword (NL time lanes) per thread --------------
+  // ---------------- consumers: RD trials x one superword (NL time lanes) per thread --------------
+  constexpr int RD = trials_per_thread(NL);
   const int g = tid / p.T;       // trial group inside the CTA (warp-uniform: T is a multiple of 32)
   const int ti = tid - g * p.T;  // superword inside the time tile
-  uint4 acc[kRD], hi[NL == 8 ? kRD : 1];
-#pragma unroll
-  for (int j = 0; j < kRD; ++j) acc[j] = make_uint4(0, 0, 0, 0);
-#pragma unroll
-  for (int j = 0; j < (NL == 8 ? kRD : 1); ++j) hi[j] = make_uint4(0, 0, 0, 0);
+  Lanes<NL> lanes;
+  lanes.init();
   const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
-  const uint32_t meta_row = (uint32_t)p.G * 16u;  // bytes between consecutive channels (quads) of the table
-  const uint32_t meta_off = data_bytes + (uint32_t)g * 16u;
+  const uint32_t entry_bytes = MODE == kModeDelta ? 16u : 2u * RD;  // table bytes per (channel | quad, trial group)
+  const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
+  const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
 
   int s = 0;        // stage of the chunk being consumed
@@ -316,31 +463,16 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     }
     mbar_wait(bar_base + 8u * s, ph);
     const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
-    if constexpr (MODE == kModeDelta)
-      stage_delta(acc, sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row);
-    else
-      stage_general<MODE == kModeGeneralReuse>(acc, sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row);
+    lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row);
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_base + 8u * (nstages + s));  // stage may be refilled
     if (++s == nstages) {
       s = 0;
       ph ^= 1u;
     }
-    if constexpr (NL == 8) {
-      if (++since_flush == p.flush_stages) {  // the 16-bit lanes could overflow next: move their upper bytes
-        since_flush = 0;
-#pragma unroll
-        for (int j = 0; j < kRD; ++j) {
-          hi[j].x += (acc[j].x >> 8) & 0x00ff00ffu;
-          hi[j].y += (acc[j].y >> 8) & 0x00ff00ffu;
-          hi[j].z += (acc[j].z >> 8) & 0x00ff00ffu;
-          hi[j].w += (acc[j].w >> 8) & 0x00ff00ffu;
-          acc[j].x &= 0x00ff00ffu;
-          acc[j].y &= 0x00ff00ffu;
-          acc[j].z &= 0x00ff00ffu;
-          acc[j].w &= 0x00ff00ffu;
-        }
-      }
+    if (NL != 4 && ++since_flush == p.flush_stages) {  // packed lanes could overflow next: move their upper bytes
+      since_flush = 0;
+      lanes.flush();
     }
   }
 
@@ -349,30 +481,23 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   if (i >= p.H) return;
   float* obase = p.out + (long long)beam * p.out_beam_stride;
 #pragma unroll
-  for (int j = 0; j < kRD; ++j) {
-    const int jj = (blk * p.G + g) * kRD + j;
+  for (int j = 0; j < RD; ++j) {
+    const int jj = (blk * p.G + g) * RD + j;
     if (jj >= p.ndm) break;
     float* orow = obase + (long long)jj * p.pitch;
     uint32_t v[NL];
-    if constexpr (NL == 8) {  // lane = lo + 256*hi
-      v[0] = (acc[j].x & 0xffffu) + ((hi[j].x & 0xffffu) << 8);
-      v[1] = (acc[j].x >> 16) + ((hi[j].x >> 16) << 8);
-      v[2] = (acc[j].y & 0xffffu) + ((hi[j].y & 0xffffu) << 8);
-      v[3] = (acc[j].y >> 16) + ((hi[j].y >> 16) << 8);
-      v[4] = (acc[j].z & 0xffffu) + ((hi[j].z & 0xffffu) << 8);
-      v[5] = (acc[j].z >> 16) + ((hi[j].z >> 16) << 8);
-      v[6] = (acc[j].w & 0xffffu) + ((hi[j].w & 0xffffu) << 8);
-      v[7] = (acc[j].w >> 16) + ((hi[j].w >> 16) << 8);
-    } else {
-      v[0] = acc[j].x;
-      v[1] = acc[j].y;
-      v[2] = acc[j].z;
-      v[3] = acc[j].w;
-    }
+    lanes.values(j, v);
 #pragma unroll
     for (int m = 0; m < NL; ++m) {
-      const long long t = i + (long long)m * p.H;
-      if (t < p.nout) orow[t] = __uint2float_rn(v[m]);  // consecutive threads -> consecutive floats
+      const long long t = i + (long long)m * p.H;  // consecutive threads -> consecutive floats
+      if (t < p.nout) {
+        // second byte plane of uint16 input: S = S_lo + 256*S_hi.  Both plane sums are < 2^24, hence exact
+        // floats, and the fused multiply-add rounds the exact total once: fl32(S), as the definition asks.
+        if (p.accum_scale != 0.0f)
+          orow[t] = __fmaf_rn(__uint2float_rn(v[m]), p.accum_scale, orow[t]);
+        else
+          orow[t] = __uint2float_rn(v[m]);
+      }
     }
   }
 }
@@ -395,7 +520,8 @@ static cudaError_t set_smem_t() {
   X(8, kModeGeneral, 256) X(8, kModeGeneralReuse, 256) X(8, kModeDelta, 256)                   \
   X(8, kModeGeneral, 512) X(8, kModeGeneralReuse, 512) X(8, kModeDelta, 512)                   \
   X(4, kModeGeneral, 256) X(4, kModeGeneralReuse, 256) X(4, kModeDelta, 256)                   \
-  X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)
+  X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)                   \
+  X(16, kModeGeneral, 256) X(16, kModeGeneral, 512)
 
 cudaError_t configure_kernels(const dd_plan*) {
   cudaError_t e;
@@ -408,7 +534,6 @@ cudaError_t configure_kernels(const dd_plan*) {
 
 cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream) {
   TiledParams tp;
-  tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset);
   tp.meta = r.d_meta;
   tp.dmin = r.d_dmin;
   tp.span = r.d_span;
@@ -432,11 +557,18 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   const size_t smem = tiled_smem_bytes(r);
   const int nt = r.G * r.T;
+  // one launch per byte plane: low bytes stored, high bytes added with weight 256
+  for (int plane = 0; plane < r.planes; ++plane) {
+    tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset + plane * r.plane_bytes);
+    tp.accum_scale = plane == 0 ? 0.0f : 256.0f;
+    cudaError_t e = cudaErrorInvalidConfiguration;
 #define DD_GO(NL_, MODE_, NT_) \
-  if (r.NL == NL_ && r.mode == MODE_ && nt == NT_) return launch_tiled_t<NL_, MODE_, NT_>(tp, nctas, smem, stream);
-  DD_FOR_ALL_TILED(DD_GO)
+  if (r.NL == NL_ && r.mode == MODE_ && nt == NT_) e = launch_tiled_t<NL_, MODE_, NT_>(tp, nctas, smem, stream);
+    DD_FOR_ALL_TILED(DD_GO)
 #undef DD_GO
-  return cudaErrorInvalidConfiguration;
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 }  // namespace dd

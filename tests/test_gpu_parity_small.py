@@ -64,7 +64,8 @@ def test_cfg4_shaped_uint16(variant):
     assert want[0][0].max() > 2 ** 24        # the inexact regime is exercised
     plan, flat = gpu_run(w, x, variant)
     check_full(w, x, plan, flat, want)
-    assert plan.tile_info(0)["lanes"] == 4
+    if variant == TILED:   # x1 range: two byte planes of 8-bit lanes; x8 range: 32-bit lanes
+        assert plan.tile_info(0)["lanes"] == 16 and plan.tile_info(1)["lanes"] == 4
 
 
 def test_uint16_extreme_values_exact_rounding():
@@ -184,6 +185,7 @@ def test_table_modes_agree_on_fine_dm_grid(mode, monkeypatch):
     """A fine DM grid (every delay step 0 or 1) run through each table form of the tiled kernel:
     0 = one load per trial, 1 = load skipped on equal offsets, 2 = delta bits + uniform skip branch."""
     monkeypatch.setenv("DD_MODE", str(mode))
+    monkeypatch.setenv("DD_BYTES", "0")   # keep the undecimated range on 16-bit lanes (else: 8-bit lanes, next test)
     w = W.scaled(W.CONFIGS[3], nchans=260, nsamps=2 ** 14 + 5,
                  ranges=[W.DMRange(0.0, 0.1, 150, 1), W.DMRange(600.0, 0.5, 75, 4)])
     x = W.generate(w)
@@ -243,3 +245,24 @@ def test_many_flushes_and_wide_fallback():
         plan, flat = gpu_run(w, x, TILED)
         assert plan.tile_info(0)["lanes"] == lanes
         check_full(w, x, plan, flat)
+
+
+@pytest.mark.parametrize("bits", [8, 16])
+def test_byte_lanes_coarse_dm_grid(bits, monkeypatch):
+    """Undecimated range with delay steps of several samples: 8-bit lanes (uint16: low and high byte planes,
+    S = S_lo + 256 S_hi, one rounding).  Saturated rows next to random ones reach the lane bounds; 600 channels
+    cross two flushes."""
+    nch, ns = 600, 2 ** 15 + 3
+    rng = np.random.default_rng(77 + bits)
+    x = rng.integers(0, 2 ** bits, size=(2, nch, ns), dtype=np.uint8 if bits == 8 else np.uint16)
+    x[0, 100:420, :] = 2 ** bits - 1
+    x[1, ::3, 500:9000] = 2 ** bits - 1
+    w = W.Workload("bytes", 750.0, -200.0 / nch, nch, 655.36e-6, ns, 2, bits, (W.DMRange(0.0, 3.0, 70, 1),), 1, 0, 0)
+    plan, flat = gpu_run(w, x, TILED)
+    assert plan.tile_info(0)["lanes"] == 16 and plan.tile_info(0)["mode"] == 0
+    assert plan.launches() == 1 + bits // 8
+    check_full(w, x, plan, flat)
+    monkeypatch.setenv("DD_BYTES", "0")
+    plan2, flat2 = gpu_run(w, x, TILED)
+    assert plan2.tile_info(0)["lanes"] == (8 if bits == 8 else 4)
+    assert np.array_equal(flat.view(np.uint32)[flat != -1.0], flat2.view(np.uint32)[flat2 != -1.0])
