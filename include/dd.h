@@ -99,8 +99,9 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
 
 /*
  * dd_execute_host: the same path from HOST buffers, end to end: copies in_host to a plan-owned device
- * buffer, runs dd_execute, copies the result back to out_host, all enqueued on `cuda_stream`, then
- * synchronises that stream before returning.  Layouts as in dd_execute, except that whole rows are
+ * buffer, runs the kernels of dd_execute on `cuda_stream` a few trial blocks at a time and copies each finished
+ * piece of the DM-time plane back to out_host on a plan-owned copy stream while the next piece is computed
+ * (pinned host memory is needed for that overlap), then waits for everything before returning.  Layouts as in dd_execute, except that whole rows are
  * copied back, so the pad floats of out_host are overwritten with unspecified values.  The staging buffers are
  * allocated on first use (DD_ERR_NOMEM if that fails) and freed by dd_plan_destroy.
  */

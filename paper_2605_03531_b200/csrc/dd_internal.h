@@ -105,16 +105,21 @@ struct dd_plan {
   mutable long long prof_calls = 0;
   std::vector<cudaEvent_t> prof_events;
   mutable std::vector<int> prof_kind, prof_range, prof_count;  // per slot*max_launches
-  // host-path staging
+  // host path: staging buffers, a copy stream and events so that the device-to-host copy of finished trial
+  // blocks overlaps the dedispersion of the following ones
   void* h_in_dev = nullptr;
   float* h_out_dev = nullptr;
+  cudaStream_t copy_stream = nullptr;
+  std::vector<cudaEvent_t> host_events;
 };
 
 namespace dd {
 
 // launchers (dd_kernels.cu); all enqueue on `stream` and return the CUDA error of the launch
 cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream);
-cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream);  // all planes
+// all byte planes of the trial blocks blk0 .. blk0+nblk-1 (nblk <= 0: to the end of the range)
+cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream, int blk0 = 0,
+                         int nblk = 0);
 cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_dev, float* out_dev,
                           cudaStream_t stream);
 cudaError_t configure_kernels(const dd_plan* p);  // opt in to the dynamic shared memory sizes

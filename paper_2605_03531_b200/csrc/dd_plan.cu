@@ -383,6 +383,8 @@ int dd_plan_destroy(dd_plan_t* p) {
   if (p->ws && p->ws_owned) cudaFree(p->ws);
   if (p->h_in_dev) cudaFree(p->h_in_dev);
   if (p->h_out_dev) cudaFree(p->h_out_dev);
+  for (cudaEvent_t e : p->host_events) cudaEventDestroy(e);
+  if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
   delete p;
   return DD_OK;
 }
@@ -443,10 +445,62 @@ int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void*
   if (!plan->h_out_dev) {
     if (cudaMalloc(&plan->h_out_dev, out_bytes) != cudaSuccess) { plan->h_out_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
   }
+  if (!plan->copy_stream) DD_CUDA(cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
+  const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
+  // The DM-time plane is 3.6x the input: its copy back is the larger half of the transfer time.  Every range is
+  // dedispersed in a few launches of consecutive trial blocks; as soon as one is done (event), its rows -- one
+  // contiguous piece per beam -- go back on the copy stream while the next blocks are computed.
+  constexpr int kPieces = 8;  // per range: pieces of >= 1 trial block, ~14 waves of CTAs each for config 3
+  size_t nev = 0;
+  auto next_event = [&](cudaEvent_t* ev) -> cudaError_t {
+    if (nev == plan->host_events.size()) {
+      cudaEvent_t e;
+      cudaError_t rc = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+      if (rc != cudaSuccess) return rc;
+      plan->host_events.push_back(e);
+    }
+    *ev = plan->host_events[nev++];
+    return cudaSuccess;
+  };
+  auto copy_rows = [&](const dd::RangePlan& r, int j0, int j1) -> cudaError_t {  // trials j0 .. j1-1, all beams
+    cudaEvent_t ev;
+    cudaError_t rc = next_event(&ev);
+    if (rc != cudaSuccess) return rc;
+    if ((rc = cudaEventRecord(ev, stream)) != cudaSuccess) return rc;
+    if ((rc = cudaStreamWaitEvent(plan->copy_stream, ev, 0)) != cudaSuccess) return rc;
+    for (int b = 0; b < plan->nbeams; ++b) {
+      const size_t off = (size_t)b * plan->beam_stride + r.offset + (size_t)j0 * r.pitch;
+      rc = cudaMemcpyAsync(out_host + off, plan->h_out_dev + off, (size_t)(j1 - j0) * r.pitch * sizeof(float),
+                           cudaMemcpyDeviceToHost, plan->copy_stream);
+      if (rc != cudaSuccess) return rc;
+    }
+    return cudaSuccess;
+  };
   DD_CUDA(cudaMemcpyAsync(plan->h_in_dev, in_host, in_bytes, cudaMemcpyHostToDevice, stream));
-  int rc = dd_execute(plan, plan->h_in_dev, plan->h_out_dev, cuda_stream);
-  if (rc != DD_OK) return rc;
-  DD_CUDA(cudaMemcpyAsync(out_host, plan->h_out_dev, out_bytes, cudaMemcpyDeviceToHost, stream));
+  for (const auto& r : plan->ranges) {
+    if (all_direct || !r.tiled_ok) continue;
+    if (!plan->ws) return DD_ERR_NOMEM;
+    DD_CUDA(dd::launch_pack(plan, r, plan->h_in_dev, stream));
+  }
+  for (const auto& r : plan->ranges) {
+    if (all_direct || !r.tiled_ok) {
+      if (!r.d_delays) return DD_ERR_INVALID;
+      DD_CUDA(dd::launch_direct(plan, r, plan->h_in_dev, plan->h_out_dev, stream));
+      DD_CUDA(copy_rows(r, 0, r.ndm));
+      continue;
+    }
+    const int per = std::max(1, (r.nblocks + kPieces - 1) / kPieces);
+    for (int b0 = 0; b0 < r.nblocks; b0 += per) {
+      const int nb = std::min(per, r.nblocks - b0);
+      DD_CUDA(dd::launch_tiled(plan, r, plan->h_out_dev, stream, b0, nb));
+      DD_CUDA(copy_rows(r, b0 * r.Dcta, std::min(r.ndm, (b0 + nb) * r.Dcta)));
+    }
+  }
+  // the caller's stream, which this call synchronises, waits for the last copy
+  cudaEvent_t done;
+  DD_CUDA(next_event(&done));
+  DD_CUDA(cudaEventRecord(done, plan->copy_stream));
+  DD_CUDA(cudaStreamWaitEvent(stream, done, 0));
   DD_CUDA(cudaStreamSynchronize(stream));
   return DD_OK;
 }

@@ -95,7 +95,8 @@ struct TiledParams {
   const int32_t* span;  // [nblocks][Cpad] delay spread of the block = staged row length beyond T
   float* out;           // beam 0, this range
   long long out_beam_stride, pitch, Wp, H, nout, ntau;
-  int ndm, Cpad, G, T, Cc, nstages, nblocks;
+  int ndm, Cpad, G, T, Cc, nstages;
+  int blk0, nblk;    // trial blocks of this launch: blk0 .. blk0 + nblk - 1
   int rowpitch;      // superwords per staged row = T + Smax
   int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
   float accum_scale;  // 0: store; else out = value * accum_scale + out (high byte plane of uint16 input)
@@ -357,8 +358,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const int tid = threadIdx.x;
   // CTA -> (trial block fastest, time tile, beam): CTAs resident together share a time tile in L2
   const long long lin = blockIdx.x;
-  const int blk = (int)(lin % p.nblocks);
-  const long long rest = lin / p.nblocks;
+  const int blk = p.blk0 + (int)(lin % p.nblk);
+  const long long rest = lin / p.nblk;
   const long long tau = rest % p.ntau;
   const int beam = (int)(rest / p.ntau);
 
@@ -532,7 +533,9 @@ cudaError_t configure_kernels(const dd_plan*) {
   return cudaSuccess;
 }
 
-cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream) {
+cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream, int blk0, int nblk) {
+  if (nblk <= 0) nblk = r.nblocks - blk0;
+  if (blk0 < 0 || nblk <= 0 || blk0 + nblk > r.nblocks) return cudaErrorInvalidValue;
   TiledParams tp;
   tp.meta = r.d_meta;
   tp.dmin = r.d_dmin;
@@ -550,10 +553,11 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.T = r.T;
   tp.Cc = r.Cc;
   tp.nstages = r.stages;
-  tp.nblocks = r.nblocks;
+  tp.blk0 = blk0;
+  tp.nblk = nblk;
   tp.rowpitch = r.T + r.Smax;
   tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;
-  const long long nctas = (long long)r.nblocks * r.ntau * p->nbeams;
+  const long long nctas = (long long)nblk * r.ntau * p->nbeams;
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   const size_t smem = tiled_smem_bytes(r);
   const int nt = r.G * r.T;

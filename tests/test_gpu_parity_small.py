@@ -266,3 +266,24 @@ def test_byte_lanes_coarse_dm_grid(bits, monkeypatch):
     plan2, flat2 = gpu_run(w, x, TILED)
     assert plan2.tile_info(0)["lanes"] == (8 if bits == 8 else 4)
     assert np.array_equal(flat.view(np.uint32)[flat != -1.0], flat2.view(np.uint32)[flat2 != -1.0])
+
+
+@pytest.mark.parametrize("bits", [8, 16])
+def test_host_path_pieces_and_beams(bits):
+    """dd_execute_host dedisperses a few trial blocks per launch and copies each finished piece back on its own
+    stream: several pieces per range, two beams, delta / byte-plane / 32-bit-lane ranges."""
+    import torch
+    nch, ns = 96, 2 ** 14
+    rng = np.random.default_rng(900 + bits)
+    x = rng.integers(0, 2 ** bits, size=(2, nch, ns), dtype=np.uint8 if bits == 8 else np.uint16)
+    w = W.Workload("hostpieces", 750.0, -200.0 / nch, nch, 1.31072e-3, ns, 2, bits,
+                   (W.DMRange(0.0, 0.1, 700, 1), W.DMRange(70.0, 2.5, 300, 1), W.DMRange(820.0, 5.0, 41, 4)), 1, 0, 0)
+    want = oracle_full(w, x)
+    from paper_2605_03531_b200 import binding as B
+    plan = B.Plan.from_workload(w)
+    hin = torch.from_numpy(x.view(np.int16) if bits == 16 else x).pin_memory()
+    hout = torch.full((plan.out_elems(),), -1.0, dtype=torch.float32).pin_memory()
+    for _ in range(2):   # twice: the events and the staging buffers are reused
+        hout.fill_(-1.0)
+        plan.execute_host(hin, hout, torch.cuda.current_stream())
+        check_full(w, x, plan, hout.numpy(), want, check_pad=False)
