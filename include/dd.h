@@ -74,6 +74,10 @@ typedef struct dd_plan dd_plan_t; /* opaque */
 #define DD_KERNEL_AUTO 0   /* the tiled kernel below, tile shape chosen per range */
 #define DD_KERNEL_DIRECT 1 /* one thread per (trial, sample), delays from a global table: slow, simple */
 #define DD_KERNEL_TILED 2  /* shared-memory staged, register-blocked, packed-lane adder (the product path) */
+#define DD_KERNEL_SHARED 3 /* the tiled kernel with partial sums shared between neighbouring trials whose delays
+                              coincide over a channel quad (delta-coded ranges; other ranges as DD_KERNEL_TILED):
+                              an exact shortcut that executes fewer adds than the brute-force count of
+                              PAPER.md:421.  Same bits. */
 
 /*
  * dd_plan_create: host work (delay tables, per-range sizes, tile shapes) plus device allocations and

@@ -14,7 +14,7 @@ from .build import LIB, build
 
 DD_OK = 0
 DD_ERR_INVALID, DD_ERR_TOO_SHORT, DD_ERR_OVERFLOW, DD_ERR_ALIGN, DD_ERR_CUDA, DD_ERR_NOMEM = -1, -2, -3, -4, -5, -6
-DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED = 0, 1, 2
+DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED, DD_KERNEL_SHARED = 0, 1, 2, 3
 
 # every symbol include/dd.h declares
 SYMBOLS = [

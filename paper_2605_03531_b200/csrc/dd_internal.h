@@ -31,7 +31,11 @@ __host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? 
 //   kModeDelta         every delay step inside a trial group is 0 or 1 (fine DM grids): per channel the
 //                      offset of the group's first trial plus one "changed" bit per later trial; a changed
 //                      bit advances the address by one superword and reloads, otherwise the registers are reused
-enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2 };
+//   kModeDeltaShare    kModeDelta plus sharing of partial sums (variant DD_KERNEL_SHARED): while
+//                      no channel of a quad changes its delay, the quad's sum wa+wb+wc+wd is the same for
+//                      consecutive trials and is added as ONE term.  Same table, same bits, fewer executed adds.
+enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3 };
+__host__ __device__ constexpr bool is_delta(int mode) { return mode == kModeDelta || mode == kModeDeltaShare; }
 
 // kModeDelta processes channels in quads A,B,C,D.  The changed bits of a quad share one 32-bit word laid
 // out so that each byte feeds one R2P (register -> 7 predicates): bit n%7 of byte n/7, n = (j-1)*4 + q
@@ -45,7 +49,7 @@ __host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 
 // Meta bytes per pipeline stage of Cc channels and G trial groups: one 16-bit superword offset per
 // (channel, trial), or one 16-byte entry per channel quad in delta mode.
 __host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int NL, int Cc, int G) {
-  return mode == kModeDelta ? (size_t)(Cc / 4) * (size_t)G * 16 : (size_t)Cc * (size_t)G * 2 * trials_per_thread(NL);
+  return is_delta(mode) ? (size_t)(Cc / 4) * (size_t)G * 16 : (size_t)Cc * (size_t)G * 2 * trials_per_thread(NL);
 }
 
 struct RangePlan {

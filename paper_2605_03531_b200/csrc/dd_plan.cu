@@ -573,7 +573,9 @@ int dd_plan_set_workspace(dd_plan_t* p, void* dev, int64_t bytes) {
 
 int dd_plan_set_kernel(dd_plan_t* p, int32_t variant) {
   if (!p) return DD_ERR_INVALID;
-  if (variant != DD_KERNEL_AUTO && variant != DD_KERNEL_DIRECT && variant != DD_KERNEL_TILED) return DD_ERR_INVALID;
+  if (variant != DD_KERNEL_AUTO && variant != DD_KERNEL_DIRECT && variant != DD_KERNEL_TILED &&
+      variant != DD_KERNEL_SHARED)
+    return DD_ERR_INVALID;
   if (variant == DD_KERNEL_DIRECT) {
     int rc = ensure_direct_tables(p, false);
     if (rc != DD_OK) return rc;

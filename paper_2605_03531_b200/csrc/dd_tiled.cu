@@ -108,7 +108,8 @@ __host__ __device__ inline size_t tiled_stage_bytes(int mode, int NL, int Cc, in
 constexpr int kBarRegion = 128;  // bytes reserved for the mbarriers at the start of dynamic smem
 
 size_t tiled_smem_bytes(const RangePlan& r) {
-  return kBarRegion + (size_t)r.stages * tiled_stage_bytes(r.mode, r.NL, r.Cc, r.T + r.Smax, r.G);
+  // + 512: delta mode prefetches one table row (G <= 16 entries of 16 bytes) past the last quad of a stage
+  return kBarRegion + (size_t)r.stages * tiled_stage_bytes(r.mode, r.NL, r.Cc, r.T + r.Smax, r.G) + 512;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -156,49 +157,79 @@ __device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint32_t sdata,
 // delta mode: channels in quads A..D; one table entry per quad =
 //   {changed bits (delta_bit), offA | offB<<16, offC | offD<<16, bit j: some channel of the quad changes at trial step j}
 // off = byte offset of the superword of the group's first trial, counted from the start of the stage
-template <int J>
-__device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t& aa,
-                                            uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits, uint32_t any) {
+__device__ __forceinline__ void sum4(uint4& t, const uint4& a, const uint4& b, const uint4& c, const uint4& d) {
+  t.x = a.x + b.x + c.x + d.x;
+  t.y = a.y + b.y + c.y + d.y;
+  t.z = a.z + b.z + c.z + d.z;
+  t.w = a.w + b.w + c.w + d.w;
+}
+__device__ __forceinline__ void add1(uint4& acc, const uint4& t) {
+  acc.x += t.x;
+  acc.y += t.y;
+  acc.z += t.z;
+  acc.w += t.w;
+}
+
+template <int J, bool SHARE>
+__device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint4& t4,
+                                            uint32_t& aa, uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits,
+                                            uint32_t any) {
   if constexpr (J < kRD) {
     // A predicated-off LDS still occupies a slot of the shared-memory data pipe (ncu: one wavefront per
     // skipped load, 36 % of the pipe in the first version), so the whole trial step of the quad is skipped
     // by ONE branch on its "any channel changed" bit: neighbouring channels have nearly the same delay
-    // curve and almost always change at the same trial.  `any` sits in a uniform register (stage_delta),
-    // which makes this a BRA.U without reconvergence bookkeeping.
+    // curve and often change at the same trial.  `any` sits in a uniform register (stage_delta),
+    // which makes this a branch without reconvergence bookkeeping.
     if (any & (1u << J)) {
       lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
       lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
       lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
       lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
+      if constexpr (SHARE) sum4(t4, wa, wb, wc, wd);
     }
-    add_pair(acc[J], wa, wb);
-    add_pair(acc[J], wc, wd);
-    delta_steps<J + 1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bits, any);
+    if constexpr (SHARE) {
+      add1(acc[J], t4);  // the quad's sum is unchanged since the last taken step: one term per word
+    } else {
+      add_pair(acc[J], wa, wb);
+      add_pair(acc[J], wc, wd);
+    }
+    delta_steps<J + 1, SHARE>(acc, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
   }
 }
 
+template <bool SHARE>
 __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes,
                                             uint32_t meta_row) {
+  uint4 m;
+  lds_sw(m, smeta);
 #pragma unroll 1
   for (int cc = 0; cc < Cc; cc += 4) {
-    uint4 m;
-    lds_sw(m, smeta);
-    smeta += meta_row;
     // byte offsets inside the stage, row of the channel included (16 bits each: choose_tile keeps the data
     // of a delta-mode stage below 64 KB)
     uint32_t aa = sdata + (m.y & 0xffffu);
     uint32_t ab = sdata + (m.y >> 16);
     uint32_t ac = sdata + (m.z & 0xffffu);
     uint32_t ad = sdata + (m.z >> 16);
-    uint4 wa, wb, wc, wd;
+    const uint32_t bits = m.x;
+    // the table entry is the same for the whole warp: a warp reduction hands it over in a uniform register
+    const uint32_t any = __reduce_or_sync(0xffffffffu, m.w);
+    uint4 wa, wb, wc, wd, t4;
     lds_sw(wa, aa);
     lds_sw(wb, ab);
     lds_sw(wc, ac);
     lds_sw(wd, ad);
-    add_pair(acc[0], wa, wb);
-    add_pair(acc[0], wc, wd);
-    // the table entry is the same for the whole warp: a warp reduction hands it over in a uniform register
-    delta_steps<1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, m.x, __reduce_or_sync(0xffffffffu, m.w));
+    // next quad's entry (the last one reads the first entry of the following stage slot or the pad: unused),
+    // fetched now so that its latency hides behind this quad's adds
+    smeta += meta_row;
+    lds_sw(m, smeta);
+    if constexpr (SHARE) {
+      sum4(t4, wa, wb, wc, wd);
+      add1(acc[0], t4);
+    } else {
+      add_pair(acc[0], wa, wb);
+      add_pair(acc[0], wc, wd);
+    }
+    delta_steps<1, SHARE>(acc, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
   }
 }
 
@@ -269,8 +300,8 @@ struct Lanes<4> {  // four 32-bit lanes: plain sums
   }
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
-    if constexpr (MODE == kModeDelta)
-      stage_delta(acc, sdata, smeta, Cc, row_bytes, meta_row);
+    if constexpr (is_delta(MODE))
+      stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
     else
       stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
   }
@@ -289,8 +320,8 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
   }
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
-    if constexpr (MODE == kModeDelta)
-      stage_delta(acc, sdata, smeta, Cc, row_bytes, meta_row);
+    if constexpr (is_delta(MODE))
+      stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
     else
       stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
   }
@@ -449,7 +480,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   Lanes<NL> lanes;
   lanes.init();
   const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
-  const uint32_t entry_bytes = MODE == kModeDelta ? 16u : 2u * RD;  // table bytes per (channel | quad, trial group)
+  const uint32_t entry_bytes = is_delta(MODE) ? 16u : 2u * RD;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
   const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
@@ -520,6 +551,7 @@ static cudaError_t set_smem_t() {
 #define DD_FOR_ALL_TILED(X)                                                                    \
   X(8, kModeGeneral, 256) X(8, kModeGeneralReuse, 256) X(8, kModeDelta, 256)                   \
   X(8, kModeGeneral, 512) X(8, kModeGeneralReuse, 512) X(8, kModeDelta, 512)                   \
+  X(8, kModeDeltaShare, 256) X(8, kModeDeltaShare, 512) X(4, kModeDeltaShare, 256) X(4, kModeDeltaShare, 512) \
   X(4, kModeGeneral, 256) X(4, kModeGeneralReuse, 256) X(4, kModeDelta, 256)                   \
   X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)                   \
   X(16, kModeGeneral, 256) X(16, kModeGeneral, 512)
@@ -561,13 +593,14 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   const size_t smem = tiled_smem_bytes(r);
   const int nt = r.G * r.T;
+  const int mode = (r.mode == kModeDelta && p->variant == DD_KERNEL_SHARED) ? (int)kModeDeltaShare : r.mode;
   // one launch per byte plane: low bytes stored, high bytes added with weight 256
   for (int plane = 0; plane < r.planes; ++plane) {
     tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset + plane * r.plane_bytes);
     tp.accum_scale = plane == 0 ? 0.0f : 256.0f;
     cudaError_t e = cudaErrorInvalidConfiguration;
 #define DD_GO(NL_, MODE_, NT_) \
-  if (r.NL == NL_ && r.mode == MODE_ && nt == NT_) e = launch_tiled_t<NL_, MODE_, NT_>(tp, nctas, smem, stream);
+  if (r.NL == NL_ && mode == MODE_ && nt == NT_) e = launch_tiled_t<NL_, MODE_, NT_>(tp, nctas, smem, stream);
     DD_FOR_ALL_TILED(DD_GO)
 #undef DD_GO
     if (e != cudaSuccess) return e;

@@ -287,3 +287,20 @@ def test_host_path_pieces_and_beams(bits):
         hout.fill_(-1.0)
         plan.execute_host(hin, hout, torch.cuda.current_stream())
         check_full(w, x, plan, hout.numpy(), want, check_pad=False)
+
+
+def test_shared_partial_sums_variant():
+    """DD_KERNEL_SHARED: the sum of a channel quad is reused across neighbouring trials
+    while none of its delays changes.  Fewer executed adds, identical bits (delta ranges; others unchanged)."""
+    SHARED = 3
+    w = W.scaled(W.CONFIGS[3], nchans=272, nsamps=2 ** 15 + 3,
+                 ranges=[W.DMRange(0.0, 0.1, 203, 1), W.DMRange(200.0, 0.2, 150, 2), W.DMRange(600.0, 3.0, 41, 4)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, SHARED)
+    assert [plan.tile_info(r)["mode"] for r in range(3)] == [2, 2, 0]
+    check_full(w, x, plan, flat)
+    # saturated input: the quad sum 4*1020 still fits its 16-bit lane
+    xs = np.full_like(x, 255)
+    xs[0, 7, 50:90] = 0
+    plan, flat = gpu_run(w, xs, SHARED)
+    check_full(w, xs, plan, flat)
