@@ -32,11 +32,11 @@
 extern "C" {
 #endif
 
-#define DD_VERSION 100 /* major*100 + minor */
+#define DD_VERSION 101 /* major*100 + minor */
 
 typedef enum dd_status {
   DD_OK = 0,
-  DD_ERR_INVALID = -1,   /* null pointer; nchans<1; chan_width>=0; tsamp<=0; nsamps<1; nbeams<1;
+  DD_ERR_INVALID = -1,   /* null pointer; nchans<1; chan_width==0; lowest channel <= 0 MHz; unknown layout; tsamp<=0; nsamps<1; nbeams<1;
                             in_bits not 8/16; nranges<1; decim not in {1,2,4,8}; ndm<1; dm_lo<0; dm_step<0;
                             bad range index; unknown kernel variant */
   DD_ERR_TOO_SHORT = -2, /* some range has nout_r < 1 (largest delay >= decimated length) */
@@ -57,8 +57,10 @@ typedef struct dd_range {
 
 /* The filterbank and the DM plan.  `ranges` is copied by dd_plan_create. */
 typedef struct dd_config {
-  double f_top_mhz;       /* frequency of channel 0, the highest (reference) channel, MHz */
-  double chan_width_mhz;  /* f_c = f_top + c*chan_width; must be negative */
+  double f_top_mhz;       /* frequency of channel 0, MHz: the highest channel if chan_width < 0, the lowest if > 0 */
+  double chan_width_mhz;  /* f_c = f_top + c*chan_width, non-zero.  Delays are always referenced to the HIGHEST
+                             channel (Eq. 1.1); with chan_width > 0 (ascending band) that is channel nchans-1 and
+                             the result equals that of the same data with the channel order reversed. */
   int32_t nchans;
   double tsamp_s;         /* sampling time of the input, seconds */
   int64_t nsamps;         /* time samples per channel */
@@ -66,7 +68,15 @@ typedef struct dd_config {
   int32_t in_bits;        /* 8 (uint8) or 16 (uint16) unsigned samples */
   int32_t nranges;
   const dd_range_t* ranges;
+  int32_t in_layout;      /* DD_LAYOUT_*: how `in` is stored */
 } dd_config_t;
+
+/* Input layouts.  DD_LAYOUT_CHANNEL_MAJOR [nbeams][nchans][nsamps] (time contiguous) is BASELINE.json's
+ * "channels x time samples".  DD_LAYOUT_SPECTRUM_MAJOR [nbeams][nsamps][nchans] (channel contiguous) is how the
+ * thesis's shared-memory ring buffers hold a beam: blocks of 800 / 25600 spectra of 4096 channels
+ * (2.2); the corner turn is fused into the pack / decimation kernel. */
+#define DD_LAYOUT_CHANNEL_MAJOR 0
+#define DD_LAYOUT_SPECTRUM_MAJOR 1
 
 typedef struct dd_plan dd_plan_t; /* opaque */
 
@@ -91,8 +101,8 @@ int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out);
  * dd_execute: enqueue the whole hot path on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  * legacy default stream): pack/decimate kernels for every range, then the dedispersion kernels, which
  * write fp32 results straight into out_dev.  No host synchronisation, no allocation.
- *   in_dev : [nbeams][nchans][nsamps], time contiguous, uint8 or uint16 (in_bits), 16-byte aligned,
- *            read only.  (PAPER.md:351 keeps spectra time-major; channel-major is BASELINE.json's layout.)
+ *   in_dev : [nbeams][nchans][nsamps] (time contiguous) or [nbeams][nsamps][nchans] (in_layout), uint8 or
+ *            uint16 (in_bits), 16-byte aligned, read only.
  *   out_dev: dd_plan_out_elems() floats, 16-byte aligned.  Beam b, range r, trial j, sample t' lives at
  *            out_dev[b*beam_stride + offset_r + j*pitch_r + t'],  t' < nout_r; the pitch_r - nout_r pad
  *            floats of each row are left untouched.

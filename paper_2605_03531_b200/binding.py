@@ -15,6 +15,7 @@ from .build import LIB, build
 DD_OK = 0
 DD_ERR_INVALID, DD_ERR_TOO_SHORT, DD_ERR_OVERFLOW, DD_ERR_ALIGN, DD_ERR_CUDA, DD_ERR_NOMEM = -1, -2, -3, -4, -5, -6
 DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED, DD_KERNEL_SHARED = 0, 1, 2, 3
+DD_LAYOUT_CHANNEL_MAJOR, DD_LAYOUT_SPECTRUM_MAJOR = 0, 1
 
 # every symbol include/dd.h declares
 SYMBOLS = [
@@ -34,6 +35,7 @@ class dd_config_t(ctypes.Structure):
         ("f_top_mhz", ctypes.c_double), ("chan_width_mhz", ctypes.c_double), ("nchans", ctypes.c_int32),
         ("tsamp_s", ctypes.c_double), ("nsamps", ctypes.c_int64), ("nbeams", ctypes.c_int32),
         ("in_bits", ctypes.c_int32), ("nranges", ctypes.c_int32), ("ranges", ctypes.POINTER(dd_range_t)),
+        ("in_layout", ctypes.c_int32),
     ]
 
 
@@ -112,13 +114,14 @@ class Plan:
     """Owns a dd_plan_t*.  Methods mirror the C entry points one to one."""
 
     def __init__(self, f_top_mhz: float, chan_width_mhz: float, nchans: int, tsamp_s: float, nsamps: int,
-                 ranges: Sequence[Tuple[float, float, int, int]], nbeams: int = 1, in_bits: int = 8):
+                 ranges: Sequence[Tuple[float, float, int, int]], nbeams: int = 1, in_bits: int = 8,
+                 in_layout: int = DD_LAYOUT_CHANNEL_MAJOR):
         lib = _load()
         arr = (dd_range_t * max(1, len(ranges)))()
         for i, (lo, step, ndm, decim) in enumerate(ranges):
             arr[i] = dd_range_t(float(lo), float(step), int(ndm), int(decim))
         cfg = dd_config_t(float(f_top_mhz), float(chan_width_mhz), int(nchans), float(tsamp_s), int(nsamps),
-                          int(nbeams), int(in_bits), len(ranges), arr)
+                          int(nbeams), int(in_bits), len(ranges), arr, int(in_layout))
         h = ctypes.c_void_p()
         _chk(lib.dd_plan_create(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create")
         self._h = h
@@ -127,9 +130,14 @@ class Plan:
         self.ranges = [(float(a), float(b), int(c), int(d)) for a, b, c, d in ranges]
 
     @classmethod
-    def from_workload(cls, w) -> "Plan":
-        return cls(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, w.nsamps,
-                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits)
+    def from_workload(cls, w, in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, ascending: bool = False) -> "Plan":
+        """ascending=True describes the same band listed from its lowest channel upwards (the data must then be
+        given in that order)."""
+        f0, cw = w.f_top_mhz, w.chan_width_mhz
+        if ascending:
+            f0, cw = f0 + (w.nchans - 1) * cw, -cw
+        return cls(f0, cw, w.nchans, w.tsamp_s, w.nsamps,
+                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits, in_layout)
 
     # -- dd_plan_destroy
     def destroy(self) -> None:

@@ -92,8 +92,10 @@ struct RangePlan {
 
 struct dd_plan {
   // config
-  double f_top = 0, cw = 0, tsamp = 0;
+  double f_top = 0, cw = 0, tsamp = 0;  // internal order: channel 0 = highest frequency, cw < 0
   int nchans = 0, nbeams = 0, in_bits = 8;
+  int layout = 0;      // DD_LAYOUT_* of the caller's input
+  int ascending = 0;   // caller's channel c is internal channel nchans-1-c
   int64_t nsamps = 0;
   std::vector<dd::RangePlan> ranges;
   int64_t beam_stride = 0, out_elems = 0;

@@ -66,7 +66,8 @@ __device__ __forceinline__ void load_lane4(const Tin* __restrict__ row, int64_t 
 
 template <typename Tin, int K, int NL>
 __global__ void __launch_bounds__(256) dd_pack_kernel(const Tin* __restrict__ in, uint4* __restrict__ P, int nchans,
-                                                      int Cpad, int64_t nsamps, int64_t ns_r, int64_t H, int64_t Wp) {
+                                                      int Cpad, int64_t nsamps, int64_t ns_r, int64_t H, int64_t Wp,
+                                                      int rev) {
   const int64_t i0 = 4 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
   if (i0 >= Wp) return;
   const int c = blockIdx.y;
@@ -78,7 +79,7 @@ __global__ void __launch_bounds__(256) dd_pack_kernel(const Tin* __restrict__ in
     for (int e = 0; e < 4; ++e) dst[e] = z;
     return;
   }
-  const Tin* row = in + ((int64_t)beam * nchans + c) * nsamps;
+  const Tin* row = in + ((int64_t)beam * nchans + (rev ? nchans - 1 - c : c)) * nsamps;  // rev: ascending band
   uint32_t v[NL][4];
 #pragma unroll
   for (int m = 0; m < NL; ++m) load_lane4<Tin, K>(row, i0 + (int64_t)m * H, ns_r, v[m]);
@@ -108,7 +109,8 @@ static cudaError_t launch_pack_t(const dd_plan* p, const RangePlan& r, const voi
   dim3 grid((unsigned)((quads + 255) / 256), (unsigned)r.Cpad, (unsigned)p->nbeams);
   const Tin* in = static_cast<const Tin*>(in_dev);
 #define DD_PACK(K)                                                                                              \
-  dd_pack_kernel<Tin, K, NL><<<grid, block, 0, stream>>>(in, P, p->nchans, r.Cpad, p->nsamps, r.ns, r.H, r.Wp); \
+  dd_pack_kernel<Tin, K, NL><<<grid, block, 0, stream>>>(in, P, p->nchans, r.Cpad, p->nsamps, r.ns, r.H, r.Wp, \
+                                                         p->ascending);                                           \
   break
   switch (r.decim) {
     case 1: DD_PACK(1);
@@ -127,7 +129,7 @@ static cudaError_t launch_pack_t(const dd_plan* p, const RangePlan& r, const voi
 template <typename Tin>
 __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restrict__ in, uint4* __restrict__ P0,
                                                             uint4* __restrict__ P1, int nchans, int Cpad, int64_t nsamps,
-                                                            int64_t H, int64_t Wp) {
+                                                            int64_t H, int64_t Wp, int rev) {
   const int64_t i0 = 4 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
   if (i0 >= Wp) return;
   const int c = blockIdx.y;
@@ -143,7 +145,7 @@ __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restric
     }
     return;
   }
-  const Tin* row = in + ((int64_t)beam * nchans + c) * nsamps;
+  const Tin* row = in + ((int64_t)beam * nchans + (rev ? nchans - 1 - c : c)) * nsamps;
   uint32_t lo[4][4] = {}, hi[4][4] = {};  // [superword e][word q]
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
@@ -175,7 +177,78 @@ __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restric
   }
 }
 
+// a2 for spectrum-major input [beam][time][channel] (the layout of the thesis's shared-memory ring buffers,
+// PAPER.md:351): the corner turn is fused into the pack.  CTA = kTcCh channels x kTcTi superword indices.
+// Phase 1 reads the NL*kTcTi*decim spectra slices of the tile with consecutive threads on consecutive
+// channels (coalesced) and sums `decim` spectra into shared memory; phase 2 builds the superwords of every
+// channel and writes them with consecutive threads on consecutive superwords.
+constexpr int kTcCh = 128, kTcTi = 4;
+template <typename Tin, int NL>
+__global__ void __launch_bounds__(256) dd_pack_tc_kernel(const Tin* __restrict__ in, uint4* __restrict__ P0,
+                                                         uint4* __restrict__ P1, int nchans, int Cpad, int64_t nsamps,
+                                                         int64_t ns_r, int decim, int64_t H, int64_t Wp, int rev) {
+  __shared__ uint32_t vals[NL][kTcTi][kTcCh + 1];
+  const int64_t i0 = (int64_t)blockIdx.x * kTcTi;
+  const int c0 = blockIdx.y * kTcCh;
+  const int beam = blockIdx.z;
+  const Tin* x = in + (int64_t)beam * nsamps * nchans;
+  for (int idx = threadIdx.x; idx < NL * kTcTi * kTcCh; idx += blockDim.x) {
+    const int cl = idx % kTcCh, ti = (idx / kTcCh) % kTcTi, m = idx / (kTcCh * kTcTi);
+    const int c = c0 + cl;
+    const int64_t s = i0 + ti + (int64_t)m * H;  // decimated sample index
+    uint32_t a = 0;
+    if (c < nchans && s < ns_r) {
+      const Tin* src = x + (int64_t)decim * s * nchans + (rev ? nchans - 1 - c : c);
+      for (int q = 0; q < decim; ++q) a += (uint32_t)src[(int64_t)q * nchans];
+    }
+    vals[m][ti][cl] = a;
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < kTcTi * kTcCh; idx += blockDim.x) {
+    const int ti = idx % kTcTi, cl = idx / kTcTi;
+    const int c = c0 + cl;
+    if (c >= Cpad || i0 + ti >= Wp) continue;
+    const int64_t o = ((int64_t)beam * Cpad + c) * Wp + i0 + ti;
+    uint32_t v[NL];
+#pragma unroll
+    for (int m = 0; m < NL; ++m) v[m] = vals[m][ti][cl];
+    if constexpr (NL == 4) {
+      P0[o] = make_uint4(v[0], v[1], v[2], v[3]);
+    } else if constexpr (NL == 8) {
+      P0[o] = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
+    } else {  // 16 byte lanes; uint16 input: low bytes to plane 0, high bytes to plane 1
+      uint32_t lo[4], hi[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        lo[q] = (v[4 * q] & 0xffu) | ((v[4 * q + 1] & 0xffu) << 8) | ((v[4 * q + 2] & 0xffu) << 16) | (v[4 * q + 3] << 24);
+        hi[q] = (v[4 * q] >> 8) | ((v[4 * q + 1] >> 8) << 8) | ((v[4 * q + 2] >> 8) << 16) | ((v[4 * q + 3] >> 8) << 24);
+      }
+      P0[o] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+      if (sizeof(Tin) == 2) P1[o] = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    }
+  }
+}
+
+template <typename Tin, int NL>
+static cudaError_t launch_pack_tc_t(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream) {
+  uint4* P0 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset);
+  uint4* P1 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset + r.plane_bytes);
+  dim3 grid((unsigned)((r.Wp + kTcTi - 1) / kTcTi), (unsigned)((r.Cpad + kTcCh - 1) / kTcCh), (unsigned)p->nbeams);
+  dd_pack_tc_kernel<Tin, NL><<<grid, 256, 0, stream>>>(static_cast<const Tin*>(in_dev), P0, P1, p->nchans, r.Cpad,
+                                                       p->nsamps, r.ns, r.decim, r.H, r.Wp, p->ascending);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream) {
+  if (p->layout == DD_LAYOUT_SPECTRUM_MAJOR) {
+    if (p->in_bits == 8)
+      return r.NL == 16 ? launch_pack_tc_t<uint8_t, 16>(p, r, in_dev, stream)
+             : r.NL == 8 ? launch_pack_tc_t<uint8_t, 8>(p, r, in_dev, stream)
+                         : launch_pack_tc_t<uint8_t, 4>(p, r, in_dev, stream);
+    return r.NL == 16 ? launch_pack_tc_t<uint16_t, 16>(p, r, in_dev, stream)
+           : r.NL == 8 ? launch_pack_tc_t<uint16_t, 8>(p, r, in_dev, stream)
+                       : launch_pack_tc_t<uint16_t, 4>(p, r, in_dev, stream);
+  }
   if (r.NL == 16) {
     uint4* P0 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset);
     uint4* P1 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset + r.plane_bytes);
@@ -183,10 +256,10 @@ cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev
     dim3 grid((unsigned)((r.Wp / 4 + 255) / 256), (unsigned)r.Cpad, (unsigned)p->nbeams);
     if (p->in_bits == 8)
       dd_pack_bytes_kernel<uint8_t><<<grid, block, 0, stream>>>(static_cast<const uint8_t*>(in_dev), P0, nullptr, p->nchans,
-                                                                r.Cpad, p->nsamps, r.H, r.Wp);
+                                                                r.Cpad, p->nsamps, r.H, r.Wp, p->ascending);
     else
       dd_pack_bytes_kernel<uint16_t><<<grid, block, 0, stream>>>(static_cast<const uint16_t*>(in_dev), P0, P1, p->nchans,
-                                                                 r.Cpad, p->nsamps, r.H, r.Wp);
+                                                                 r.Cpad, p->nsamps, r.H, r.Wp, p->ascending);
     return cudaGetLastError();
   }
   if (p->in_bits == 8) {
@@ -201,17 +274,18 @@ cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev
 template <typename Tin>
 __global__ void __launch_bounds__(256) dd_direct_kernel(const Tin* __restrict__ in, const int32_t* __restrict__ delays,
                                                         float* __restrict__ out, int nchans, long long nsamps, int decim,
-                                                        long long nout, long long pitch, long long out_beam_stride) {
+                                                        long long nout, long long pitch, long long out_beam_stride,
+                                                        long long chan_stride, long long time_stride, int rev) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nout) return;
   const int j = blockIdx.y;
   const int beam = blockIdx.z;
   const Tin* x = in + (long long)beam * nchans * nsamps;
-  const int32_t* d = delays + (long long)j * nchans;
+  const int32_t* d = delays + (long long)j * nchans;  // internal order: channel 0 = highest frequency
   uint32_t s = 0;
   for (int c = 0; c < nchans; ++c) {
-    const Tin* src = x + (long long)c * nsamps + (long long)decim * (t + d[c]);
-    for (int q = 0; q < decim; ++q) s += (uint32_t)src[q];
+    const Tin* src = x + (long long)(rev ? nchans - 1 - c : c) * chan_stride + (long long)decim * (t + d[c]) * time_stride;
+    for (int q = 0; q < decim; ++q) s += (uint32_t)src[q * time_stride];
   }
   out[(long long)beam * out_beam_stride + (long long)j * pitch + t] = __uint2float_rn(s);
 }
@@ -220,14 +294,16 @@ cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_d
                           cudaStream_t stream) {
   dim3 block(256);
   dim3 grid((unsigned)((r.nout + 255) / 256), (unsigned)r.ndm, (unsigned)p->nbeams);
+  const bool tc = p->layout == DD_LAYOUT_SPECTRUM_MAJOR;
+  const long long cs = tc ? 1 : p->nsamps, ts = tc ? p->nchans : 1;
   if (p->in_bits == 8) {
     dd_direct_kernel<uint8_t><<<grid, block, 0, stream>>>(static_cast<const uint8_t*>(in_dev), r.d_delays,
                                                           out_dev + r.offset, p->nchans, p->nsamps, r.decim, r.nout,
-                                                          r.pitch, p->beam_stride);
+                                                          r.pitch, p->beam_stride, cs, ts, p->ascending);
   } else {
     dd_direct_kernel<uint16_t><<<grid, block, 0, stream>>>(static_cast<const uint16_t*>(in_dev), r.d_delays,
                                                            out_dev + r.offset, p->nchans, p->nsamps, r.decim, r.nout,
-                                                           r.pitch, p->beam_stride);
+                                                           r.pitch, p->beam_stride, cs, ts, p->ascending);
   }
   return cudaGetLastError();
 }

@@ -286,11 +286,13 @@ const char* dd_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
   if (!cfg || !plan_out) return DD_ERR_INVALID;
   *plan_out = nullptr;
-  if (cfg->nchans < 1 || !(cfg->chan_width_mhz < 0.0) || !(cfg->tsamp_s > 0.0) || cfg->nsamps < 1 ||
+  if (cfg->nchans < 1 || !(cfg->chan_width_mhz != 0.0) || !(cfg->tsamp_s > 0.0) || cfg->nsamps < 1 ||
+      (cfg->in_layout != DD_LAYOUT_CHANNEL_MAJOR && cfg->in_layout != DD_LAYOUT_SPECTRUM_MAJOR) ||
       cfg->nbeams < 1 || !(cfg->in_bits == 8 || cfg->in_bits == 16) || cfg->nranges < 1 || !cfg->ranges ||
       !(cfg->f_top_mhz > 0.0) || cfg->nchans > 65535 || cfg->nbeams > 65535)
     return DD_ERR_INVALID;
-  if (!(cfg->f_top_mhz + (double)(cfg->nchans - 1) * cfg->chan_width_mhz > 0.0)) return DD_ERR_INVALID;
+  const double f_last = cfg->f_top_mhz + (double)(cfg->nchans - 1) * cfg->chan_width_mhz;
+  if (!(f_last > 0.0)) return DD_ERR_INVALID;
   for (int r = 0; r < cfg->nranges; ++r) {
     const dd_range_t& q = cfg->ranges[r];
     if (!(q.decim == 1 || q.decim == 2 || q.decim == 4 || q.decim == 8) || q.ndm < 1 || q.ndm > 65535 ||
@@ -303,8 +305,12 @@ int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
   if (!p) return DD_ERR_NOMEM;
   int rc = DD_OK;
   try {
-    p->f_top = cfg->f_top_mhz;
-    p->cw = cfg->chan_width_mhz;
+    // internally channel 0 is always the highest frequency (the reference of Eq. 1.1); an ascending band is
+    // the same band read backwards, and the pack / direct kernels reverse the channel index while loading
+    p->ascending = cfg->chan_width_mhz > 0.0;
+    p->f_top = p->ascending ? f_last : cfg->f_top_mhz;
+    p->cw = -fabs(cfg->chan_width_mhz);
+    p->layout = cfg->in_layout;
     p->tsamp = cfg->tsamp_s;
     p->nchans = cfg->nchans;
     p->nbeams = cfg->nbeams;

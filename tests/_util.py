@@ -30,12 +30,20 @@ def oracle_full(w: W.Workload, x: np.ndarray):
     return res
 
 
-def gpu_run(w: W.Workload, x: np.ndarray, variant: int = 0, host_path: bool = False):
-    """CUDA path through the C ABI.  Returns (plan, flat float32 numpy output)."""
+def gpu_run(w: W.Workload, x: np.ndarray, variant: int = 0, host_path: bool = False, in_layout: int = 0,
+            ascending: bool = False):
+    """CUDA path through the C ABI.  Returns (plan, flat float32 numpy output).  `x` is always given as
+    [beam][channel][time] with channel 0 the highest frequency (the oracle's order); for the other input
+    conventions of the ABI it is re-laid out here (channel order reversed / spectra contiguous) before the call."""
     import torch
     from paper_2605_03531_b200 import binding as B
 
-    plan = B.Plan.from_workload(w)
+    plan = B.Plan.from_workload(w, in_layout=in_layout, ascending=ascending)
+    if ascending:
+        x = x[:, ::-1, :]
+    if in_layout == B.DD_LAYOUT_SPECTRUM_MAJOR:
+        x = x.transpose(0, 2, 1)
+    x = np.ascontiguousarray(x)
     plan.set_kernel(variant)
     n = plan.out_elems()
     if host_path:

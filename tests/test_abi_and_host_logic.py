@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
     for name in declared:
         assert hasattr(lib, name), name
     assert sorted(B.SYMBOLS) == declared          # the binding mirrors the header one to one
-    assert B.dd_version() == 100
+    assert B.dd_version() == 101
     assert B.dd_strerror(0) == "ok" and "short" in B.dd_strerror(B.DD_ERR_TOO_SHORT)
 
 

@@ -304,3 +304,39 @@ def test_shared_partial_sums_variant():
     xs[0, 7, 50:90] = 0
     plan, flat = gpu_run(w, xs, SHARED)
     check_full(w, xs, plan, flat)
+
+
+# ---- NEXT-1 (SURVEY.md 8(f)): spectrum-major input, ascending bands ------------------------------------
+
+@pytest.mark.parametrize("variant", [DIRECT, TILED])
+@pytest.mark.parametrize("layout,ascending", [(1, False), (0, True), (1, True)])
+def test_input_layouts_uint8(variant, layout, ascending):
+    """[beam][time][channel] input (the thesis's ring-buffer order) and bands listed from the lowest
+    channel upwards give the bits of the channel-major, descending description of the same data."""
+    w = W.scaled(W.CONFIGS[3], nchans=150, nsamps=2 ** 14 + 9, nbeams=2,
+                 ranges=[W.DMRange(0.0, 0.1, 90, 1), W.DMRange(50.0, 2.0, 33, 1), W.DMRange(200.0, 0.2, 70, 2),
+                         W.DMRange(600.0, 0.5, 40, 4)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, variant, in_layout=layout, ascending=ascending)
+    check_full(w, x, plan, flat)
+
+
+@pytest.mark.parametrize("layout,ascending", [(1, False), (1, True), (0, True)])
+def test_input_layouts_uint16(layout, ascending):
+    w = W.scaled(W.CONFIGS[4], nchans=200, nsamps=2 ** 15,
+                 ranges=[W.DMRange(0.0, 0.25, 60, 1), W.DMRange(1000.0, 1.0, 37, 8)])
+    x = W.generate(w)
+    for variant in (DIRECT, TILED):
+        plan, flat = gpu_run(w, x, variant, in_layout=layout, ascending=ascending)
+        check_full(w, x, plan, flat)
+
+
+def test_bad_layout_and_zero_width_are_rejected():
+    from paper_2605_03531_b200 import binding as B
+    for kw in ({"in_layout": 7}, {}):
+        with pytest.raises(B.DDError) as e:
+            B.Plan(500.0, 0.0 if not kw else -1.0, 16, 1.024e-3, 4096, [(0.0, 1.0, 3, 1)], **kw)
+        assert e.value.code == B.DD_ERR_INVALID
+    with pytest.raises(B.DDError) as e:   # ascending band whose lowest channel is not above 0 MHz
+        B.Plan(-10.0, 1.0, 16, 1.024e-3, 4096, [(0.0, 1.0, 3, 1)])
+    assert e.value.code == B.DD_ERR_INVALID
