@@ -192,16 +192,43 @@ __global__ void __launch_bounds__(256) dd_pack_tc_kernel(const Tin* __restrict__
   const int c0 = blockIdx.y * kTcCh;
   const int beam = blockIdx.z;
   const Tin* x = in + (int64_t)beam * nsamps * nchans;
-  for (int idx = threadIdx.x; idx < NL * kTcTi * kTcCh; idx += blockDim.x) {
-    const int cl = idx % kTcCh, ti = (idx / kTcCh) % kTcTi, m = idx / (kTcCh * kTcTi);
-    const int c = c0 + cl;
-    const int64_t s = i0 + ti + (int64_t)m * H;  // decimated sample index
-    uint32_t a = 0;
-    if (c < nchans && s < ns_r) {
-      const Tin* src = x + (int64_t)decim * s * nchans + (rev ? nchans - 1 - c : c);
-      for (int q = 0; q < decim; ++q) a += (uint32_t)src[(int64_t)q * nchans];
+  if (!rev && nchans % 4 == 0) {
+    // fast path: a warp reads the 128 channels of one spectrum slice with one 4-channel vector load per thread
+    const int l = threadIdx.x & 31, wq = threadIdx.x >> 5;
+    const int c = c0 + 4 * l;
+#pragma unroll
+    for (int rr = 0; rr < NL * kTcTi / 8; ++rr) {
+      const int row = wq + 8 * rr, m = row / kTcTi, ti = row % kTcTi;
+      const int64_t s = i0 + ti + (int64_t)m * H;  // decimated sample index
+      uint32_t a[4] = {0, 0, 0, 0};
+      if (c < nchans && s < ns_r) {
+        const Tin* src = x + (int64_t)decim * s * nchans + c;
+#pragma unroll 4
+        for (int q = 0; q < decim; ++q) {
+          if constexpr (sizeof(Tin) == 1) {
+            const uint32_t t = __ldg(reinterpret_cast<const uint32_t*>(src + (int64_t)q * nchans));
+            a[0] += t & 0xffu, a[1] += (t >> 8) & 0xffu, a[2] += (t >> 16) & 0xffu, a[3] += t >> 24;
+          } else {
+            const uint2 t = __ldg(reinterpret_cast<const uint2*>(src + (int64_t)q * nchans));
+            a[0] += t.x & 0xffffu, a[1] += t.x >> 16, a[2] += t.y & 0xffffu, a[3] += t.y >> 16;
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) vals[m][ti][4 * l + k] = a[k];
     }
-    vals[m][ti][cl] = a;
+  } else {
+    for (int idx = threadIdx.x; idx < NL * kTcTi * kTcCh; idx += blockDim.x) {
+      const int cl = idx % kTcCh, ti = (idx / kTcCh) % kTcTi, m = idx / (kTcCh * kTcTi);
+      const int c = c0 + cl;
+      const int64_t s = i0 + ti + (int64_t)m * H;  // decimated sample index
+      uint32_t a = 0;
+      if (c < nchans && s < ns_r) {
+        const Tin* src = x + (int64_t)decim * s * nchans + (rev ? nchans - 1 - c : c);
+        for (int q = 0; q < decim; ++q) a += (uint32_t)src[(int64_t)q * nchans];
+      }
+      vals[m][ti][cl] = a;
+    }
   }
   __syncthreads();
   for (int idx = threadIdx.x; idx < kTcTi * kTcCh; idx += blockDim.x) {
