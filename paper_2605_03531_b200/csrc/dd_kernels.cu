@@ -18,6 +18,13 @@
 
 namespace dd {
 
+// Two consecutive superwords as one 256-bit store (STG.256): a warp then writes whole 32-byte sectors.
+__device__ __forceinline__ void store2(uint4* dst, const uint4& a, const uint4& b) {  // dst 32-byte aligned
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w),
+               "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
+               : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
 // a2: pack + time decimation
 // ------------------------------------------------------------------------------------------------
@@ -83,22 +90,23 @@ __global__ void __launch_bounds__(256) dd_pack_kernel(const Tin* __restrict__ in
   uint32_t v[NL][4];
 #pragma unroll
   for (int m = 0; m < NL; ++m) load_lane4<Tin, K>(row, i0 + (int64_t)m * H, ns_r, v[m]);
+  uint4 w[4];
 #pragma unroll
   for (int e = 0; e < 4; ++e) {
-    uint4 w;
     if constexpr (NL == 8) {
-      w.x = v[0][e] | (v[1][e] << 16);
-      w.y = v[2][e] | (v[3][e] << 16);
-      w.z = v[4][e] | (v[5][e] << 16);
-      w.w = v[6][e] | (v[7][e] << 16);
+      w[e].x = v[0][e] | (v[1][e] << 16);
+      w[e].y = v[2][e] | (v[3][e] << 16);
+      w[e].z = v[4][e] | (v[5][e] << 16);
+      w[e].w = v[6][e] | (v[7][e] << 16);
     } else {
-      w.x = v[0][e];
-      w.y = v[1][e];
-      w.z = v[2][e];
-      w.w = v[3][e];
+      w[e].x = v[0][e];
+      w[e].y = v[1][e];
+      w[e].z = v[2][e];
+      w[e].w = v[3][e];
     }
-    dst[e] = w;
   }
+  store2(dst, w[0], w[1]);  // i0 is a multiple of 4 and Wp of 8: 64-byte aligned
+  store2(dst + 2, w[2], w[3]);
 }
 
 template <typename Tin, int NL>
@@ -171,9 +179,12 @@ __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restric
     }
   }
 #pragma unroll
-  for (int e = 0; e < 4; ++e) {
-    P0[o + e] = make_uint4(lo[e][0], lo[e][1], lo[e][2], lo[e][3]);
-    if (kTwo) P1[o + e] = make_uint4(hi[e][0], hi[e][1], hi[e][2], hi[e][3]);
+  for (int e = 0; e < 4; e += 2) {
+    store2(P0 + o + e, make_uint4(lo[e][0], lo[e][1], lo[e][2], lo[e][3]),
+           make_uint4(lo[e + 1][0], lo[e + 1][1], lo[e + 1][2], lo[e + 1][3]));
+    if (kTwo)
+      store2(P1 + o + e, make_uint4(hi[e][0], hi[e][1], hi[e][2], hi[e][3]),
+             make_uint4(hi[e + 1][0], hi[e + 1][1], hi[e + 1][2], hi[e + 1][3]));
   }
 }
 
