@@ -46,10 +46,11 @@ __host__ __device__ constexpr int delta_bit(int j, int q) { return (((j - 1) * 4
 // for a block whose delays spread over `spread` superwords.
 __host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 + 7) / 8 * 8; }
 
-// Meta bytes per pipeline stage of Cc channels and G trial groups: one 16-bit superword offset per
-// (channel, trial), or one 16-byte entry per channel quad in delta mode.
+// Meta bytes per pipeline stage of Cc channels and G trial groups: one 16-byte entry per (channel, trial
+// group) -- eight 16-bit superword offsets, or (NL = 16) four 32-bit byte offsets inside the stage, row
+// included -- or one 16-byte entry per channel quad in delta mode.
 __host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int NL, int Cc, int G) {
-  return is_delta(mode) ? (size_t)(Cc / 4) * (size_t)G * 16 : (size_t)Cc * (size_t)G * 2 * trials_per_thread(NL);
+  return (size_t)(is_delta(mode) ? Cc / 4 : Cc) * (size_t)G * 16;
 }
 
 struct RangePlan {

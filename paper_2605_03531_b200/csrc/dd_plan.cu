@@ -200,7 +200,7 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
   const size_t nbc = (size_t)r.nblocks * r.Cpad;
   std::vector<int32_t> dmin(nbc, 0), span(nbc, 0);
   const bool delta = r.mode == dd::kModeDelta;
-  const size_t words_per_entry = delta ? 4 : r.RD / 2;  // 16-bit offsets, two per word
+  const size_t words_per_entry = 4;
   const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
   std::vector<uint32_t> meta(nentries * words_per_entry, 0);
   // rows past nchans are the zero rows of the packed input: delay 0 for every trial
@@ -225,7 +225,12 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
             }
         } else {
           uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * words_per_entry];
-          for (int j = 0; j < r.RD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));
+          if (r.NL == 16) {  // byte offsets inside the stage, row of the channel included
+            for (int j = 0; j < r.RD; ++j)
+              e[j] = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg + j, c) - d0)) * 16u;
+          } else {
+            for (int j = 0; j < r.RD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));
+          }
         }
       }
     }

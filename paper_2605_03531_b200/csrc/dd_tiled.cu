@@ -233,7 +233,7 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
   }
 }
 
-// 8-bit lanes (NL = 16): channels in pairs, one table entry (kRD16 16-bit superword offsets) per channel.
+// 8-bit lanes (NL = 16): channels in pairs, one table entry (kRD16 32-bit byte offsets) per channel.
 // A loaded word w holds the bytes b0..b3 of four time lanes.  Two accumulators per word:
 //   e += w & 0x00ff00ff            two 16-bit lanes: A0 | A2 << 16 (sums of b0 and b2)   LOP3 + half an IADD3 per channel
 //   r += w >> 8                    = A1 + 2^8 A2 + 2^16 A3  (mod 2^32)                    one LEA.HI per channel
@@ -253,24 +253,18 @@ __device__ __forceinline__ void add_bytes(uint4& e, uint4& r, const uint4& a, co
 }
 
 __device__ __forceinline__ void stage_bytes(uint4 (&e)[kRD16], uint4 (&r)[kRD16], uint32_t sdata, uint32_t smeta, int Cc,
-                                            uint32_t row_bytes, uint32_t meta_row) {
+                                            uint32_t meta_row) {
 #pragma unroll 1
   for (int cc = 0; cc < Cc; cc += 2) {
-    uint32_t ma0, ma1, mb0, mb1;
-    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(ma0), "=r"(ma1) : "r"(smeta));
-    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(mb0), "=r"(mb1) : "r"(smeta + meta_row));
+    uint4 ma, mb;  // byte offsets of the four trials inside the stage (row included): one add per address
+    lds_sw(ma, smeta);
+    lds_sw(mb, smeta + meta_row);
     smeta += 2 * meta_row;
-    const uint32_t ra = sdata, rb = sdata + row_bytes;
-    sdata += 2 * row_bytes;
-#pragma unroll
-    for (int j = 0; j < kRD16; ++j) {
-      const uint32_t wa = j < 2 ? ma0 : ma1, wb = j < 2 ? mb0 : mb1;
-      const uint32_t oa = (j & 1) ? (wa >> 16) : (wa & 0xffffu), ob = (j & 1) ? (wb >> 16) : (wb & 0xffffu);
-      uint4 xa, xb;
-      lds_sw(xa, ra + oa * kSuperwordBytes);
-      lds_sw(xb, rb + ob * kSuperwordBytes);
-      add_bytes(e[j], r[j], xa, xb);
-    }
+    uint4 xa, xb;
+    lds_sw(xa, sdata + ma.x), lds_sw(xb, sdata + mb.x), add_bytes(e[0], r[0], xa, xb);
+    lds_sw(xa, sdata + ma.y), lds_sw(xb, sdata + mb.y), add_bytes(e[1], r[1], xa, xb);
+    lds_sw(xa, sdata + ma.z), lds_sw(xb, sdata + mb.z), add_bytes(e[2], r[2], xa, xb);
+    lds_sw(xa, sdata + ma.w), lds_sw(xb, sdata + mb.w), add_bytes(e[3], r[3], xa, xb);
   }
 }
 
@@ -348,7 +342,7 @@ struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upp
   }
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
-    stage_bytes(e, r, sdata, smeta, Cc, row_bytes, meta_row);
+    stage_bytes(e, r, sdata, smeta, Cc, meta_row);
   }
   // invariant: e = A0 | A2 << 16,  r = A1 + 2^8 A2 + 2^16 A3 (mod 2^32),  lane sum = A + 256 * (he | hq lane)
   static __device__ __forceinline__ void flush_word(uint32_t& e, uint32_t& r, uint32_t& he, uint32_t& hq) {
@@ -480,7 +474,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   Lanes<NL> lanes;
   lanes.init();
   const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
-  const uint32_t entry_bytes = is_delta(MODE) ? 16u : 2u * RD;  // table bytes per (channel | quad, trial group)
+  const uint32_t entry_bytes = 16u;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
   const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
