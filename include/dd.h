@@ -98,6 +98,13 @@ typedef struct dd_plan dd_plan_t; /* opaque */
 int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out);
 
 /*
+ * dd_plan_create_host: the host half of dd_plan_create only -- validation, delay tables (Eq. 1.1), per-range
+ * sizes, tile shapes and the tables the tiled kernel reads -- without any CUDA call.  The plan answers every
+ * query below but cannot execute (dd_execute returns DD_ERR_INVALID).  For inspection and CPU-side tests.
+ */
+int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out);
+
+/*
  * dd_execute: enqueue the whole hot path on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  * legacy default stream): pack/decimate kernels for every range, then the dedispersion kernels, which
  * write fp32 results straight into out_dev.  No host synchronisation, no allocation.
@@ -135,7 +142,8 @@ int dd_plan_beam_stride(const dd_plan_t* plan, int64_t* floats);
  * nout_r rounded up to a multiple of 32; offset_floats = start of the range within one beam. */
 int dd_plan_range_info(const dd_plan_t* plan, int32_t r, int64_t* ns_r, int64_t* maxd_r, int64_t* nout_r,
                        int64_t* pitch_floats, int64_t* offset_floats);
-/* Test hook: copies the delay table of range r, int32 [ndm_r][nchans], into host_buf. */
+/* Test hook: copies the delay table of range r, int32 [ndm_r][nchans], into host_buf.  Channel 0 is the highest
+ * frequency (for an ascending band that is the caller's last channel). */
 int dd_plan_get_delays(const dd_plan_t* plan, int32_t r, int32_t* host_buf);
 /* Sum over beams and ranges of ndm_r * nout_r (the "DM-trial x samples" of one execute) and the
  * brute-force add count, that number times nchans (O(m x N) per trial). */
@@ -159,6 +167,17 @@ int dd_plan_set_kernel(dd_plan_t* plan, int32_t variant);
  * group of 8 trials are 0 or 1; one changed bit per trial). */
 int dd_plan_tile_info(const dd_plan_t* plan, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta,
                       int32_t* lanes, int32_t* flush_chans, int32_t* mode);
+
+/* More of the tile shape of range r (any pointer may be NULL): trial groups per CTA, channels per pipeline
+ * stage, ring depth, superwords per staged channel row, channel rows incl. zero padding, trial blocks, and
+ * whether the range runs the tiled kernel at all (0: delay steps too large for shared memory -> direct kernel). */
+int dd_plan_tile_shape(const dd_plan_t* plan, int32_t r, int32_t* trial_groups, int32_t* chans_per_stage,
+                       int32_t* stages, int32_t* row_superwords, int32_t* cpad, int32_t* nblocks, int32_t* tiled);
+/* Test hook: the tables of the tiled kernel for range r as they are uploaded.  which = 0: the per-trial table
+ * (uint32 words; layout per mode in DESIGN.md "Data layout"), 1: start of the staged row per (trial block,
+ * channel) (int32 superwords, multiple of 8), 2: its length beyond the time tile (int32).  *bytes = size; the
+ * table is copied when host_buf != NULL (DD_ERR_NOMEM if cap_bytes is too small). */
+int dd_plan_table(const dd_plan_t* plan, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes);
 
 /* ---- per-kernel timing (measurement hook) ------------------------------------------------------- */
 

@@ -22,6 +22,7 @@ SYMBOLS = [
     "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
+    "dd_plan_create_host", "dd_plan_tile_shape", "dd_plan_table",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
 ]
 
@@ -74,6 +75,9 @@ def _load():
         lib.dd_plan_set_workspace.argtypes = [vp, vp, i64]
         lib.dd_plan_set_kernel.argtypes = [vp, i32]
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
+        lib.dd_plan_create_host.argtypes = [P(dd_config_t), P(vp)]
+        lib.dd_plan_tile_shape.argtypes = [vp, i32] + [P(i32)] * 7
+        lib.dd_plan_table.argtypes = [vp, i32, i32, vp, ctypes.c_int64, P(ctypes.c_int64)]
         lib.dd_plan_set_profiling.argtypes = [vp, i32]
         lib.dd_plan_kernel_times.argtypes = [vp, i32, i32, P(ctypes.c_float), P(i32), P(i32), P(i32)]
         lib.dd_strerror.argtypes = [ctypes.c_int]
@@ -115,7 +119,7 @@ class Plan:
 
     def __init__(self, f_top_mhz: float, chan_width_mhz: float, nchans: int, tsamp_s: float, nsamps: int,
                  ranges: Sequence[Tuple[float, float, int, int]], nbeams: int = 1, in_bits: int = 8,
-                 in_layout: int = DD_LAYOUT_CHANNEL_MAJOR):
+                 in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, host_only: bool = False):
         lib = _load()
         arr = (dd_range_t * max(1, len(ranges)))()
         for i, (lo, step, ndm, decim) in enumerate(ranges):
@@ -123,21 +127,25 @@ class Plan:
         cfg = dd_config_t(float(f_top_mhz), float(chan_width_mhz), int(nchans), float(tsamp_s), int(nsamps),
                           int(nbeams), int(in_bits), len(ranges), arr, int(in_layout))
         h = ctypes.c_void_p()
-        _chk(lib.dd_plan_create(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create")
+        if host_only:
+            _chk(lib.dd_plan_create_host(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create_host")
+        else:
+            _chk(lib.dd_plan_create(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create")
         self._h = h
         self.nranges = len(ranges)
         self.nchans, self.nbeams, self.in_bits, self.nsamps = int(nchans), int(nbeams), int(in_bits), int(nsamps)
         self.ranges = [(float(a), float(b), int(c), int(d)) for a, b, c, d in ranges]
 
     @classmethod
-    def from_workload(cls, w, in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, ascending: bool = False) -> "Plan":
+    def from_workload(cls, w, in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, ascending: bool = False,
+                      host_only: bool = False) -> "Plan":
         """ascending=True describes the same band listed from its lowest channel upwards (the data must then be
         given in that order)."""
         f0, cw = w.f_top_mhz, w.chan_width_mhz
         if ascending:
             f0, cw = f0 + (w.nchans - 1) * cw, -cw
         return cls(f0, cw, w.nchans, w.tsamp_s, w.nsamps,
-                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits, in_layout)
+                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits, in_layout, host_only)
 
     # -- dd_plan_destroy
     def destroy(self) -> None:
@@ -223,6 +231,21 @@ class Plan:
         vals = [ctypes.c_int32() for _ in range(5)]
         _chk(_load().dd_plan_tile_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_tile_info")
         return {k: v.value for k, v in zip(["dm_per_cta", "words_per_cta", "lanes", "flush_chans", "mode"], vals)}
+
+    def tile_shape(self, r: int) -> dict:
+        vals = [ctypes.c_int32() for _ in range(7)]
+        _chk(_load().dd_plan_tile_shape(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_tile_shape")
+        keys = ["trial_groups", "chans_per_stage", "stages", "row_superwords", "cpad", "nblocks", "tiled"]
+        return {k: v.value for k, v in zip(keys, vals)}
+
+    def table(self, r: int, which: int):
+        """Tables of the tiled kernel (test hook): which = 0 per-trial table (uint32), 1 row starts, 2 row spans."""
+        import numpy as np
+        n = ctypes.c_int64()
+        _chk(_load().dd_plan_table(self._h, r, which, None, 0, ctypes.byref(n)), "dd_plan_table")
+        buf = np.empty(n.value // 4, dtype=np.uint32 if which == 0 else np.int32)
+        _chk(_load().dd_plan_table(self._h, r, which, buf.ctypes.data, n.value, ctypes.byref(n)), "dd_plan_table")
+        return buf
 
     def set_profiling(self, max_executes: int) -> None:
         _chk(_load().dd_plan_set_profiling(self._h, int(max_executes)), "dd_plan_set_profiling")

@@ -81,7 +81,9 @@ struct RangePlan {
   int64_t ws_offset = 0;  // byte offset of this range's packed array in the workspace
   int64_t ws_bytes = 0;
   size_t smem_bytes = 0;
-  // device tables
+  // tables of the tiled kernel: host copies (built by dd_plan.cu build_tables) and their device twins
+  std::vector<uint32_t> h_meta;
+  std::vector<int32_t> h_dmin, h_span;
   uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] RD 16-bit offsets (delay - dmin, superwords);
                                 // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits}
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)

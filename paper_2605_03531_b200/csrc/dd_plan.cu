@@ -196,13 +196,17 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
 // line-aligned fill shared memory a line per wavefront, misaligned ones 16 bytes at a time -- ncu,
 // profiles/) and its length beyond T (rounded up likewise); per trial group the offsets into the row in
 // the form the range's mode wants (dd_internal.h).  Trials past the end of the range repeat the last one.
-int upload_tables(const dd_plan& p, dd::RangePlan& r) {
+void build_tables(const dd_plan& p, dd::RangePlan& r) {
   const size_t nbc = (size_t)r.nblocks * r.Cpad;
-  std::vector<int32_t> dmin(nbc, 0), span(nbc, 0);
+  std::vector<int32_t>& dmin = r.h_dmin;
+  std::vector<int32_t>& span = r.h_span;
+  dmin.assign(nbc, 0);
+  span.assign(nbc, 0);
   const bool delta = r.mode == dd::kModeDelta;
   const size_t words_per_entry = 4;
   const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
-  std::vector<uint32_t> meta(nentries * words_per_entry, 0);
+  std::vector<uint32_t>& meta = r.h_meta;
+  meta.assign(nentries * words_per_entry, 0);
   // rows past nchans are the zero rows of the packed input: delay 0 for every trial
   auto delay = [&](int j, int c) { return c < p.nchans ? r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c] : 0; };
   for (int b = 0; b < r.nblocks; ++b) {
@@ -235,12 +239,15 @@ int upload_tables(const dd_plan& p, dd::RangePlan& r) {
       }
     }
   }
-  DD_CUDA(cudaMalloc(&r.d_meta, meta.size() * sizeof(uint32_t)));
-  DD_CUDA(cudaMalloc(&r.d_dmin, nbc * sizeof(int32_t)));
-  DD_CUDA(cudaMalloc(&r.d_span, nbc * sizeof(int32_t)));
-  DD_CUDA(cudaMemcpy(r.d_meta, meta.data(), meta.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
-  DD_CUDA(cudaMemcpy(r.d_dmin, dmin.data(), nbc * sizeof(int32_t), cudaMemcpyHostToDevice));
-  DD_CUDA(cudaMemcpy(r.d_span, span.data(), nbc * sizeof(int32_t), cudaMemcpyHostToDevice));
+}
+
+int upload_tables(dd::RangePlan& r) {
+  DD_CUDA(cudaMalloc(&r.d_meta, r.h_meta.size() * sizeof(uint32_t)));
+  DD_CUDA(cudaMalloc(&r.d_dmin, r.h_dmin.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMalloc(&r.d_span, r.h_span.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMemcpy(r.d_meta, r.h_meta.data(), r.h_meta.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_dmin, r.h_dmin.data(), r.h_dmin.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_span, r.h_span.data(), r.h_span.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   return DD_OK;
 }
 
@@ -288,7 +295,8 @@ const char* dd_strerror(int code) {
 
 const char* dd_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 
-int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
+// Host half of a plan: validation, delay tables, tile shapes, the tables of the tiled kernel.  No CUDA call.
+static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) {
   if (!cfg || !plan_out) return DD_ERR_INVALID;
   *plan_out = nullptr;
   if (cfg->nchans < 1 || !(cfg->chan_width_mhz != 0.0) || !(cfg->tsamp_s > 0.0) || cfg->nsamps < 1 ||
@@ -354,6 +362,25 @@ int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
     delete p;
     return rc;
   }
+  try {
+    for (auto& r : p->ranges)
+      if (r.tiled_ok) build_tables(*p, r);
+  } catch (const std::bad_alloc&) {
+    delete p;
+    return DD_ERR_NOMEM;
+  }
+  p->device = -1;  // host only until dd_plan_create puts it on a device
+  *plan_out = p;
+  return DD_OK;
+}
+
+int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) { return plan_create_host(cfg, plan_out); }
+
+int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
+  dd_plan* p = nullptr;
+  int rc = plan_create_host(cfg, &p);
+  if (rc != DD_OK) return rc;
+  *plan_out = nullptr;
   cudaError_t e = cudaGetDevice(&p->device);
   if (e != cudaSuccess) {
     delete p;
@@ -365,7 +392,7 @@ int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
     return cuda_fail(e, "cudaFuncSetAttribute");
   }
   for (auto& r : p->ranges) {
-    rc = r.tiled_ok ? upload_tables(*p, r) : DD_OK;
+    rc = r.tiled_ok ? upload_tables(r) : DD_OK;
     if (rc != DD_OK) break;
   }
   if (rc == DD_OK) rc = ensure_direct_tables(p, /*only_untiled=*/true);
@@ -401,7 +428,7 @@ int dd_plan_destroy(dd_plan_t* p) {
 }
 
 int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* cuda_stream) {
-  if (!plan || !in_dev || !out_dev) return DD_ERR_INVALID;
+  if (!plan || !in_dev || !out_dev || plan->device < 0) return DD_ERR_INVALID;
   if (!aligned16(in_dev) || !aligned16(out_dev)) return DD_ERR_ALIGN;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
@@ -446,7 +473,7 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
 }
 
 int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
-  if (!plan || !in_host || !out_host) return DD_ERR_INVALID;
+  if (!plan || !in_host || !out_host || plan->device < 0) return DD_ERR_INVALID;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const size_t in_bytes = (size_t)plan->nbeams * plan->nchans * plan->nsamps * (plan->in_bits / 8);
   const size_t out_bytes = (size_t)plan->out_elems * sizeof(float);
@@ -631,6 +658,33 @@ int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* m
     if (range) range[i] = p->prof_range[k];
   }
   *n = cnt;
+  return DD_OK;
+}
+
+int dd_plan_table(const dd_plan_t* p, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes) {
+  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 2) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  const void* src = which == 0 ? (const void*)q.h_meta.data() : which == 1 ? (const void*)q.h_dmin.data() : (const void*)q.h_span.data();
+  const size_t n = which == 0 ? q.h_meta.size() * 4 : which == 1 ? q.h_dmin.size() * 4 : q.h_span.size() * 4;
+  *bytes = (int64_t)n;
+  if (host_buf) {
+    if (cap_bytes < (int64_t)n) return DD_ERR_NOMEM;
+    memcpy(host_buf, src, n);
+  }
+  return DD_OK;
+}
+
+int dd_plan_tile_shape(const dd_plan_t* p, int32_t r, int32_t* trial_groups, int32_t* chans_per_stage, int32_t* stages,
+                       int32_t* row_superwords, int32_t* cpad, int32_t* nblocks, int32_t* tiled) {
+  if (!p || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  if (trial_groups) *trial_groups = q.G;
+  if (chans_per_stage) *chans_per_stage = q.Cc;
+  if (stages) *stages = q.stages;
+  if (row_superwords) *row_superwords = q.T + q.Smax;
+  if (cpad) *cpad = q.Cpad;
+  if (nblocks) *nblocks = q.nblocks;
+  if (tiled) *tiled = q.tiled_ok;
   return DD_OK;
 }
 

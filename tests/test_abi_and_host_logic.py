@@ -24,7 +24,7 @@ def test_library_exports_every_declared_symbol():
 
     lib = ctypes.CDLL(build())
     declared = _declared_symbols()
-    assert len(declared) >= 17
+    assert len(declared) >= 20
     for name in declared:
         assert hasattr(lib, name), name
     assert sorted(B.SYMBOLS) == declared          # the binding mirrors the header one to one
@@ -37,7 +37,7 @@ def test_argument_validation_happens_before_cuda():
 
     ok = dict(f_top_mhz=500.0, chan_width_mhz=-1.0, nchans=16, tsamp_s=1e-3, nsamps=100000, ranges=[(0.0, 1.0, 4, 1)])
     bad = [
-        dict(chan_width_mhz=1.0), dict(chan_width_mhz=0.0), dict(nchans=0), dict(tsamp_s=0.0), dict(nsamps=0),
+        dict(chan_width_mhz=0.0), dict(in_layout=2), dict(f_top_mhz=10.0, chan_width_mhz=-1.0), dict(nchans=0), dict(tsamp_s=0.0), dict(nsamps=0),
         dict(ranges=[(0.0, 1.0, 4, 3)]), dict(ranges=[(0.0, 1.0, 0, 1)]), dict(ranges=[(-1.0, 1.0, 4, 1)]),
         dict(ranges=[]), dict(in_bits=12), dict(nbeams=0), dict(chan_width_mhz=-100.0),
     ]
@@ -53,6 +53,8 @@ def test_argument_validation_happens_before_cuda():
     with pytest.raises(B.DDError) as e:
         B.Plan(500.0, -200.0 / 16, 16, 1.024e-3, 100, [(0.0, 1.0, 11, 1)])
     assert e.value.code == B.DD_ERR_TOO_SHORT
+    # ascending bands (chan_width > 0) and spectrum-major input are valid descriptions
+    B.Plan(500.0, 1.0, 16, 1e-3, 100000, [(0.0, 1.0, 4, 1)], in_layout=B.DD_LAYOUT_SPECTRUM_MAJOR, host_only=True).destroy()
     lib = B._load()
     assert lib.dd_plan_destroy(None) == 0
     assert lib.dd_execute(None, None, None, None) == B.DD_ERR_INVALID

@@ -1,0 +1,129 @@
+"""CPU-only checks of the plan builder (step a1 and the host logic of the tiled kernel): no GPU needed.
+
+dd_plan_create_host builds everything dd_plan_create builds except the device copies.  The delay tables are
+compared with the oracle's (Eq. 1.1); the tables the tiled kernel reads (offsets / delta bits,
+row starts and lengths) are decoded here, independently of the kernel, and must reproduce the delay table for
+every (trial block, channel, trial) of all five BASELINE configs, padding rows and padding trials included.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_03531_b200 import binding as B
+from paper_2605_03531_b200 import workloads as W
+
+
+def _host_plan(w, **kw):
+    return B.Plan.from_workload(W.scaled(w, nbeams=1) if w.nbeams > 1 else w, host_only=True, **kw)
+
+
+def _padded_delays(plan, r, shape, rd):
+    """[nblocks*Dcta][Cpad]: trials past the end repeat the last one, channel rows past nchans have delay 0."""
+    d = plan.get_delays(r).astype(np.int64)
+    ndm, nch = d.shape
+    dcta = shape["trial_groups"] * rd
+    rows = np.minimum(np.arange(shape["nblocks"] * dcta), ndm - 1)
+    out = np.zeros((rows.size, shape["cpad"]), dtype=np.int64)
+    out[:, :nch] = d[rows]
+    return out
+
+
+def _decode(plan, r):
+    """Delays implied by the kernel tables: [nblocks][Dcta][Cpad] (absolute, superwords)."""
+    info, shape = plan.tile_info(r), plan.tile_shape(r)
+    rd = 4 if info["lanes"] == 16 else 8
+    g, cc, cpad, rowp, nb = (shape[k] for k in ("trial_groups", "chans_per_stage", "cpad", "row_superwords", "nblocks"))
+    meta = plan.table(r, 0)
+    dmin = plan.table(r, 1).astype(np.int64).reshape(nb, cpad)
+    span = plan.table(r, 2).astype(np.int64).reshape(nb, cpad)
+    rowoff = (np.arange(cpad) % cc) * rowp                                    # superwords, row of the channel in its stage
+    if info["mode"] == 2:                                                     # delta table, one entry per channel quad
+        e = meta.reshape(nb, cpad // 4, g, 4).astype(np.int64)
+        rel = np.zeros((nb, g, rd, cpad), dtype=np.int64)
+        anyb = np.zeros((nb, cpad // 4, g), dtype=np.int64)
+        for q in range(4):
+            field = (e[..., 1 + q // 2] >> (16 * (q % 2))) & 0xFFFF           # [nb][quad][g] byte offset in the stage
+            assert (field % 16 == 0).all()
+            first = field // 16 - rowoff[q::4][None, :, None]
+            cur = first.copy()
+            rel[:, :, 0, q::4] = first.transpose(0, 2, 1)
+            for j in range(1, rd):
+                n = (j - 1) * 4 + q
+                bit = (e[..., 0] >> ((n // 7) * 8 + n % 7)) & 1
+                anyb |= bit << j
+                cur = cur + bit
+                rel[:, :, j, q::4] = cur.transpose(0, 2, 1)
+        assert np.array_equal(anyb, e[..., 3]), "any-changed bits are the OR of the quad's changed bits"
+        assert (e[..., 0] & 0x80808080 == 0).all()                            # bit 7 of each byte is unused
+    elif info["lanes"] == 16:                                                 # 32-bit byte offsets, row included
+        e = meta.reshape(nb, cpad, g, 4).astype(np.int64)
+        assert (e % 16 == 0).all()
+        rel = (e // 16 - rowoff[None, :, None, None]).transpose(0, 2, 3, 1)
+    else:                                                                     # 16-bit superword offsets
+        e = meta.view(np.uint16).reshape(nb, cpad, g, 8).astype(np.int64)
+        rel = e.transpose(0, 2, 3, 1)
+    assert (rel >= 0).all() and (rel <= span[:, None, None, :]).all(), "every load stays inside the staged row"
+    assert (dmin % 8 == 0).all() and (span % 8 == 0).all(), "staged rows start and end on 128-byte lines"
+    assert (span + info["words_per_cta"] <= rowp).all()
+    absd = rel + dmin[:, None, None, :]
+    return absd.reshape(nb * g * rd, cpad), rd, shape
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_kernel_tables_reproduce_the_delay_table(cfg):
+    w = W.CONFIGS[cfg]
+    plan = _host_plan(w)
+    for r, rg in enumerate(w.ranges):
+        want = oracle.delay_table(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, rg.decim, rg.dm_lo, rg.dm_step, rg.ndm)
+        assert np.array_equal(plan.get_delays(r).astype(np.int64), want), (cfg, r)   # a1 against the oracle
+        assert plan.tile_shape(r)["tiled"] == 1
+        got, rd, shape = _decode(plan, r)
+        assert np.array_equal(got, _padded_delays(plan, r, shape, rd)), (cfg, r)
+        # shared memory of the launch: ring + barriers + prefetch pad fits the 227 KB opt-in limit
+        meta_stage = (shape["chans_per_stage"] // 4 if plan.tile_info(r)["mode"] == 2 else shape["chans_per_stage"]) \
+            * shape["trial_groups"] * 16
+        stage = -(-(shape["chans_per_stage"] * shape["row_superwords"] * 16 + meta_stage) // 128) * 128
+        assert 128 + shape["stages"] * stage + 512 <= 227 * 1024 and shape["stages"] >= 2
+    plan.destroy()
+
+
+def test_lane_widths_and_modes_of_the_five_configs():
+    """Which adder each range gets: delta-coded 16-bit lanes for the fine DM grids of
+    config 3, 8-bit lanes for undecimated coarse grids, 32-bit lanes for decimated uint16."""
+    want = {1: [(16, 0)], 2: [(16, 0)], 3: [(8, 2), (8, 2), (8, 2)], 4: [(16, 0), (4, None)], 5: [(16, 0)]}
+    for cfg, exp in want.items():
+        plan = _host_plan(W.CONFIGS[cfg])
+        for r, (lanes, mode) in enumerate(exp):
+            info = plan.tile_info(r)
+            assert info["lanes"] == lanes and (mode is None or info["mode"] == mode), (cfg, r, info)
+            if lanes == 8:   # 255 + flush*maxval <= 65535, at most 256 flushes
+                maxval = 255 * plan.ranges[r][3]
+                assert 255 + info["flush_chans"] * maxval <= 65535
+                assert -(-plan.tile_shape(r)["cpad"] // info["flush_chans"]) <= 256
+        assert plan.launches() == sum(1 + (2 if (cfg == 4 and r == 0) else 1) for r in range(len(exp)))
+        plan.destroy()
+
+
+def test_ascending_band_has_the_descending_delay_table():
+    w = W.scaled(W.CONFIGS[3], nchans=4096, nsamps=2 ** 16)
+    a, d = _host_plan(w, ascending=True), _host_plan(w)
+    for r in range(len(w.ranges)):
+        assert np.array_equal(a.get_delays(r), d.get_delays(r))
+        assert np.array_equal(a.table(r, 0), d.table(r, 0))
+    assert [a.range_info(r) for r in range(3)] == [d.range_info(r) for r in range(3)]
+
+
+def test_host_only_plans_cannot_execute_and_edge_shapes_build():
+    lib = B._load()
+    for nch, ndm, step, decim, bits in [(1, 5, 10.0, 1, 8), (3, 7, 2.0, 2, 8), (33, 37, 0.7, 1, 8), (64, 9, 3.0, 8, 16),
+                                        (30000, 3, 0.01, 1, 8), (40000, 3, 0.01, 1, 8)]:
+        p = B.Plan(700.0, -300.0 / nch, nch, 1e-3, 20000, [(0.0, step, ndm, decim)], in_bits=bits, host_only=True)
+        got, rd, shape = _decode(p, 0)
+        assert np.array_equal(got, _padded_delays(p, 0, shape, rd))
+        assert lib.dd_execute(p._h, 16, 16, None) == B.DD_ERR_INVALID      # no device half
+        info = p.tile_info(0)
+        if info["mode"] == 2 or decim > 1:          # delta-coded or decimated: 16-bit lanes while they can hold the sums
+            assert info["lanes"] == (8 if bits == 8 and nch <= 30720 else 4)
+        else:                                       # undecimated, coarse steps: byte lanes (uint16: two planes)
+            assert info["lanes"] == (16 if nch <= 30720 else 4)
+        p.destroy()
