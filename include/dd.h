@@ -191,6 +191,30 @@ int dd_plan_set_profiling(dd_plan_t* plan, int32_t max_executes);
 int dd_plan_kernel_times(const dd_plan_t* plan, int32_t slot, int32_t cap, float* ms, int32_t* kind,
                          int32_t* range, int32_t* n);
 
+/* ---- streaming over blocks of spectra --------------------------------------------- */
+
+/*
+ * The thesis's pipeline receives a beam as a sequence of shared-memory blocks (800 or 25600 spectra of 4096
+ * channels).  A stream dedisperses such a sequence: cfg->nsamps is the BLOCK length B (a multiple of
+ * every range's decim).  The stream keeps the last `hist` >= max_r(maxd_r * decim_r) input samples on the device,
+ * puts each new block behind them and runs an ordinary plan over that window of hist + B samples:
+ *   dd_stream_create : builds that plan (query it through dd_stream_plan: out_elems, range_info, ...) and the
+ *                      device window buffers, history zeroed.
+ *   dd_stream_push   : block_dev = the next B samples of every beam, [nbeams][nchans][B] or [nbeams][B][nchans]
+ *                      (cfg->in_layout); out_dev as for dd_execute on the window plan.  Enqueues copy + dd_execute +
+ *                      carry on `cuda_stream`.  For range r the LAST B/decim_r samples of every row are new:
+ *                      row[nout_r - B/decim_r + i] = S_r[j][p*B/decim_r - maxd_r + i] for push number p, so the new
+ *                      pieces of consecutive pushes join exactly (the first maxd_r new samples of push 0 include the
+ *                      zero pre-history); the samples before them repeat the tail of the previous push.
+ * One push per stream may be in flight at a time.
+ */
+typedef struct dd_stream dd_stream_t; /* opaque */
+int dd_stream_create(const dd_config_t* cfg, dd_stream_t** stream_out);
+int dd_stream_push(dd_stream_t* s, const void* block_dev, float* out_dev, void* cuda_stream);
+const dd_plan_t* dd_stream_plan(const dd_stream_t* s);
+int dd_stream_info(const dd_stream_t* s, int64_t* block_samples, int64_t* hist_samples, int64_t* pushes);
+int dd_stream_destroy(dd_stream_t* s);
+
 /* ---- errors ---------------------------------------------------------------------------------- */
 const char* dd_strerror(int code);       /* static string for a dd_status */
 const char* dd_last_cuda_error(void);    /* text of the last CUDA failure seen by this thread ("" if none) */

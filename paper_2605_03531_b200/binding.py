@@ -23,6 +23,7 @@ SYMBOLS = [
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
     "dd_plan_create_host", "dd_plan_tile_shape", "dd_plan_table",
+    "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
 ]
 
@@ -76,6 +77,12 @@ def _load():
         lib.dd_plan_set_kernel.argtypes = [vp, i32]
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
         lib.dd_plan_create_host.argtypes = [P(dd_config_t), P(vp)]
+        lib.dd_stream_create.argtypes = [P(dd_config_t), P(vp)]
+        lib.dd_stream_push.argtypes = [vp, vp, vp, vp]
+        lib.dd_stream_plan.argtypes = [vp]
+        lib.dd_stream_plan.restype = vp
+        lib.dd_stream_info.argtypes = [vp, P(ctypes.c_int64), P(ctypes.c_int64), P(ctypes.c_int64)]
+        lib.dd_stream_destroy.argtypes = [vp]
         lib.dd_plan_tile_shape.argtypes = [vp, i32] + [P(i32)] * 7
         lib.dd_plan_table.argtypes = [vp, i32, i32, vp, ctypes.c_int64, P(ctypes.c_int64)]
         lib.dd_plan_set_profiling.argtypes = [vp, i32]
@@ -150,7 +157,8 @@ class Plan:
     # -- dd_plan_destroy
     def destroy(self) -> None:
         if getattr(self, "_h", None):
-            _load().dd_plan_destroy(self._h)
+            if getattr(self, "_owned", True):
+                _load().dd_plan_destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -267,3 +275,49 @@ class Plan:
         base = beam * self.beam_stride() + info["offset"]
         flat = out.reshape(-1)[base: base + info["ndm"] * info["pitch"]]
         return flat.reshape(info["ndm"], info["pitch"])[:, : info["nout"]]
+
+
+class Stream:
+    """Owns a dd_stream_t*: dedispersion of a sequence of blocks with a carried halo (dd_stream_* of include/dd.h).
+    `nsamps` of the description is the block length."""
+
+    def __init__(self, f_top_mhz: float, chan_width_mhz: float, nchans: int, tsamp_s: float, block_samps: int,
+                 ranges: Sequence[Tuple[float, float, int, int]], nbeams: int = 1, in_bits: int = 8,
+                 in_layout: int = DD_LAYOUT_CHANNEL_MAJOR):
+        lib = _load()
+        arr = (dd_range_t * max(1, len(ranges)))()
+        for i, (lo, step, ndm, decim) in enumerate(ranges):
+            arr[i] = dd_range_t(float(lo), float(step), int(ndm), int(decim))
+        cfg = dd_config_t(float(f_top_mhz), float(chan_width_mhz), int(nchans), float(tsamp_s), int(block_samps),
+                          int(nbeams), int(in_bits), len(ranges), arr, int(in_layout))
+        h = ctypes.c_void_p()
+        _chk(lib.dd_stream_create(ctypes.byref(cfg), ctypes.byref(h)), "dd_stream_create")
+        self._h = h
+        plan = Plan.__new__(Plan)           # non-owning view of the window plan, for the queries
+        plan._h = ctypes.c_void_p(lib.dd_stream_plan(h))
+        plan._owned = False
+        plan.nranges = len(ranges)
+        plan.nchans, plan.nbeams, plan.in_bits = int(nchans), int(nbeams), int(in_bits)
+        plan.ranges = [(float(a), float(b), int(c), int(d)) for a, b, c, d in ranges]
+        self.plan = plan
+        b, hs, n = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        _chk(lib.dd_stream_info(h, ctypes.byref(b), ctypes.byref(hs), ctypes.byref(n)), "dd_stream_info")
+        self.block, self.hist = b.value, hs.value
+        plan.nsamps = self.block + self.hist
+
+    def push(self, block_dev, out_dev, stream=None) -> None:
+        bp = block_dev if isinstance(block_dev, int) else block_dev.data_ptr()
+        op = out_dev if isinstance(out_dev, int) else out_dev.data_ptr()
+        _chk(_load().dd_stream_push(self._h, bp, op, _stream_ptr(stream)), "dd_stream_push")
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None):
+            self.plan._h = None
+            _load().dd_stream_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -340,3 +340,39 @@ def test_bad_layout_and_zero_width_are_rejected():
     with pytest.raises(B.DDError) as e:   # ascending band whose lowest channel is not above 0 MHz
         B.Plan(-10.0, 1.0, 16, 1.024e-3, 4096, [(0.0, 1.0, 3, 1)])
     assert e.value.code == B.DD_ERR_INVALID
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+def test_streaming_blocks_join_exactly(layout):
+    """dd_stream_*: a long filterbank pushed block by block (PAPER.md:351 ring-buffer blocks) with a carried halo.
+    The new samples of consecutive pushes, concatenated, are the oracle's dedispersion of the whole series."""
+    import torch
+    from paper_2605_03531_b200 import binding as B
+    nch, block, npush = 64, 4096, 5
+    w = W.Workload("stream", 750.0, -200.0 / nch, nch, 1.31072e-3, block * npush, 2, 8,
+                   (W.DMRange(0.0, 0.1, 120, 1), W.DMRange(30.0, 4.0, 50, 1), W.DMRange(200.0, 0.5, 60, 4)), 1, 0, 0)
+    x = _rng_filterbank(w.nbeams, nch, w.nsamps, 8, 4242)
+    want = oracle_full(w, x)                       # [beam][range] -> [ndm][N/k - maxd]
+    st = B.Stream(w.f_top_mhz, w.chan_width_mhz, nch, w.tsamp_s, block,
+                  [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], nbeams=2, in_layout=layout)
+    assert st.hist % 64 == 0 and st.block == block
+    out = torch.empty(st.plan.out_elems(), dtype=torch.float32, device="cuda")
+    pieces = [[[] for _ in w.ranges] for _ in range(w.nbeams)]
+    for p in range(npush):
+        blk = x[:, :, p * block:(p + 1) * block]
+        blk = np.ascontiguousarray(blk.transpose(0, 2, 1) if layout == 1 else blk)
+        st.push(torch.from_numpy(blk).cuda(), out, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        flat = out.cpu().numpy()
+        for b in range(w.nbeams):
+            for r, rg in enumerate(w.ranges):
+                rows = st.plan.view_range(flat, r, beam=b)
+                pieces[b][r].append(rows[:, rows.shape[1] - block // rg.decim:].copy())
+    for b in range(w.nbeams):
+        for r, rg in enumerate(w.ranges):
+            got = np.concatenate(pieces[b][r], axis=1)
+            maxd = st.plan.range_info(r)["maxd"]
+            ref = want[b][r]
+            assert ref.shape[1] == got.shape[1] - maxd
+            assert np.array_equal(got[:, maxd:].view(np.uint32), ref.view(np.uint32)), (b, r)
+    st.destroy()
