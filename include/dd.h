@@ -98,6 +98,14 @@ typedef struct dd_plan dd_plan_t; /* opaque */
 int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out);
 
 /*
+ * dd_plan_create_tail: a plan over cfg->nsamps input samples that produces, for every range, only the outputs
+ * whose sums end in the last new_samps input samples: rows of nout_r = new_samps/decim_r + (0..15/decim_r) samples
+ * ending at the same last sample as dd_plan_create's rows.  Each range skips the leading input it does not need
+ * (in steps of 16 samples).  Used by the stream calls below; layouts and queries as for dd_plan_create.
+ */
+int dd_plan_create_tail(const dd_config_t* cfg, int64_t new_samps, dd_plan_t** plan_out);
+
+/*
  * dd_plan_create_host: the host half of dd_plan_create only -- validation, delay tables (Eq. 1.1), per-range
  * sizes, tile shapes and the tables the tiled kernel reads -- without any CUDA call.  The plan answers every
  * query below but cannot execute (dd_execute returns DD_ERR_INVALID).  For inspection and CPU-side tests.
@@ -197,7 +205,7 @@ int dd_plan_kernel_times(const dd_plan_t* plan, int32_t slot, int32_t cap, float
  * The thesis's pipeline receives a beam as a sequence of shared-memory blocks (800 or 25600 spectra of 4096
  * channels).  A stream dedisperses such a sequence: cfg->nsamps is the BLOCK length B (a multiple of
  * every range's decim).  The stream keeps the last `hist` >= max_r(maxd_r * decim_r) input samples on the device,
- * puts each new block behind them and runs an ordinary plan over that window of hist + B samples:
+ * puts each new block behind them and runs a tail plan (dd_plan_create_tail, new_samps = B) over that window:
  *   dd_stream_create : builds that plan (query it through dd_stream_plan: out_elems, range_info, ...) and the
  *                      device window buffers, history zeroed.
  *   dd_stream_push   : block_dev = the next B samples of every beam, [nbeams][nchans][B] or [nbeams][B][nchans]
@@ -205,7 +213,7 @@ int dd_plan_kernel_times(const dd_plan_t* plan, int32_t slot, int32_t cap, float
  *                      carry on `cuda_stream`.  For range r the LAST B/decim_r samples of every row are new:
  *                      row[nout_r - B/decim_r + i] = S_r[j][p*B/decim_r - maxd_r + i] for push number p, so the new
  *                      pieces of consecutive pushes join exactly (the first maxd_r new samples of push 0 include the
- *                      zero pre-history); the samples before them repeat the tail of the previous push.
+ *                      zero pre-history); the up to 15/decim_r samples before them repeat the previous push.
  * One push per stream may be in flight at a time.
  */
 typedef struct dd_stream dd_stream_t; /* opaque */

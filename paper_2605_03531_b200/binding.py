@@ -22,7 +22,7 @@ SYMBOLS = [
     "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
-    "dd_plan_create_host", "dd_plan_tile_shape", "dd_plan_table",
+    "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_tile_shape", "dd_plan_table",
     "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
 ]
@@ -77,6 +77,7 @@ def _load():
         lib.dd_plan_set_kernel.argtypes = [vp, i32]
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
         lib.dd_plan_create_host.argtypes = [P(dd_config_t), P(vp)]
+        lib.dd_plan_create_tail.argtypes = [P(dd_config_t), ctypes.c_int64, P(vp)]
         lib.dd_stream_create.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_stream_push.argtypes = [vp, vp, vp, vp]
         lib.dd_stream_plan.argtypes = [vp]

@@ -58,6 +58,7 @@ struct RangePlan {
   double dm_lo = 0, dm_step = 0;
   int ndm = 0, decim = 1;
   int64_t ns = 0, maxd = 0, nout = 0, pitch = 0, offset = 0;
+  int64_t in_off = 0;  // first input sample this range reads (0 unless the plan keeps only the tail: dd_plan_create_tail)
   std::vector<int32_t> delays;  // host copy [ndm][nchans]
   // tiled kernel shape
   int NL = 8;        // lanes per superword
@@ -100,6 +101,7 @@ struct dd_plan {
   int layout = 0;      // DD_LAYOUT_* of the caller's input
   int ascending = 0;   // caller's channel c is internal channel nchans-1-c
   int64_t nsamps = 0;
+  int64_t tail_new = 0;  // > 0: every range produces only its last tail_new/decim (+ < 16) samples
   std::vector<dd::RangePlan> ranges;
   int64_t beam_stride = 0, out_elems = 0;
   int64_t dm_samples = 0, adds = 0;

@@ -74,7 +74,7 @@ __device__ __forceinline__ void load_lane4(const Tin* __restrict__ row, int64_t 
 template <typename Tin, int K, int NL>
 __global__ void __launch_bounds__(256) dd_pack_kernel(const Tin* __restrict__ in, uint4* __restrict__ P, int nchans,
                                                       int Cpad, int64_t nsamps, int64_t ns_r, int64_t H, int64_t Wp,
-                                                      int rev) {
+                                                      int rev, int64_t off) {
   const int64_t i0 = 4 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
   if (i0 >= Wp) return;
   const int c = blockIdx.y;
@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(256) dd_pack_kernel(const Tin* __restrict__ in
     for (int e = 0; e < 4; ++e) dst[e] = z;
     return;
   }
-  const Tin* row = in + ((int64_t)beam * nchans + (rev ? nchans - 1 - c : c)) * nsamps;  // rev: ascending band
+  const Tin* row = in + ((int64_t)beam * nchans + (rev ? nchans - 1 - c : c)) * nsamps + off;  // rev: ascending band
   uint32_t v[NL][4];
 #pragma unroll
   for (int m = 0; m < NL; ++m) load_lane4<Tin, K>(row, i0 + (int64_t)m * H, ns_r, v[m]);
@@ -118,7 +118,7 @@ static cudaError_t launch_pack_t(const dd_plan* p, const RangePlan& r, const voi
   const Tin* in = static_cast<const Tin*>(in_dev);
 #define DD_PACK(K)                                                                                              \
   dd_pack_kernel<Tin, K, NL><<<grid, block, 0, stream>>>(in, P, p->nchans, r.Cpad, p->nsamps, r.ns, r.H, r.Wp, \
-                                                         p->ascending);                                           \
+                                                         p->ascending, r.in_off);                                 \
   break
   switch (r.decim) {
     case 1: DD_PACK(1);
@@ -137,7 +137,7 @@ static cudaError_t launch_pack_t(const dd_plan* p, const RangePlan& r, const voi
 template <typename Tin>
 __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restrict__ in, uint4* __restrict__ P0,
                                                             uint4* __restrict__ P1, int nchans, int Cpad, int64_t nsamps,
-                                                            int64_t H, int64_t Wp, int rev) {
+                                                            int64_t ns_r, int64_t H, int64_t Wp, int rev, int64_t off) {
   const int64_t i0 = 4 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
   if (i0 >= Wp) return;
   const int c = blockIdx.y;
@@ -153,14 +153,14 @@ __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restric
     }
     return;
   }
-  const Tin* row = in + ((int64_t)beam * nchans + (rev ? nchans - 1 - c : c)) * nsamps;
+  const Tin* row = in + ((int64_t)beam * nchans + (rev ? nchans - 1 - c : c)) * nsamps + off;
   uint32_t lo[4][4] = {}, hi[4][4] = {};  // [superword e][word q]
 #pragma unroll
   for (int m = 0; m < 16; ++m) {
     const int64_t s = i0 + (int64_t)m * H;
     uint32_t v[4];
     const Tin* src = row + s;
-    if (s + 4 <= nsamps && (reinterpret_cast<uintptr_t>(src) & (4 * sizeof(Tin) - 1)) == 0) {
+    if (s + 4 <= ns_r && (reinterpret_cast<uintptr_t>(src) & (4 * sizeof(Tin) - 1)) == 0) {
       if constexpr (kTwo) {
         const uint2 t = __ldg(reinterpret_cast<const uint2*>(src));
         v[0] = t.x & 0xffffu, v[1] = t.x >> 16, v[2] = t.y & 0xffffu, v[3] = t.y >> 16;
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(256) dd_pack_bytes_kernel(const Tin* __restric
       }
     } else {
 #pragma unroll
-      for (int e = 0; e < 4; ++e) v[e] = s + e < nsamps ? (uint32_t)row[s + e] : 0u;
+      for (int e = 0; e < 4; ++e) v[e] = s + e < ns_r ? (uint32_t)row[s + e] : 0u;
     }
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
@@ -197,7 +197,8 @@ constexpr int kTcCh = 128, kTcTi = 4;
 template <typename Tin, int NL>
 __global__ void __launch_bounds__(256) dd_pack_tc_kernel(const Tin* __restrict__ in, uint4* __restrict__ P0,
                                                          uint4* __restrict__ P1, int nchans, int Cpad, int64_t nsamps,
-                                                         int64_t ns_r, int decim, int64_t H, int64_t Wp, int rev) {
+                                                         int64_t ns_r, int decim, int64_t H, int64_t Wp, int rev,
+                                                         int64_t off) {
   __shared__ uint32_t vals[NL][kTcTi][kTcCh + 1];
   const int64_t i0 = (int64_t)blockIdx.x * kTcTi;
   const int c0 = blockIdx.y * kTcCh;
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(256) dd_pack_tc_kernel(const Tin* __restrict__
       const int64_t s = i0 + ti + (int64_t)m * H;  // decimated sample index
       uint32_t a[4] = {0, 0, 0, 0};
       if (c < nchans && s < ns_r) {
-        const Tin* src = x + (int64_t)decim * s * nchans + c;
+        const Tin* src = x + ((int64_t)decim * s + off) * nchans + c;
 #pragma unroll 4
         for (int q = 0; q < decim; ++q) {
           if constexpr (sizeof(Tin) == 1) {
@@ -235,7 +236,7 @@ __global__ void __launch_bounds__(256) dd_pack_tc_kernel(const Tin* __restrict__
       const int64_t s = i0 + ti + (int64_t)m * H;  // decimated sample index
       uint32_t a = 0;
       if (c < nchans && s < ns_r) {
-        const Tin* src = x + (int64_t)decim * s * nchans + (rev ? nchans - 1 - c : c);
+        const Tin* src = x + ((int64_t)decim * s + off) * nchans + (rev ? nchans - 1 - c : c);
         for (int q = 0; q < decim; ++q) a += (uint32_t)src[(int64_t)q * nchans];
       }
       vals[m][ti][cl] = a;
@@ -273,7 +274,7 @@ static cudaError_t launch_pack_tc_t(const dd_plan* p, const RangePlan& r, const 
   uint4* P1 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws_offset + r.plane_bytes);
   dim3 grid((unsigned)((r.Wp + kTcTi - 1) / kTcTi), (unsigned)((r.Cpad + kTcCh - 1) / kTcCh), (unsigned)p->nbeams);
   dd_pack_tc_kernel<Tin, NL><<<grid, 256, 0, stream>>>(static_cast<const Tin*>(in_dev), P0, P1, p->nchans, r.Cpad,
-                                                       p->nsamps, r.ns, r.decim, r.H, r.Wp, p->ascending);
+                                                       p->nsamps, r.ns, r.decim, r.H, r.Wp, p->ascending, r.in_off);
   return cudaGetLastError();
 }
 
@@ -294,10 +295,10 @@ cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev
     dim3 grid((unsigned)((r.Wp / 4 + 255) / 256), (unsigned)r.Cpad, (unsigned)p->nbeams);
     if (p->in_bits == 8)
       dd_pack_bytes_kernel<uint8_t><<<grid, block, 0, stream>>>(static_cast<const uint8_t*>(in_dev), P0, nullptr, p->nchans,
-                                                                r.Cpad, p->nsamps, r.H, r.Wp, p->ascending);
+                                                                r.Cpad, p->nsamps, r.ns, r.H, r.Wp, p->ascending, r.in_off);
     else
       dd_pack_bytes_kernel<uint16_t><<<grid, block, 0, stream>>>(static_cast<const uint16_t*>(in_dev), P0, P1, p->nchans,
-                                                                 r.Cpad, p->nsamps, r.H, r.Wp, p->ascending);
+                                                                 r.Cpad, p->nsamps, r.ns, r.H, r.Wp, p->ascending, r.in_off);
     return cudaGetLastError();
   }
   if (p->in_bits == 8) {
@@ -313,7 +314,8 @@ template <typename Tin>
 __global__ void __launch_bounds__(256) dd_direct_kernel(const Tin* __restrict__ in, const int32_t* __restrict__ delays,
                                                         float* __restrict__ out, int nchans, long long nsamps, int decim,
                                                         long long nout, long long pitch, long long out_beam_stride,
-                                                        long long chan_stride, long long time_stride, int rev) {
+                                                        long long chan_stride, long long time_stride, int rev,
+                                                        long long off) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nout) return;
   const int j = blockIdx.y;
@@ -322,7 +324,7 @@ __global__ void __launch_bounds__(256) dd_direct_kernel(const Tin* __restrict__ 
   const int32_t* d = delays + (long long)j * nchans;  // internal order: channel 0 = highest frequency
   uint32_t s = 0;
   for (int c = 0; c < nchans; ++c) {
-    const Tin* src = x + (long long)(rev ? nchans - 1 - c : c) * chan_stride + (long long)decim * (t + d[c]) * time_stride;
+    const Tin* src = x + (long long)(rev ? nchans - 1 - c : c) * chan_stride + ((long long)decim * (t + d[c]) + off) * time_stride;
     for (int q = 0; q < decim; ++q) s += (uint32_t)src[q * time_stride];
   }
   out[(long long)beam * out_beam_stride + (long long)j * pitch + t] = __uint2float_rn(s);
@@ -337,11 +339,11 @@ cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_d
   if (p->in_bits == 8) {
     dd_direct_kernel<uint8_t><<<grid, block, 0, stream>>>(static_cast<const uint8_t*>(in_dev), r.d_delays,
                                                           out_dev + r.offset, p->nchans, p->nsamps, r.decim, r.nout,
-                                                          r.pitch, p->beam_stride, cs, ts, p->ascending);
+                                                          r.pitch, p->beam_stride, cs, ts, p->ascending, r.in_off);
   } else {
     dd_direct_kernel<uint16_t><<<grid, block, 0, stream>>>(static_cast<const uint16_t*>(in_dev), r.d_delays,
                                                            out_dev + r.offset, p->nchans, p->nsamps, r.decim, r.nout,
-                                                           r.pitch, p->beam_stride, cs, ts, p->ascending);
+                                                           r.pitch, p->beam_stride, cs, ts, p->ascending, r.in_off);
   }
   return cudaGetLastError();
 }

@@ -296,7 +296,7 @@ const char* dd_strerror(int code) {
 const char* dd_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 
 // Host half of a plan: validation, delay tables, tile shapes, the tables of the tiled kernel.  No CUDA call.
-static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) {
+static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new = 0) {
   if (!cfg || !plan_out) return DD_ERR_INVALID;
   *plan_out = nullptr;
   if (cfg->nchans < 1 || !(cfg->chan_width_mhz != 0.0) || !(cfg->tsamp_s > 0.0) || cfg->nsamps < 1 ||
@@ -329,6 +329,7 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) {
     p->nbeams = cfg->nbeams;
     p->in_bits = cfg->in_bits;
     p->nsamps = cfg->nsamps;
+    p->tail_new = tail_new;
     p->ranges.resize(cfg->nranges);
     int64_t offset = 0;
     for (int i = 0; i < cfg->nranges && rc == DD_OK; ++i) {
@@ -337,9 +338,12 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) {
       r.dm_step = cfg->ranges[i].dm_step;
       r.ndm = cfg->ranges[i].ndm;
       r.decim = cfg->ranges[i].decim;
-      r.ns = p->nsamps / r.decim;
       if (!build_delays(*p, r)) { rc = DD_ERR_TOO_SHORT; break; }
       r.maxd = r.delays[(size_t)(r.ndm - 1) * p->nchans + (p->nchans - 1)];
+      // a tail plan skips the input this range does not need for its last tail_new/decim outputs (16-sample
+      // granularity keeps the vector loads of the pack kernels aligned)
+      if (tail_new > 0) r.in_off = std::max<int64_t>(0, (p->nsamps - tail_new - r.maxd * r.decim) / 16 * 16);
+      r.ns = (p->nsamps - r.in_off) / r.decim;
       r.nout = r.ns - r.maxd;
       if (r.nout < 1) { rc = DD_ERR_TOO_SHORT; break; }
       r.pitch = round_up(r.nout, 32);
@@ -376,9 +380,18 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) {
 
 int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) { return plan_create_host(cfg, plan_out); }
 
-int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) {
+static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new);
+
+int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) { return plan_create_device(cfg, plan_out, 0); }
+
+int dd_plan_create_tail(const dd_config_t* cfg, int64_t new_samps, dd_plan_t** plan_out) {
+  if (new_samps < 1 || !cfg || new_samps > cfg->nsamps) return DD_ERR_INVALID;
+  return plan_create_device(cfg, plan_out, new_samps);
+}
+
+static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new) {
   dd_plan* p = nullptr;
-  int rc = plan_create_host(cfg, &p);
+  int rc = plan_create_host(cfg, &p, tail_new);
   if (rc != DD_OK) return rc;
   *plan_out = nullptr;
   cudaError_t e = cudaGetDevice(&p->device);

@@ -3,12 +3,13 @@
 // The thesis's pipeline receives a beam as a sequence of shared-memory blocks (800 or 25600 spectra of 4096
 // channels).  A dispersed pulse straddles block boundaries: the sum for output sample t needs
 // input up to t + maxd.  A stream keeps the last `hist` input samples on the device, places every new block
-// behind them and runs the ordinary plan (dd_execute) on that window; per range the last block/decim output
-// samples of each trial are new, and consecutive pushes join without a gap or an overlap:
+// behind them and runs a tail plan (dd_plan_create_tail: each range reads only the end of the window it needs)
+// on that window; per range the last block/decim output samples of each trial are new, and consecutive pushes
+// join without a gap or an overlap:
 //
 //   window of push p   = input samples [p*B - hist, (p+1)*B)            (zeros before the first block)
-//   output t' of range r = S_r[j][(p*B - hist)/decim_r + t'],  t' < nout_r = (hist + B)/decim_r - maxd_r
-//   new samples        = t' in [nout_r - B/decim_r, nout_r)  <->  absolute index [p*B/k - maxd_r, (p+1)*B/k - maxd_r)
+//   rows of range r    = nout_r = B/decim_r + (< 16) samples, the last one being S_r[j][(p+1)*B/k - maxd_r - 1]
+//   new samples        = the last B/decim_r of a row  <->  absolute index [p*B/k - maxd_r, (p+1)*B/k - maxd_r)
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -66,7 +67,8 @@ int dd_stream_create(const dd_config_t* cfg, dd_stream_t** stream_out) {
   s->layout = cfg->in_layout;
   dd_config_t inner = *cfg;
   inner.nsamps = hist + cfg->nsamps;
-  int rc = dd_plan_create(&inner, &s->plan);
+  // only the last block/decim (+ < 16) samples of every row are computed: no work is repeated between pushes
+  int rc = dd_plan_create_tail(&inner, cfg->nsamps, &s->plan);
   if (rc != DD_OK) {
     delete s;
     return rc;
