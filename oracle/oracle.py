@@ -14,7 +14,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle_dedisp.c")
 _LIB = os.path.join(_HERE, "liboracle_dedisp.so")
+_SRC_SPS = os.path.join(_HERE, "oracle_sps.c")
+_LIB_SPS = os.path.join(_HERE, "liboracle_sps.so")
 _lib = None
+_lib_sps = None
 
 _ERRORS = {-1: "invalid argument", -2: "window exceeds the valid span (too short)", -3: "out of memory"}
 
@@ -28,6 +31,13 @@ def build(force: bool = False) -> str:
             check=True,
         )
         os.replace(tmp, _LIB)
+    if force or not os.path.exists(_LIB_SPS) or os.path.getmtime(_LIB_SPS) < os.path.getmtime(_SRC_SPS):
+        tmp = _LIB_SPS + ".tmp.%d" % os.getpid()
+        subprocess.run(  # no FMA contraction: the operation order of oracle_sps.c is part of its definition
+            ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC_SPS, "-lm"],
+            check=True,
+        )
+        os.replace(tmp, _LIB_SPS)
     return _LIB
 
 
@@ -118,3 +128,32 @@ def dedisperse(y: np.ndarray, delays: np.ndarray, sel=None, t0: int = 0, nt: int
     rc = _load().oracle_dedisperse(_ptr(y), nchans, ns_r, _ptr(delays), ndm, _ptr(sel_arr), len(sel_arr), t0, nt, _ptr(out))
     _check(rc, "dedisperse")
     return out
+
+
+def sps(rows: np.ndarray, n: int, nwidths: int, threshold: float):
+    """Boxcar single-pulse search on rows of the DM-time plane (oracle_sps.c).
+
+    rows: float32 [nrows][pitch], the first n samples of each row valid.  Returns dict of
+    snr float32 [nrows][K], tmax int32, count int32, mean float64 [nrows], sigma float64 [nrows].
+    """
+    global _lib_sps
+    if _lib_sps is None:
+        build()
+        lib = ctypes.CDLL(_LIB_SPS)
+        vp, i64 = ctypes.c_void_p, ctypes.c_int64
+        lib.oracle_sps.argtypes = [vp, i64, i64, i64, ctypes.c_int, ctypes.c_double, vp, vp, vp, vp, vp]
+        lib.oracle_sps.restype = ctypes.c_int
+        _lib_sps = lib
+    if rows.ndim != 2 or rows.dtype != np.float32:
+        raise ValueError("oracle sps: rows must be a 2-D float32 array")
+    rows = np.ascontiguousarray(rows)
+    nrows, pitch = rows.shape
+    snr = np.empty((nrows, nwidths), dtype=np.float32)
+    tmax = np.empty((nrows, nwidths), dtype=np.int32)
+    count = np.empty((nrows, nwidths), dtype=np.int32)
+    mean = np.empty(nrows, dtype=np.float64)
+    sigma = np.empty(nrows, dtype=np.float64)
+    rc = _lib_sps.oracle_sps(_ptr(rows), nrows, pitch, n, nwidths, float(threshold), _ptr(snr), _ptr(tmax), _ptr(count),
+                             _ptr(mean), _ptr(sigma))
+    _check(rc, "sps")
+    return {"snr": snr, "tmax": tmax, "count": count, "mean": mean, "sigma": sigma}
