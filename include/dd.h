@@ -223,6 +223,26 @@ const dd_plan_t* dd_stream_plan(const dd_stream_t* s);
 int dd_stream_info(const dd_stream_t* s, int64_t* block_samples, int64_t* hist_samples, int64_t* pushes);
 int dd_stream_destroy(dd_stream_t* s);
 
+/* ---- single-pulse search on the DM-time plane -------------------------------------- */
+
+/*
+ * "The SPS module searches for statistically significant single pulses above a user-specified
+ * threshold using time-domain boxcar filtering."  Per row x[0..nout_r) of the plane written by dd_execute:
+ *     mean = (sum x)/n, sigma = sqrt((sum x^2)/n - mean^2)                        (sums exact, then IEEE double)
+ *     for k < nwidths, w = 2^k:  B[t] = sum_{i<w} x[t+i], t <= n-w
+ *         tmax  = first t with the largest B,   snr = sigma > 0 ? (B[tmax] - w*mean)/(sigma*sqrt(w)) : 0
+ *         count = number of t with B[t] > w*mean + threshold*sigma*sqrt(w)
+ *     (w > n: snr 0, tmax -1, count 0).
+ * dd_sps_rows: rows of the outputs = nbeams * (sum of ndm_r); row = beam*(sum ndm) + (trials of earlier ranges) + j.
+ * dd_sps_execute: plane_dev = the output buffer of dd_execute for this plan; snr_dev / tmax_dev / count_dev hold
+ *     rows*nwidths elements ([row][k]); 1 <= nwidths <= 12; threshold finite.  Enqueues one kernel per range on
+ *     `cuda_stream`.  DD_ERR_OVERFLOW if (nchans*(2^in_bits-1)*decim)^2 * nout_r >= 2^63 for some range (sum x^2
+ *     would not be exact; uint8 SPOTLIGHT-shaped data is far below).
+ */
+int dd_sps_rows(const dd_plan_t* plan, int64_t* rows);
+int dd_sps_execute(const dd_plan_t* plan, const float* plane_dev, int32_t nwidths, double threshold, float* snr_dev,
+                   int32_t* tmax_dev, int32_t* count_dev, void* cuda_stream);
+
 /* ---- errors ---------------------------------------------------------------------------------- */
 const char* dd_strerror(int code);       /* static string for a dd_status */
 const char* dd_last_cuda_error(void);    /* text of the last CUDA failure seen by this thread ("" if none) */

@@ -23,7 +23,7 @@ SYMBOLS = [
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
     "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_tile_shape", "dd_plan_table",
-    "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
+    "dd_sps_rows", "dd_sps_execute", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
 ]
 
@@ -78,6 +78,8 @@ def _load():
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
         lib.dd_plan_create_host.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_plan_create_tail.argtypes = [P(dd_config_t), ctypes.c_int64, P(vp)]
+        lib.dd_sps_rows.argtypes = [vp, P(ctypes.c_int64)]
+        lib.dd_sps_execute.argtypes = [vp, vp, i32, ctypes.c_double, vp, vp, vp, vp]
         lib.dd_stream_create.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_stream_push.argtypes = [vp, vp, vp, vp]
         lib.dd_stream_plan.argtypes = [vp]
@@ -255,6 +257,18 @@ class Plan:
         buf = np.empty(n.value // 4, dtype=np.uint32 if which == 0 else np.int32)
         _chk(_load().dd_plan_table(self._h, r, which, buf.ctypes.data, n.value, ctypes.byref(n)), "dd_plan_table")
         return buf
+
+    # -- single-pulse search on the DM-time plane
+    def sps_rows(self) -> int:
+        v = ctypes.c_int64()
+        _chk(_load().dd_sps_rows(self._h, ctypes.byref(v)), "dd_sps_rows")
+        return v.value
+
+    def sps_execute(self, plane_dev, nwidths: int, threshold: float, snr_dev, tmax_dev, count_dev, stream=None) -> None:
+        """All buffers are torch CUDA tensors (or raw device pointers): float32 / int32 / int32 [rows][nwidths]."""
+        ptr = lambda a: a if isinstance(a, int) else a.data_ptr()  # noqa: E731
+        _chk(_load().dd_sps_execute(self._h, ptr(plane_dev), int(nwidths), float(threshold), ptr(snr_dev), ptr(tmax_dev),
+                                    ptr(count_dev), _stream_ptr(stream)), "dd_sps_execute")
 
     def set_profiling(self, max_executes: int) -> None:
         _chk(_load().dd_plan_set_profiling(self._h, int(max_executes)), "dd_plan_set_profiling")

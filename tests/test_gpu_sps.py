@@ -1,0 +1,80 @@
+"""GPU parity of the boxcar single-pulse search (dd_sps_execute) against oracle/oracle_sps.c.
+The oracle's input is the ORACLE's own DM-time plane, never the GPU's; both must agree bit for bit (float snr
+included: the few double operations per row are done in the same order with round-to-nearest on both sides)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_03531_b200 import workloads as W
+
+from _util import gpu_run, oracle_full
+
+pytestmark = pytest.mark.gpu
+
+
+def _sps_both(w, x, K, thr):
+    import torch
+    plan, flat = gpu_run(w, x, 2)
+    rows = plan.sps_rows()
+    plane = torch.from_numpy(flat).cuda()
+    snr = torch.full((rows, K), -7.0, dtype=torch.float32, device="cuda")
+    tmax = torch.full((rows, K), -7, dtype=torch.int32, device="cuda")
+    cnt = torch.full((rows, K), -7, dtype=torch.int32, device="cuda")
+    plan.sps_execute(plane, K, thr, snr, tmax, cnt, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    got = {"snr": snr.cpu().numpy(), "tmax": tmax.cpu().numpy(), "count": cnt.cpu().numpy()}
+    want_planes = oracle_full(w, x)
+    ref = {"snr": [], "tmax": [], "count": []}
+    for b in range(w.nbeams):
+        for r in range(len(w.ranges)):
+            res = oracle.sps(np.ascontiguousarray(want_planes[b][r]), want_planes[b][r].shape[1], K, thr)
+            for k in ref:
+                ref[k].append(res[k])
+    ref = {k: np.concatenate(v, axis=0) for k, v in ref.items()}
+    return plan, got, ref
+
+
+@pytest.mark.parametrize("K,thr", [(1, 3.0), (6, 5.0), (12, 2.5)])
+def test_sps_matches_oracle_multirange(K, thr):
+    w = W.scaled(W.CONFIGS[3], nchans=96, nsamps=2 ** 14 + 37, nbeams=2,
+                 ranges=[W.DMRange(0.0, 0.1, 37, 1), W.DMRange(40.0, 3.0, 21, 1), W.DMRange(600.0, 0.5, 19, 4)])
+    x = W.generate(w)
+    x[0, :, 6000:6012] = np.minimum(x[0, :, 6000:6012].astype(np.int32) + 9, 255).astype(np.uint8)   # a DM-0 pulse
+    plan, got, ref = _sps_both(w, x, K, thr)
+    assert got["tmax"].shape == (2 * (37 + 21 + 19), K)
+    for k in ("tmax", "count"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
+    # the injected pulse is found at DM 0 by a filter of about its width
+    assert ref["snr"][0].max() > 6 and abs(int(ref["tmax"][0, np.argmax(ref["snr"][0])]) - 6000) <= 16
+
+
+def test_sps_short_rows_constant_rows_and_wide_filters():
+    """Rows shorter than the widest filters and than one tile; a constant plane (sigma = 0)."""
+    nch = 8
+    w = W.Workload("spsedge", 500.0, -200.0 / nch, nch, 1.024e-3, 700, 1, 8, (W.DMRange(0.0, 1.0, 5, 1), W.DMRange(0.0, 1.0, 3, 4)), 1, 0, 0)
+    x = np.full((1, nch, 700), 100, dtype=np.uint8)
+    plan, got, ref = _sps_both(w, x, 12, 1.0)
+    for k in ("tmax", "count"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert (got["snr"] == 0).all() and (got["tmax"][:, -1] == -1).all()
+    x = np.random.default_rng(3).integers(0, 256, size=(1, nch, 700), dtype=np.uint8)
+    plan, got, ref = _sps_both(w, x, 12, -50.0)
+    for k in ("tmax", "count"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
+
+
+def test_sps_rejects_inexact_sums_and_bad_arguments():
+    import torch
+    from paper_2605_03531_b200 import binding as B
+    plan = B.Plan(500.0, -200.0 / 4096, 4096, 1.31072e-3, 2 ** 18, [(0.0, 1.0, 2, 1)], in_bits=16)   # (4096*65535)^2 * n > 2^63
+    buf = torch.zeros(16, device="cuda")
+    with pytest.raises(B.DDError) as e:
+        plan.sps_execute(buf, 4, 5.0, buf, buf, buf)
+    assert e.value.code == B.DD_ERR_OVERFLOW
+    plan8 = B.Plan(500.0, -200.0 / 16, 16, 1e-3, 4096, [(0.0, 1.0, 2, 1)])
+    for K, thr in ((0, 1.0), (13, 1.0), (4, float("nan")), (4, float("inf"))):
+        with pytest.raises(B.DDError) as e:
+            plan8.sps_execute(buf, K, thr, buf, buf, buf)
+        assert e.value.code == B.DD_ERR_INVALID
