@@ -10,10 +10,12 @@
 // round-to-nearest intrinsics in the stated order (no FMA contraction), so the results are bit-exact.
 //
 // One CTA per row.  Phase A: S1, S2 with vector loads and a block reduction.  Phase B: tiles of kTile samples plus
-// a halo of the widest filter are turned into an exclusive prefix sum P in shared memory (int64); every boxcar of
-// every width is then P[t+w] - P[t].  The plane is read twice (the second pass mostly from L2): HBM-bound.
+// a halo of the widest filter are staged in shared memory with coalesced loads and turned into an exclusive prefix
+// sum P (int64); every boxcar of every width is then P[t+w] - P[t].  The plane is read twice (the second pass mostly from L2): HBM-bound.
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <type_traits>
 
 #include "dd_internal.h"
 
@@ -38,19 +40,23 @@ __device__ __forceinline__ unsigned long long shfl_down_u64(unsigned long long v
   return __shfl_down_sync(0xffffffffu, v, o);
 }
 
+// K = number of widths; WIDE = boxcar sums may reach 2^32 (64-bit prefix sums), else 32-bit modular prefix sums
+// (a difference of two of them is the exact boxcar because it is below 2^32).
+template <int K, bool WIDE>
 __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) {
+  using acc_t = typename std::conditional<WIDE, unsigned long long, uint32_t>::type;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  long long* P = reinterpret_cast<long long*>(smem_raw);  // [kSpsTile + halo + 1]
+  acc_t* P = reinterpret_cast<acc_t*>(smem_raw);  // [kSpsTile + halo + 1]
   __shared__ unsigned long long red[2][kSpsThreads / 32];
   __shared__ unsigned long long s_thr[kSpsMaxK];  // B >= s_thr  <=>  B > w*mean + threshold*den
   __shared__ double s_wmean[kSpsMaxK], s_den[kSpsMaxK];
   __shared__ double s_sigma;
   __shared__ unsigned long long s_best[kSpsMaxK][kSpsThreads / 32];
   __shared__ int s_tb[kSpsMaxK][kSpsThreads / 32], s_cnt[kSpsMaxK][kSpsThreads / 32];
-  __shared__ long long s_warp_tot[kSpsThreads / 32];
+  __shared__ unsigned long long s_warp_tot[kSpsThreads / 32];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n = p.n, K = p.K;
+  const int n = p.n;
   const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
 
   // ---------------- phase A: exact sums ---------------------------------------------------------------
@@ -98,52 +104,63 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
   __syncthreads();
 
   // ---------------- phase B: boxcars from a prefix sum per tile -------------------------------------------
-  const int halo = 1 << (K - 1);
+  constexpr int halo = 1 << (K - 1);
   const int span = kSpsTile + halo;          // prefix entries P[0..span]
-  const int per = (span + kSpsThreads - 1) / kSpsThreads;
-  unsigned long long best[kSpsMaxK];
-  int tb[kSpsMaxK], cnt[kSpsMaxK];
+  const int per = ((span + kSpsThreads - 1) / kSpsThreads) | 1;
+  acc_t best[K], thr[K];
+  int tb[K], cnt[K];
 #pragma unroll
-  for (int k = 0; k < kSpsMaxK; ++k) best[k] = 0, tb[k] = 0x7fffffff, cnt[k] = 0;
+  for (int k = 0; k < K; ++k) {
+    // sums are >= 0, so the thread's first window (t = tid) is its first maximum until a larger sum shows up
+    best[k] = 0, tb[k] = tid + (1 << k) <= n ? tid : 0x7fffffff, cnt[k] = 0;
+    // thresholds above the reach of acc_t can never be met: 2^32-1 is below 2^32 only for sums that small
+    thr[k] = WIDE ? (acc_t)s_thr[k] : (s_thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_thr[k]);
+  }
+  bool never[K];  // (narrow sums) threshold not representable: count stays 0
+#pragma unroll
+  for (int k = 0; k < K; ++k) never[k] = !WIDE && s_thr[k] > 0xffffffffull;
 
+  uint32_t* V = reinterpret_cast<uint32_t*>(smem_raw + (size_t)(span + 2) / 2 * 2 * sizeof(acc_t));  // the tile's samples, [span]
   for (int tile0 = 0; tile0 < n; tile0 += kSpsTile) {
-    // thread-local sums of `per` consecutive samples, then a block-wide exclusive scan of the thread totals
-    const int i0 = tid * per;
-    long long loc = 0;
-    for (int i = i0; i < i0 + per && i < span; ++i) {
+    // stage the tile + halo with coalesced loads (samples past the end of the row count as 0)
+    for (int i = tid; i < span; i += kSpsThreads) {
       const int t = tile0 + i;
-      loc += t < n ? (long long)x[t] : 0ll;
+      V[i] = t < n ? (uint32_t)x[t] : 0u;
     }
-    long long inc = loc;
+    __syncthreads();
+    // thread-local sums of `per` consecutive samples (per is odd: conflict-free), then a block-wide exclusive
+    // scan of the thread totals
+    const int i0 = tid * per;
+    acc_t loc = 0;
+    for (int i = i0; i < i0 + per && i < span; ++i) loc += V[i];
+    acc_t inc = loc;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const long long v = __shfl_up_sync(0xffffffffu, inc, o);
+      const acc_t v = __shfl_up_sync(0xffffffffu, inc, o);
       if (lane >= o) inc += v;
     }
     if (lane == 31) s_warp_tot[warp] = inc;
     __syncthreads();
-    long long base = inc - loc;
-    for (int wq = 0; wq < warp; ++wq) base += s_warp_tot[wq];
+    acc_t base = inc - loc;
+    for (int wq = 0; wq < warp; ++wq) base += (acc_t)s_warp_tot[wq];
     if (tid == 0) P[0] = 0;
     for (int i = i0; i < i0 + per && i < span; ++i) {
-      const int t = tile0 + i;
-      base += t < n ? (long long)x[t] : 0ll;   // second read of the thread's samples: L1 hit
+      base += V[i];
       P[i + 1] = base;
     }
     __syncthreads();
+    const bool interior = tile0 + span <= n;  // every window of every width of this tile lies inside the row
     for (int tl = tid; tl < kSpsTile; tl += kSpsThreads) {
       const int t = tile0 + tl;
       if (t >= n) break;
-      const long long p0 = P[tl];
+      const acc_t p0 = P[tl];
 #pragma unroll
-      for (int k = 0; k < kSpsMaxK; ++k) {
-        if (k < K) {
-          const int w = 1 << k;
-          if (t + w <= n) {
-            const unsigned long long b = (unsigned long long)(P[tl + w] - p0);
-            if (tb[k] == 0x7fffffff || b > best[k]) best[k] = b, tb[k] = t;   // t increases: first maximum kept
-            cnt[k] += b >= s_thr[k];
-          }
+      for (int k = 0; k < K; ++k) {
+        const int w = 1 << k;
+        if (interior || t + w <= n) {
+          const acc_t b = P[tl + w] - p0;
+          if (b > best[k]) best[k] = b, tb[k] = t;   // t increases: first maximum kept
+          cnt[k] += (b >= thr[k]) && !never[k];
         }
       }
     }
@@ -152,8 +169,8 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
 
   // ---------------- reduce over the block: larger sum wins, ties go to the smaller t ----------------------
 #pragma unroll
-  for (int k = 0; k < kSpsMaxK; ++k) {
-    if (k < K) {
+  for (int k = 0; k < K; ++k) {
+    {
       unsigned long long b = best[k];
       int t = tb[k], c = cnt[k];
 #pragma unroll
@@ -189,6 +206,18 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
   }
 }
 
+template <int K, bool WIDE>
+static cudaError_t launch_sps(const SpsParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
+  static bool attr_set = false;  // per instantiation
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(dd_sps_kernel<K, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  dd_sps_kernel<K, WIDE><<<grid, kSpsThreads, smem, stream>>>(sp);
+  return cudaGetLastError();
+}
+
 }  // namespace dd
 
 extern "C" {
@@ -214,13 +243,7 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
     rows_per_beam += r.ndm;
   }
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  const size_t smem = (size_t)(dd::kSpsTile + (1 << (nwidths - 1)) + 1) * sizeof(long long);
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(dd::dd_sps_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess)
-      return DD_ERR_CUDA;
-    attr_set = true;
-  }
+  const size_t span = (size_t)dd::kSpsTile + ((size_t)1 << (nwidths - 1));
   int64_t row0 = 0;
   for (const auto& r : p->ranges) {
     dd::SpsParams sp;
@@ -235,8 +258,22 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
     sp.count = count_dev;
     sp.row0 = row0;
     sp.rows_per_beam = rows_per_beam;
-    dd::dd_sps_kernel<<<dim3((unsigned)r.ndm, (unsigned)p->nbeams), dd::kSpsThreads, smem, stream>>>(sp);
-    if (cudaGetLastError() != cudaSuccess) return DD_ERR_CUDA;
+    // 32-bit prefix sums while the widest boxcar of the largest possible samples stays below 2^32
+    const double vmax = (double)p->nchans * (double)((1 << p->in_bits) - 1) * (double)r.decim;
+    const bool wide = vmax * (double)(1 << (nwidths - 1)) >= 4294967296.0;
+    const size_t smem = (span + 2) / 2 * 2 * (wide ? 8 : 4) + span * 4;
+    const dim3 grid((unsigned)r.ndm, (unsigned)p->nbeams);
+    cudaError_t e = cudaErrorInvalidValue;
+#define DD_SPS(K_)                                                                                                  \
+  case K_:                                                                                                          \
+    e = wide ? dd::launch_sps<K_, true>(sp, grid, smem, stream) : dd::launch_sps<K_, false>(sp, grid, smem, stream); \
+    break;
+    switch (nwidths) {
+      DD_SPS(1) DD_SPS(2) DD_SPS(3) DD_SPS(4) DD_SPS(5) DD_SPS(6) DD_SPS(7) DD_SPS(8) DD_SPS(9) DD_SPS(10) DD_SPS(11)
+      DD_SPS(12)
+    }
+#undef DD_SPS
+    if (e != cudaSuccess) return DD_ERR_CUDA;
     row0 += r.ndm;
   }
   return DD_OK;
