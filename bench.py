@@ -273,6 +273,34 @@ def run_ours(args, w):
                "api": "dd_execute_host (C ABI, pinned host buffers)"}
         del hin, hout
 
+    # NEXT-2: boxcar single-pulse search over the plane just written -- an extra, HBM-bound step
+    # reported beside the metric, not inside `value`
+    sps = None
+    if not args.no_sps and w.in_bits == 8:
+        K, thr = 8, 6.0
+        rows = plan.sps_rows()
+        snr = torch.empty((rows, K), dtype=torch.float32, device=dev)
+        tmx = torch.empty((rows, K), dtype=torch.int32, device=dev)
+        cnt = torch.empty((rows, K), dtype=torch.int32, device=dev)
+        for _ in range(2):
+            plan.sps_execute(out, K, thr, snr, tmx, cnt, stream)
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        s0.record(stream)
+        for _ in range(3):
+            plan.sps_execute(out, K, thr, snr, tmx, cnt, stream)
+        s1.record(stream)
+        torch.cuda.synchronize()
+        sps_ms = s0.elapsed_time(s1) / 3
+        plane_bytes = plan.out_elems() * 4
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        sps = {"kernel": "dd_sps_kernel", "widths": K, "threshold": thr, "ms": sps_ms, "rows": rows,
+               "roofline": {"bound": "hbm", "achieved": plane_bytes / (sps_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                            "frac": plane_bytes / (sps_ms * 1e-3) / 1e9 / hbm,
+                            "algorithmic_bytes": "the DM-time plane read once (4 B per DM-trial sample)"},
+               "candidates_above_threshold": int(cnt.sum().item())}
+        del snr, tmx, cnt
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, done, threads, desc = oracle_sample_run(w, x_host, args.ref_trials)
@@ -289,7 +317,7 @@ def run_ours(args, w):
                        "l2": "inputs larger than L2 (1.07 GB input, 4.0 GB packed copy, 3.8 GB output per step)",
                        "parallelism": "replicas: one beam per GPU, no collective"},
             "input_gb_per_s": world * w.nchans * w.nsamps * (w.in_bits // 8) / (ms_total / args.steps * 1e-3) / 1e9,
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps,
             "gpu_launches": plan.launches() * args.steps, "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
@@ -309,6 +337,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sps", action="store_true")
     args = ap.parse_args(argv)
     w = W.CONFIGS[args.workload]
     if w.nbeams > 1:
