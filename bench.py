@@ -39,7 +39,7 @@ WORKLOAD_KEY = 3  # BASELINE.json configs[2]
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum per dd_tiled_kernel launch (mean of the 3 ranges) from the
 # committed `ncu --set full` capture (profiles/); None until one exists for the current kernel.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.56e9  # profiles/r1_dd_tiled_kernel_ncu_full.md: (4.447 GB range 0 + 2.669 GB range 2) / 2
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.55e9  # profiles/r1_dd_tiled_kernel_ncu_full.md: (4.440 GB range 0 + 2.657 GB range 2) / 2
 
 
 def _measured_peaks():

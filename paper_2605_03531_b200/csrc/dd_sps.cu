@@ -39,6 +39,15 @@ struct SpsParams {
 __device__ __forceinline__ unsigned long long shfl_down_u64(unsigned long long v, int o) {
   return __shfl_down_sync(0xffffffffu, v, o);
 }
+// four consecutive prefix sums starting at a multiple of four: one or two vector loads from shared memory
+__device__ __forceinline__ void load4(const uint32_t* P, uint32_t (&v)[4]) {
+  const uint4 q = *reinterpret_cast<const uint4*>(P);
+  v[0] = q.x, v[1] = q.y, v[2] = q.z, v[3] = q.w;
+}
+__device__ __forceinline__ void load4(const unsigned long long* P, unsigned long long (&v)[4]) {
+  const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(P), b = *reinterpret_cast<const ulonglong2*>(P + 2);
+  v[0] = a.x, v[1] = a.y, v[2] = b.x, v[3] = b.y;
+}
 
 // K = number of widths; WIDE = boxcar sums may reach 2^32 (64-bit prefix sums), else 32-bit modular prefix sums
 // (a difference of two of them is the exact boxcar because it is below 2^32).
@@ -111,8 +120,7 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
   int tb[K], cnt[K];
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    // sums are >= 0, so the thread's first window (t = tid) is its first maximum until a larger sum shows up
-    best[k] = 0, tb[k] = tid + (1 << k) <= n ? tid : 0x7fffffff, cnt[k] = 0;
+    best[k] = 0, tb[k] = 0x7fffffff, cnt[k] = 0;
     // thresholds above the reach of acc_t can never be met: 2^32-1 is below 2^32 only for sums that small
     thr[k] = WIDE ? (acc_t)s_thr[k] : (s_thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_thr[k]);
   }
@@ -150,17 +158,49 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
     }
     __syncthreads();
     const bool interior = tile0 + span <= n;  // every window of every width of this tile lies inside the row
-    for (int tl = tid; tl < kSpsTile; tl += kSpsThreads) {
-      const int t = tile0 + tl;
-      if (t >= n) break;
-      const acc_t p0 = P[tl];
+    if (interior) {
+      // four consecutive samples per thread and step: the prefix sums come in vectors, the maximum of the four
+      // boxcars is compared with the running best once, and only a new best looks for its position
+      for (int q = tid; q < kSpsTile / 4; q += kSpsThreads) {
+        const int tl = 4 * q, t = tile0 + tl;
+        acc_t a[4], a4[4];
+        load4(P + tl, a);
+        load4(P + tl + 4, a4);
 #pragma unroll
-      for (int k = 0; k < K; ++k) {
-        const int w = 1 << k;
-        if (interior || t + w <= n) {
-          const acc_t b = P[tl + w] - p0;
-          if (b > best[k]) best[k] = b, tb[k] = t;   // t increases: first maximum kept
-          cnt[k] += (b >= thr[k]) && !never[k];
+        for (int k = 0; k < K; ++k) {
+          acc_t b[4];
+          if (k == 0) {
+            b[0] = a[1] - a[0], b[1] = a[2] - a[1], b[2] = a[3] - a[2], b[3] = a4[0] - a[3];
+          } else if (k == 1) {
+            b[0] = a[2] - a[0], b[1] = a[3] - a[1], b[2] = a4[0] - a[2], b[3] = a4[1] - a[3];
+          } else if (k == 2) {
+            b[0] = a4[0] - a[0], b[1] = a4[1] - a[1], b[2] = a4[2] - a[2], b[3] = a4[3] - a[3];
+          } else {
+            acc_t c[4];
+            load4(P + tl + (1 << k), c);
+            b[0] = c[0] - a[0], b[1] = c[1] - a[1], b[2] = c[2] - a[2], b[3] = c[3] - a[3];
+          }
+          if (!never[k]) cnt[k] += (b[0] >= thr[k]) + (b[1] >= thr[k]) + (b[2] >= thr[k]) + (b[3] >= thr[k]);
+          const acc_t m01 = b[0] > b[1] ? b[0] : b[1], m23 = b[2] > b[3] ? b[2] : b[3], m = m01 > m23 ? m01 : m23;
+          if (m > best[k] || tb[k] == 0x7fffffff) {  // rare once the row's level is reached; t increases, so the first maximum is kept
+            best[k] = m;
+            tb[k] = t + (b[0] == m ? 0 : b[1] == m ? 1 : b[2] == m ? 2 : 3);
+          }
+        }
+      }
+    } else {
+      for (int tl = tid; tl < kSpsTile; tl += kSpsThreads) {
+        const int t = tile0 + tl;
+        if (t >= n) break;
+        const acc_t p0 = P[tl];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          const int w = 1 << k;
+          if (t + w <= n) {
+            const acc_t b = P[tl + w] - p0;
+            if (b > best[k] || tb[k] == 0x7fffffff) best[k] = b, tb[k] = t;
+            cnt[k] += (b >= thr[k]) && !never[k];
+          }
         }
       }
     }

@@ -78,3 +78,21 @@ def test_sps_rejects_inexact_sums_and_bad_arguments():
         with pytest.raises(B.DDError) as e:
             plan8.sps_execute(buf, K, thr, buf, buf, buf)
         assert e.value.code == B.DD_ERR_INVALID
+
+
+def test_sps_all_zero_rows_and_long_rows():
+    """An all-zero filterbank (every boxcar 0: the first window is the tied best) and rows spanning many tiles
+    with a late, narrow peak."""
+    nch = 4
+    w = W.Workload("spszero", 500.0, -200.0 / nch, nch, 1.024e-3, 40000, 1, 8, (W.DMRange(0.0, 1.0, 3, 1),), 1, 0, 0)
+    x = np.zeros((1, nch, 40000), dtype=np.uint8)
+    plan, got, ref = _sps_both(w, x, 10, 2.0)
+    for k in ("tmax", "count"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert (got["tmax"] == 0).all() and (got["snr"] == 0).all()
+    x[0, :, 39000:39003] = 200
+    x[0, 0, 100] = 1
+    plan, got, ref = _sps_both(w, x, 10, 2.0)
+    for k in ("tmax", "count"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
