@@ -9,7 +9,9 @@ tile shape chosen by the plan).  The oracle cannot produce 1e9 outputs in test t
     evaluated in exact integer arithmetic from the oracle's decimated input and delay table and compared
     with the float64 sum of the GPU row (exact for the uint8 configs: every term < 2^24, totals < 2^53;
     1e-7 relative for the uint16 config whose outputs are rounded once);
-  * DM = 0 (trial 0 of range 0) equals the plain channel sum.
+  * DM = 0 (trial 0 of range 0) equals the plain channel sum (PAPER.md:431);
+  * (uint8 configs) the single-pulse search over the whole plane agrees bit for bit with the oracle's search on
+    the oracle's sampled rows.
 """
 import numpy as np
 import pytest
@@ -40,6 +42,14 @@ def _run_full(key, beams_to_check):
     torch.cuda.synchronize()
     del xin
     exact = w.in_bits == 8
+    sps_k, sps_thr, sps = 8, 6.0, None
+    if exact:   # NEXT-2: single-pulse search over the whole plane, checked on the sampled trials below
+        nrows = plan.sps_rows()
+        sps = [torch.empty((nrows, sps_k), dtype=dt, device="cuda") for dt in (torch.float32, torch.int32, torch.int32)]
+        plan.sps_execute(out, sps_k, sps_thr, *sps, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        sps = [a.cpu().numpy() for a in sps]
+    rows_per_beam = sum(rg.ndm for rg in w.ranges)
     for beam in beams_to_check:
         for r, rg in enumerate(w.ranges):
             tab = oracle.delay_table(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, rg.decim, rg.dm_lo, rg.dm_step, rg.ndm)
@@ -53,6 +63,11 @@ def _run_full(key, beams_to_check):
             want = oracle.dedisperse(y, tab, sel=sel, t0=0, nt=nout)
             got = view[torch.from_numpy(sel.astype(np.int64)).cuda()].cpu().numpy()
             assert np.array_equal(got.view(np.uint32), want.view(np.uint32)), (key, beam, r)
+            if sps is not None:   # the oracle's search on the oracle's rows vs the GPU's search on the GPU's plane
+                ref = oracle.sps(want, nout, sps_k, sps_thr)
+                idx = beam * rows_per_beam + sum(q.ndm for q in w.ranges[:r]) + sel
+                assert np.array_equal(sps[0][idx].view(np.uint32), ref["snr"].view(np.uint32)), (key, beam, r)
+                assert np.array_equal(sps[1][idx], ref["tmax"]) and np.array_equal(sps[2][idx], ref["count"]), (key, beam, r)
             # (2) every trial: row sums from prefix sums (exact integers)
             Y = np.zeros((w.nchans, ns_r + 1), dtype=np.uint64)
             np.cumsum(y, axis=1, dtype=np.uint64, out=Y[:, 1:])
