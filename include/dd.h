@@ -32,7 +32,7 @@
 extern "C" {
 #endif
 
-#define DD_VERSION 101 /* major*100 + minor */
+#define DD_VERSION 200 /* major*100 + minor */
 
 typedef enum dd_status {
   DD_OK = 0,
@@ -43,7 +43,8 @@ typedef enum dd_status {
   DD_ERR_OVERFLOW = -3,  /* nchans * (2^in_bits - 1) * decim >= 2^32: exact integer sums impossible */
   DD_ERR_ALIGN = -4,     /* in_dev / out_dev / workspace not 16-byte aligned */
   DD_ERR_CUDA = -5,      /* a CUDA runtime call failed; text via dd_last_cuda_error() */
-  DD_ERR_NOMEM = -6      /* host or device allocation failed; workspace too small */
+  DD_ERR_NOMEM = -6,     /* host or device allocation failed; workspace too small */
+  DD_ERR_DEVICE = -7     /* the current CUDA device is not the one the plan / stream was created on */
 } dd_status;
 
 /* One DM range: trials DM_j = dm_lo + j*dm_step, j = 0..ndm-1, dedispersed on the input summed
@@ -102,6 +103,8 @@ int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out);
  * whose sums end in the last new_samps input samples: rows of nout_r = new_samps/decim_r + (0..15/decim_r) samples
  * ending at the same last sample as dd_plan_create's rows.  Each range skips the leading input it does not need
  * (in steps of 16 samples).  Used by the stream calls below; layouts and queries as for dd_plan_create.
+ * DD_ERR_TOO_SHORT if nsamps < new_samps + maxd_r*decim_r for some range (the window cannot supply the promised
+ * new_samps/decim_r outputs); DD_ERR_INVALID if new_samps < 1 or new_samps > nsamps.
  */
 int dd_plan_create_tail(const dd_config_t* cfg, int64_t new_samps, dd_plan_t** plan_out);
 
@@ -113,6 +116,27 @@ int dd_plan_create_tail(const dd_config_t* cfg, int64_t new_samps, dd_plan_t** p
 int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out);
 
 /*
+ * dd_plan_create_tuned: dd_plan_create (host_only = 0) or dd_plan_create_host (host_only != 0) with the automatic
+ * choices of the plan builder overridden -- for tests and measurements; the results never change, only the kernel
+ * shape.  tuning == NULL means automatic.  (The library reads no environment variables.)
+ *   mode        -1 automatic; 0 / 1 / 2 force the table form of the tiled kernel (see dd_plan_tile_info); the delta
+ *               form is refused (falls back to 0) for a range with a delay step above 1 between neighbouring trials
+ *   byte_lanes  -1 or 1 automatic; 0: never use 8-bit lanes (undecimated coarse ranges then run on 16-/32-bit lanes)
+ *   trial_groups, words_per_cta, chans_per_stage, stages
+ *               all 0: automatic; else the CTA shape: trial_groups * words_per_cta in {256, 512} threads,
+ *               words_per_cta a multiple of 32, chans_per_stage in {4, 8, .., 32}, 2 <= stages <= 8.  A shape that
+ *               fails the checks of the automatic path (shared-memory budget, offset widths) sends the range to the
+ *               direct kernel; the ring depth is lowered to what fits.
+ * DD_ERR_INVALID for out-of-range mode / byte_lanes.
+ */
+typedef struct dd_tuning {
+  int32_t mode;
+  int32_t byte_lanes;
+  int32_t trial_groups, words_per_cta, chans_per_stage, stages;
+} dd_tuning_t;
+int dd_plan_create_tuned(const dd_config_t* cfg, const dd_tuning_t* tuning, int32_t host_only, dd_plan_t** plan_out);
+
+/*
  * dd_execute: enqueue the whole hot path on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  * legacy default stream): pack/decimate kernels for every range, then the dedispersion kernels, which
  * write fp32 results straight into out_dev.  No host synchronisation, no allocation.
@@ -122,7 +146,7 @@ int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out);
  *            out_dev[b*beam_stride + offset_r + j*pitch_r + t'],  t' < nout_r; the pitch_r - nout_r pad
  *            floats of each row are left untouched.
  * One execute per plan may be in flight at a time (the workspace is shared).  The caller owns both
- * buffers and the stream.
+ * buffers and the stream.  DD_ERR_DEVICE if the current device is not the plan's.
  */
 int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* cuda_stream);
 
@@ -132,7 +156,9 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
  * piece of the DM-time plane back to out_host on a plan-owned copy stream while the next piece is computed
  * (pinned host memory is needed for that overlap), then waits for everything before returning.  Layouts as in dd_execute, except that whole rows are
  * copied back, so the pad floats of out_host are overwritten with unspecified values.  The staging buffers are
- * allocated on first use (DD_ERR_NOMEM if that fails) and freed by dd_plan_destroy.
+ * allocated on first use (DD_ERR_NOMEM if that fails) and freed by dd_plan_destroy.  Refusals (missing workspace or
+ * tables, wrong device) come before anything is enqueued; if a CUDA call fails later, both streams are drained before
+ * the error is returned, so no copy touches the caller's buffers after the call.
  */
 int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream);
 

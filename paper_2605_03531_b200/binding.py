@@ -13,7 +13,7 @@ from typing import List, Optional, Sequence, Tuple
 from .build import LIB, build
 
 DD_OK = 0
-DD_ERR_INVALID, DD_ERR_TOO_SHORT, DD_ERR_OVERFLOW, DD_ERR_ALIGN, DD_ERR_CUDA, DD_ERR_NOMEM = -1, -2, -3, -4, -5, -6
+DD_ERR_INVALID, DD_ERR_TOO_SHORT, DD_ERR_OVERFLOW, DD_ERR_ALIGN, DD_ERR_CUDA, DD_ERR_NOMEM, DD_ERR_DEVICE = -1, -2, -3, -4, -5, -6, -7
 DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED, DD_KERNEL_SHARED = 0, 1, 2, 3
 DD_LAYOUT_CHANNEL_MAJOR, DD_LAYOUT_SPECTRUM_MAJOR = 0, 1
 
@@ -22,7 +22,7 @@ SYMBOLS = [
     "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
-    "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_tile_shape", "dd_plan_table",
+    "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_create_tuned", "dd_plan_tile_shape", "dd_plan_table",
     "dd_sps_rows", "dd_sps_execute", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
 ]
@@ -41,6 +41,11 @@ class dd_config_t(ctypes.Structure):
     ]
 
 
+class dd_tuning_t(ctypes.Structure):
+    _fields_ = [("mode", ctypes.c_int32), ("byte_lanes", ctypes.c_int32), ("trial_groups", ctypes.c_int32),
+                ("words_per_cta", ctypes.c_int32), ("chans_per_stage", ctypes.c_int32), ("stages", ctypes.c_int32)]
+
+
 class DDError(RuntimeError):
     def __init__(self, code: int, what: str):
         self.code = code
@@ -57,8 +62,7 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB):
-            build()
+        build()  # returns at once when libdd.so is newer than every source; rebuilds after any edit of csrc/ or dd.h
         lib = ctypes.CDLL(LIB)  # raises OSError if the CUDA extension is missing: no fallback
         vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
         P = ctypes.POINTER
@@ -78,6 +82,7 @@ def _load():
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
         lib.dd_plan_create_host.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_plan_create_tail.argtypes = [P(dd_config_t), ctypes.c_int64, P(vp)]
+        lib.dd_plan_create_tuned.argtypes = [P(dd_config_t), P(dd_tuning_t), i32, P(vp)]
         lib.dd_sps_rows.argtypes = [vp, P(ctypes.c_int64)]
         lib.dd_sps_execute.argtypes = [vp, vp, i32, ctypes.c_double, vp, vp, vp, vp]
         lib.dd_stream_create.argtypes = [P(dd_config_t), P(vp)]
@@ -129,7 +134,9 @@ class Plan:
 
     def __init__(self, f_top_mhz: float, chan_width_mhz: float, nchans: int, tsamp_s: float, nsamps: int,
                  ranges: Sequence[Tuple[float, float, int, int]], nbeams: int = 1, in_bits: int = 8,
-                 in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, host_only: bool = False):
+                 in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, host_only: bool = False, tuning: Optional[dict] = None):
+        """tuning: None (automatic) or a dict with any of the dd_tuning_t fields (mode, byte_lanes, trial_groups,
+        words_per_cta, chans_per_stage, stages) -> dd_plan_create_tuned."""
         lib = _load()
         arr = (dd_range_t * max(1, len(ranges)))()
         for i, (lo, step, ndm, decim) in enumerate(ranges):
@@ -137,7 +144,12 @@ class Plan:
         cfg = dd_config_t(float(f_top_mhz), float(chan_width_mhz), int(nchans), float(tsamp_s), int(nsamps),
                           int(nbeams), int(in_bits), len(ranges), arr, int(in_layout))
         h = ctypes.c_void_p()
-        if host_only:
+        if tuning is not None:
+            t = dd_tuning_t(int(tuning.get("mode", -1)), int(tuning.get("byte_lanes", -1)), int(tuning.get("trial_groups", 0)),
+                            int(tuning.get("words_per_cta", 0)), int(tuning.get("chans_per_stage", 0)), int(tuning.get("stages", 0)))
+            _chk(lib.dd_plan_create_tuned(ctypes.byref(cfg), ctypes.byref(t), 1 if host_only else 0, ctypes.byref(h)),
+                 "dd_plan_create_tuned")
+        elif host_only:
             _chk(lib.dd_plan_create_host(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create_host")
         else:
             _chk(lib.dd_plan_create(ctypes.byref(cfg), ctypes.byref(h)), "dd_plan_create")
@@ -148,14 +160,15 @@ class Plan:
 
     @classmethod
     def from_workload(cls, w, in_layout: int = DD_LAYOUT_CHANNEL_MAJOR, ascending: bool = False,
-                      host_only: bool = False) -> "Plan":
+                      host_only: bool = False, tuning: Optional[dict] = None) -> "Plan":
         """ascending=True describes the same band listed from its lowest channel upwards (the data must then be
         given in that order)."""
         f0, cw = w.f_top_mhz, w.chan_width_mhz
         if ascending:
             f0, cw = f0 + (w.nchans - 1) * cw, -cw
         return cls(f0, cw, w.nchans, w.tsamp_s, w.nsamps,
-                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits, in_layout, host_only)
+                   [(r.dm_lo, r.dm_step, r.ndm, r.decim) for r in w.ranges], w.nbeams, w.in_bits, in_layout, host_only,
+                   tuning)
 
     # -- dd_plan_destroy
     def destroy(self) -> None:

@@ -126,6 +126,9 @@ struct dd_plan {
 
 namespace dd {
 
+// records "<what>: <cuda error string>" for dd_last_cuda_error() (thread-local) and returns DD_ERR_CUDA (dd_plan.cu)
+int cuda_fail(cudaError_t e, const char* what);
+
 // launchers (dd_kernels.cu); all enqueue on `stream` and return the CUDA error of the launch
 cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev, cudaStream_t stream);
 // all byte planes of the trial blocks blk0 .. blk0+nblk-1 (nblk <= 0: to the end of the range)

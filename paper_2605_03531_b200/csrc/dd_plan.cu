@@ -19,10 +19,16 @@ namespace {
 
 thread_local std::string g_last_cuda_error;
 
-int cuda_fail(cudaError_t e, const char* what) {
+}  // namespace
+
+// Records the text dd_last_cuda_error() returns (per thread) and yields DD_ERR_CUDA; shared by every source file.
+int dd::cuda_fail(cudaError_t e, const char* what) {
   g_last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
   return DD_ERR_CUDA;
 }
+
+namespace {
+using dd::cuda_fail;
 #define DD_CUDA(call)                                      \
   do {                                                     \
     cudaError_t e__ = (call);                              \
@@ -57,10 +63,8 @@ struct TileChoice {
   int G, T, Cc, stages;
 };
 
-int env_int(const char* name, int dflt) {
-  const char* s = getenv(name);
-  return (s && *s) ? atoi(s) : dflt;
-}
+// "auto" tuning: what dd_plan_create uses (dd_plan_create_tuned passes the caller's overrides instead)
+const dd_tuning_t kAutoTuning = {-1, -1, 0, 0, 0, 0};
 
 // Delay spread of one trial block: d(c, last) - d(c, first); delays are non-decreasing in j.
 inline int block_spread(const dd_plan& p, const dd::RangePlan& r, int blk, int Dcta, int c) {
@@ -69,9 +73,29 @@ inline int block_spread(const dd_plan& p, const dd::RangePlan& r, int blk, int D
   return r.delays[(size_t)j1 * p.nchans + c] - r.delays[(size_t)j0 * p.nchans + c];
 }
 
+// Superwords a staged row of (trial block, channel) holds beyond the time tile: rows start at the block's first
+// delay rounded DOWN to a 128-byte line (8 superwords) and end on a line (build_tables computes the same value).
+inline int block_span(const dd_plan& p, const dd::RangePlan& r, int blk, int Dcta, int c) {
+  const int j0 = blk * Dcta;
+  const int j1 = std::min(r.ndm - 1, j0 + Dcta - 1);
+  const int d0 = r.delays[(size_t)j0 * p.nchans + c] & ~7;
+  return (int)round_up(r.delays[(size_t)j1 * p.nchans + c] - d0, 8);
+}
+
+// Largest block_span over ALL (trial block, channel): the row pitch of the staged rows is T + this.  Delays are
+// rounded per channel, so the widest row is not always the lowest channel's (its spread can be one sample short of
+// a neighbour's, and the start alignment d0 & 7 differs per channel).
+int max_block_span(const dd_plan& p, const dd::RangePlan& r, int Dcta) {
+  const int nblocks = (r.ndm + Dcta - 1) / Dcta;
+  int smax = 0;
+  for (int b = 0; b < nblocks; ++b)
+    for (int c = 0; c < p.nchans; ++c) smax = std::max(smax, block_span(p, r, b, Dcta, c));
+  return smax;
+}
+
 // Which table form the tiled kernel uses for this range (dd_internal.h TiledMode).  Trial groups are the
 // kRD-aligned runs of trials counted from the start of the range.
-int choose_mode(const dd_plan& p, const dd::RangePlan& r) {
+int choose_mode(const dd_plan& p, const dd::RangePlan& r, const dd_tuning_t& tune) {
   bool delta = true;
   int64_t same = 0, total = 0;
   for (int j = 0; j + 1 < r.ndm; ++j) {
@@ -87,7 +111,7 @@ int choose_mode(const dd_plan& p, const dd::RangePlan& r) {
   }
   int mode = delta ? dd::kModeDelta : (total > 0 && (double)same / (double)total >= 0.25) ? dd::kModeGeneralReuse
                                                                                          : dd::kModeGeneral;
-  mode = env_int("DD_MODE", mode);  // tuning hook (measurements only); delta is refused when it does not apply
+  if (tune.mode >= 0) mode = tune.mode;  // dd_plan_create_tuned; delta is refused when it does not apply
   if (mode < 0 || mode > 2 || (mode == dd::kModeDelta && !delta)) mode = dd::kModeGeneral;
   return mode;
 }
@@ -95,7 +119,7 @@ int choose_mode(const dd_plan& p, const dd::RangePlan& r) {
 // Pick the tile shape of the tiled kernel for one range: more trials per CTA amortise the
 // L2 -> shared-memory fill of a channel row over more adds, but widen the staged window by the delay
 // spread of the block.  Cost model: staged bytes per add; constraint: >= 3 stages in 200 KB.
-void choose_tile(const dd_plan& p, dd::RangePlan& r) {
+void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
   // 16-bit lanes hold lo + 256*hi exactly when (a) 255 + flush*maxval <= 65535 between flushes and (b) the
   // hi lanes, which gain at most 255 per flush, stay below 65536: at most 256 flushes.
   const int maxval = ((1 << p.in_bits) - 1) * r.decim;
@@ -107,12 +131,12 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
     r.NL = 4;
     r.flush = 0;
   }
-  r.mode = choose_mode(p, r);
+  r.mode = choose_mode(p, r, tune);
   // Undecimated ranges that cannot use the delta table run on 8-bit lanes: half the shared-memory traffic per
-  // sample (the bound of the offsets-table modes), uint16 input as two byte planes.  DD_BYTES=0 switches it off
-  // (measurements only).
+  // sample (the bound of the offsets-table modes), uint16 input as two byte planes.  dd_tuning_t::byte_lanes = 0
+  // switches it off.
   const int flush16 = 65280 / 255;
-  if (r.decim == 1 && r.mode != dd::kModeDelta && (int64_t)p.nchans <= (int64_t)120 * flush16 && env_int("DD_BYTES", 1)) {
+  if (r.decim == 1 && r.mode != dd::kModeDelta && (int64_t)p.nchans <= (int64_t)120 * flush16 && tune.byte_lanes != 0) {
     r.NL = 16;
     r.flush = flush16;
     r.mode = dd::kModeGeneral;
@@ -121,53 +145,76 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   r.RD = dd::trials_per_thread(r.NL);
   static const int cand[][2] = {{16, 32}, {8, 64}, {4, 128}, {2, 256}, {1, 512}, {8, 32}, {4, 64}, {2, 128}, {1, 256}};
   const size_t budget = 200 * 1024;
-  double best = 1e300;
-  TileChoice bc = {1, 256, 4, 2};
-  bool found = false;
-  for (auto& gt : cand) {
-    const int G = gt[0], T = gt[1], D = G * r.RD;
+  // One candidate shape: does it fit (16-bit offsets, 64 KB of delta byte offsets, >= min_stages ring slots in
+  // `budget`), with how many stages, at what cost.  The automatic choice and a forced tile (dd_tuning_t) go
+  // through the same checks.
+  auto evaluate = [&](int G, int T, int Cc, int smax, double smean, int nblocks, int min_stages, int* stages_out,
+                      double* cost_out) -> bool {
+    const int D = G * r.RD;
+    if (T + smax > 65535) return false;  // 16-bit offsets
+    if (r.flush > 0 && Cc > r.flush) return false;
+    if (r.mode == dd::kModeDelta && (size_t)Cc * (size_t)(T + smax) * 16 > 65536) return false;  // 16-bit byte offsets
+    const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, r.NL, Cc, G);
+    const int stages = (int)std::min<size_t>(6, budget / stage);
+    if (stages < min_stages) return false;
+    // bytes staged per add: row (T + mean spread) superwords + the table row, over T*NL*D adds
+    double cost = ((T + smean) * 16.0 + dd::tiled_meta_bytes(r.mode, r.NL, 4, G) / 4.0) / ((double)T * r.NL * D);
+    // trials past the end of the last block are computed and dropped
+    cost *= (double)nblocks * D / (double)r.ndm;
+    if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
+    if (Cc < 16) cost *= 1.0 + 0.05 * (16 / Cc - 1);  // shorter stages synchronise more often
+    *stages_out = stages;
+    *cost_out = cost;
+    return true;
+  };
+  auto spreads = [&](int D, int* smax, double* smean) {
     const int nblocks = (r.ndm + D - 1) / D;
-    int smax = 0;
     double ssum = 0;
     const int cstep = std::max(1, p.nchans / 64);
     int nsamp = 0;
-    for (int b = 0; b < nblocks; ++b) {
-      smax = std::max(smax, block_spread(p, r, b, D, p.nchans - 1));
+    for (int b = 0; b < nblocks; ++b)
       for (int c = 0; c < p.nchans; c += cstep, ++nsamp) ssum += block_spread(p, r, b, D, c);
-    }
-    smax = dd::aligned_span(smax);
-    if (T + smax > 65535) continue;  // 16-bit offsets
-    const double smean = ssum / std::max(1, nsamp) + 7.0;  // rows start and end on 128-byte lines
-    for (int Cc : {32, 16, 8, 4}) {
-      if (r.flush > 0 && Cc > r.flush) continue;
-      if (r.mode == dd::kModeDelta && (size_t)Cc * (size_t)(T + smax) * 16 > 65536) continue;  // 16-bit byte offsets
-      const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, r.NL, Cc, G);
-      const int stages = (int)std::min<size_t>(6, budget / stage);
-      if (stages < (Cc >= 8 ? 3 : 2)) continue;
-      // bytes staged per add: row (T + mean spread) superwords + the table row, over T*NL*D adds
-      double cost = ((T + smean) * 16.0 + dd::tiled_meta_bytes(r.mode, r.NL, 4, G) / 4.0) / ((double)T * r.NL * D);
-      // trials past the end of the last block are computed and dropped
-      cost *= (double)nblocks * D / (double)r.ndm;
-      if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
-      if (Cc < 16) cost *= 1.0 + 0.05 * (16 / Cc - 1);  // shorter stages synchronise more often
-      if (cost < best) {
-        best = cost;
-        bc = {G, T, Cc, stages};
+    *smax = max_block_span(p, r, D);
+    *smean = ssum / std::max(1, nsamp) + 7.0;  // rows start and end on 128-byte lines
+    return nblocks;
+  };
+  double best = 1e300;
+  TileChoice bc = {1, 256, 4, 2};
+  bool found = false;
+  const bool forced = tune.trial_groups > 0 || tune.words_per_cta > 0 || tune.chans_per_stage > 0 || tune.stages > 0;
+  if (forced) {
+    // dd_plan_create_tuned: a caller-chosen shape, accepted only if it is a shape the kernels are built for and it
+    // passes the checks of the automatic path (the ring depth may be lowered to what fits)
+    const int G = tune.trial_groups, T = tune.words_per_cta, Cc = tune.chans_per_stage;
+    if (G >= 1 && T >= 32 && T % 32 == 0 && (G * T == 256 || G * T == 512) && Cc >= 4 && Cc <= 32 && Cc % 4 == 0 &&
+        tune.stages >= 2 && tune.stages <= 8) {
+      int smax, stages;
+      double smean, cost;
+      const int nblocks = spreads(G * r.RD, &smax, &smean);
+      if (evaluate(G, T, Cc, smax, smean, nblocks, 2, &stages, &cost)) {
+        bc = {G, T, Cc, std::min(stages, tune.stages)};
         found = true;
+      }
+    }
+  } else {
+    for (auto& gt : cand) {
+      const int G = gt[0], T = gt[1];
+      int smax;
+      double smean;
+      const int nblocks = spreads(G * r.RD, &smax, &smean);
+      for (int Cc : {32, 16, 8, 4}) {
+        int stages;
+        double cost;
+        if (!evaluate(G, T, Cc, smax, smean, nblocks, Cc >= 8 ? 3 : 2, &stages, &cost)) continue;
+        if (cost < best) {
+          best = cost;
+          bc = {G, T, Cc, stages};
+          found = true;
+        }
       }
     }
   }
   r.tiled_ok = found ? 1 : 0;  // otherwise the delay spread of one trial group exceeds shared memory: direct kernel
-  // tuning hook (measurements only): DD_TILE="G,T,Cc,stages"
-  if (const char* s = getenv("DD_TILE")) {
-    int g, t, cc, st;
-    if (sscanf(s, "%d,%d,%d,%d", &g, &t, &cc, &st) == 4 && (g * t == 256 || g * t == 512) && t % 32 == 0 &&
-        cc >= 4 && cc <= 32 && cc % 4 == 0 && st >= 2 && st <= 8 && (r.flush == 0 || cc <= r.flush) &&
-        (r.mode != dd::kModeDelta || (size_t)cc * (size_t)(t + 8 * g + 14) * 16 <= 65536)) {
-      bc = {g, t, cc, st};
-      r.tiled_ok = 1;
-    }
-  }
   r.G = bc.G;
   r.T = bc.T;
   r.Cc = bc.Cc;
@@ -176,9 +223,7 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r) {
   r.nblocks = (r.ndm + r.Dcta - 1) / r.Dcta;
   r.Cpad = (int)round_up(p.nchans, r.Cc);
   if (r.flush > 0) r.flush = r.flush / r.Cc * r.Cc;
-  r.Smax = 0;
-  for (int b = 0; b < r.nblocks; ++b) r.Smax = std::max(r.Smax, block_spread(p, r, b, r.Dcta, p.nchans - 1));
-  r.Smax = dd::aligned_span(r.Smax);
+  r.Smax = max_block_span(p, r, r.Dcta);  // the true maximum over every (trial block, channel)
   if (r.T + r.Smax > 65535) r.tiled_ok = 0;
   while (r.stages > 2 && dd::tiled_smem_bytes(r) > (size_t)227 * 1024) --r.stages;
   r.H = round_up((r.nout + r.NL - 1) / r.NL, 16);
@@ -215,6 +260,7 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
       const int32_t d0 = delay(j0, c) & ~7;  // delays are non-decreasing in j
       dmin[(size_t)b * r.Cpad + c] = d0;
       span[(size_t)b * r.Cpad + c] = (int32_t)round_up(delay(j0 + r.Dcta - 1, c) - d0, 8);
+      if (span[(size_t)b * r.Cpad + c] > r.Smax) r.tiled_ok = 0;  // cannot happen (Smax is this maximum); never overrun a row
       for (int g = 0; g < r.G; ++g) {
         const int jg = j0 + g * r.RD;
         if (delta) {
@@ -289,6 +335,7 @@ const char* dd_strerror(int code) {
     case DD_ERR_ALIGN: return "buffer not 16-byte aligned";
     case DD_ERR_CUDA: return "CUDA error (see dd_last_cuda_error)";
     case DD_ERR_NOMEM: return "out of memory or workspace too small";
+    case DD_ERR_DEVICE: return "current CUDA device is not the plan's device";
     default: return "unknown dd_status";
   }
 }
@@ -296,7 +343,8 @@ const char* dd_strerror(int code) {
 const char* dd_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 
 // Host half of a plan: validation, delay tables, tile shapes, the tables of the tiled kernel.  No CUDA call.
-static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new = 0) {
+static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new = 0,
+                            const dd_tuning_t* tune = nullptr) {
   if (!cfg || !plan_out) return DD_ERR_INVALID;
   *plan_out = nullptr;
   if (cfg->nchans < 1 || !(cfg->chan_width_mhz != 0.0) || !(cfg->tsamp_s > 0.0) || cfg->nsamps < 1 ||
@@ -346,11 +394,13 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_
       r.ns = (p->nsamps - r.in_off) / r.decim;
       r.nout = r.ns - r.maxd;
       if (r.nout < 1) { rc = DD_ERR_TOO_SHORT; break; }
+      // a tail plan promises the last tail_new/decim outputs of every range: the window must hold their delays
+      if (tail_new > 0 && r.nout < tail_new / r.decim) { rc = DD_ERR_TOO_SHORT; break; }
       r.pitch = round_up(r.nout, 32);
       r.offset = offset;
       offset += (int64_t)r.ndm * r.pitch;
       p->dm_samples += (int64_t)p->nbeams * r.ndm * r.nout;
-      choose_tile(*p, r);
+      choose_tile(*p, r, tune ? *tune : kAutoTuning);
       r.ws_offset = p->ws_bytes;
       p->ws_bytes += round_up(r.ws_bytes, 256);
     }
@@ -380,18 +430,26 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_
 
 int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out) { return plan_create_host(cfg, plan_out); }
 
-static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new);
+static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new,
+                              const dd_tuning_t* tune = nullptr);
 
 int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) { return plan_create_device(cfg, plan_out, 0); }
+
+int dd_plan_create_tuned(const dd_config_t* cfg, const dd_tuning_t* tuning, int32_t host_only, dd_plan_t** plan_out) {
+  if (tuning && (tuning->mode < -1 || tuning->mode > 2 || tuning->byte_lanes < -1 || tuning->byte_lanes > 1))
+    return DD_ERR_INVALID;
+  return host_only ? plan_create_host(cfg, plan_out, 0, tuning) : plan_create_device(cfg, plan_out, 0, tuning);
+}
 
 int dd_plan_create_tail(const dd_config_t* cfg, int64_t new_samps, dd_plan_t** plan_out) {
   if (new_samps < 1 || !cfg || new_samps > cfg->nsamps) return DD_ERR_INVALID;
   return plan_create_device(cfg, plan_out, new_samps);
 }
 
-static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new) {
+static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int64_t tail_new, const dd_tuning_t* tune) {
+  if (!plan_out) return DD_ERR_INVALID;
   dd_plan* p = nullptr;
-  int rc = plan_create_host(cfg, &p, tail_new);
+  int rc = plan_create_host(cfg, &p, tail_new, tune);
   if (rc != DD_OK) return rc;
   *plan_out = nullptr;
   cudaError_t e = cudaGetDevice(&p->device);
@@ -443,6 +501,11 @@ int dd_plan_destroy(dd_plan_t* p) {
 int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* cuda_stream) {
   if (!plan || !in_dev || !out_dev || plan->device < 0) return DD_ERR_INVALID;
   if (!aligned16(in_dev) || !aligned16(out_dev)) return DD_ERR_ALIGN;
+  {  // the tables and the workspace live on the device the plan was created on
+    int cur = -1;
+    DD_CUDA(cudaGetDevice(&cur));
+    if (cur != plan->device) return DD_ERR_DEVICE;
+  }
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
   // optional per-launch events (measurement hook)
@@ -485,18 +548,10 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
   return DD_OK;
 }
 
-int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
-  if (!plan || !in_host || !out_host || plan->device < 0) return DD_ERR_INVALID;
-  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+// Everything dd_execute_host enqueues.  Any failure is returned to the caller below, which drains both streams
+// before handing the error on (the caller's buffers must not be touched by copies still in flight).
+static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out_host, cudaStream_t stream) {
   const size_t in_bytes = (size_t)plan->nbeams * plan->nchans * plan->nsamps * (plan->in_bits / 8);
-  const size_t out_bytes = (size_t)plan->out_elems * sizeof(float);
-  if (!plan->h_in_dev) {
-    if (cudaMalloc(&plan->h_in_dev, in_bytes) != cudaSuccess) { plan->h_in_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
-  }
-  if (!plan->h_out_dev) {
-    if (cudaMalloc(&plan->h_out_dev, out_bytes) != cudaSuccess) { plan->h_out_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
-  }
-  if (!plan->copy_stream) DD_CUDA(cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
   const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
   // The DM-time plane is 3.6x the input: its copy back is the larger half of the transfer time.  Every range is
   // dedispersed in a few launches of consecutive trial blocks; as soon as one is done (event), its rows -- one
@@ -530,12 +585,10 @@ int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void*
   DD_CUDA(cudaMemcpyAsync(plan->h_in_dev, in_host, in_bytes, cudaMemcpyHostToDevice, stream));
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) continue;
-    if (!plan->ws) return DD_ERR_NOMEM;
     DD_CUDA(dd::launch_pack(plan, r, plan->h_in_dev, stream));
   }
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) {
-      if (!r.d_delays) return DD_ERR_INVALID;
       DD_CUDA(dd::launch_direct(plan, r, plan->h_in_dev, plan->h_out_dev, stream));
       DD_CUDA(copy_rows(r, 0, r.ndm));
       continue;
@@ -552,6 +605,41 @@ int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void*
   DD_CUDA(next_event(&done));
   DD_CUDA(cudaEventRecord(done, plan->copy_stream));
   DD_CUDA(cudaStreamWaitEvent(stream, done, 0));
+  return DD_OK;
+}
+
+int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
+  if (!plan || !in_host || !out_host || plan->device < 0) return DD_ERR_INVALID;
+  {
+    int cur = -1;
+    DD_CUDA(cudaGetDevice(&cur));
+    if (cur != plan->device) return DD_ERR_DEVICE;
+  }
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const size_t in_bytes = (size_t)plan->nbeams * plan->nchans * plan->nsamps * (plan->in_bits / 8);
+  const size_t out_bytes = (size_t)plan->out_elems * sizeof(float);
+  // everything that can be refused is checked before the first copy or launch is enqueued
+  const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
+  for (const auto& r : plan->ranges) {
+    if (all_direct || !r.tiled_ok) {
+      if (!r.d_delays) return DD_ERR_INVALID;  // uploaded by dd_plan_create / dd_plan_set_kernel
+    } else if (!plan->ws) {
+      return DD_ERR_NOMEM;
+    }
+  }
+  if (!plan->h_in_dev) {
+    if (cudaMalloc(&plan->h_in_dev, in_bytes) != cudaSuccess) { plan->h_in_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
+  }
+  if (!plan->h_out_dev) {
+    if (cudaMalloc(&plan->h_out_dev, out_bytes) != cudaSuccess) { plan->h_out_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
+  }
+  if (!plan->copy_stream) DD_CUDA(cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
+  const int rc = execute_host_enqueue(plan, in_host, out_host, stream);
+  if (rc != DD_OK) {  // drain what was enqueued: no copy may still read or write the caller's buffers after we return
+    cudaStreamSynchronize(stream);
+    cudaStreamSynchronize(plan->copy_stream);
+    return rc;
+  }
   DD_CUDA(cudaStreamSynchronize(stream));
   return DD_OK;
 }

@@ -248,12 +248,9 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
 
 template <int K, bool WIDE>
 static cudaError_t launch_sps(const SpsParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-  static bool attr_set = false;  // per instantiation
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(dd_sps_kernel<K, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per launch: the attribute is per device and the call is cheap (no static flag: not device- or thread-safe)
+  cudaError_t e = cudaFuncSetAttribute(dd_sps_kernel<K, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+  if (e != cudaSuccess) return e;
   dd_sps_kernel<K, WIDE><<<grid, kSpsThreads, smem, stream>>>(sp);
   return cudaGetLastError();
 }
@@ -313,7 +310,7 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
       DD_SPS(12)
     }
 #undef DD_SPS
-    if (e != cudaSuccess) return DD_ERR_CUDA;
+    if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_kernel launch");
     row0 += r.ndm;
   }
   return DD_OK;

@@ -17,7 +17,7 @@
 #include <new>
 #include <vector>
 
-#include "dd.h"
+#include "dd_internal.h"
 
 struct dd_stream {
   dd_plan_t* plan = nullptr;
@@ -26,6 +26,7 @@ struct dd_stream {
   void* win[2] = {nullptr, nullptr};  // [nbeams][nchans][hist+block] or [nbeams][hist+block][nchans], ping-pong
   int cur = 0;
   int64_t pushes = 0;
+  int device = -1;
 };
 
 namespace {
@@ -81,9 +82,11 @@ int dd_stream_create(const dd_config_t* cfg, dd_stream_t** stream_out) {
       return DD_ERR_NOMEM;
     }
   }
-  if (cudaDeviceSynchronize() != cudaSuccess) {
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaGetDevice(&s->device);
+  if (e != cudaSuccess) {
     dd_stream_destroy(s);
-    return DD_ERR_CUDA;
+    return dd::cuda_fail(e, "dd_stream_create");
   }
   *stream_out = s;
   return DD_OK;
@@ -91,6 +94,12 @@ int dd_stream_create(const dd_config_t* cfg, dd_stream_t** stream_out) {
 
 int dd_stream_push(dd_stream_t* s, const void* block_dev, float* out_dev, void* cuda_stream) {
   if (!s || !block_dev || !out_dev) return DD_ERR_INVALID;
+  {
+    int cur = -1;
+    cudaError_t ce = cudaGetDevice(&cur);
+    if (ce != cudaSuccess) return dd::cuda_fail(ce, "cudaGetDevice");
+    if (cur != s->device) return DD_ERR_DEVICE;
+  }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const int64_t W = s->hist + s->block;
   char* win = static_cast<char*>(s->win[s->cur]);
@@ -106,7 +115,7 @@ int dd_stream_push(dd_stream_t* s, const void* block_dev, float* out_dev, void* 
     e = cudaMemcpy2DAsync(win + (size_t)s->hist * s->bytes, (size_t)W * s->bytes, block_dev, (size_t)s->block * s->bytes,
                           (size_t)s->block * s->bytes, (size_t)s->nbeams * s->nchans, cudaMemcpyDeviceToDevice, st);
   }
-  if (e != cudaSuccess) return DD_ERR_CUDA;
+  if (e != cudaSuccess) return dd::cuda_fail(e, "cudaMemcpy2DAsync(block into window)");
   int rc = dd_execute(s->plan, win, out_dev, cuda_stream);
   if (rc != DD_OK) return rc;
   // carry: the last `hist` samples of this window become the head of the next one (other buffer: no overlap)
@@ -118,7 +127,7 @@ int dd_stream_push(dd_stream_t* s, const void* block_dev, float* out_dev, void* 
     e = cudaMemcpy2DAsync(nxt, (size_t)W * s->bytes, win + (size_t)s->block * s->bytes, (size_t)W * s->bytes,
                           (size_t)s->hist * s->bytes, (size_t)s->nbeams * s->nchans, cudaMemcpyDeviceToDevice, st);
   }
-  if (e != cudaSuccess) return DD_ERR_CUDA;
+  if (e != cudaSuccess) return dd::cuda_fail(e, "cudaMemcpy2DAsync(carry)");
   s->cur ^= 1;
   ++s->pushes;
   return DD_OK;

@@ -31,14 +31,14 @@ def oracle_full(w: W.Workload, x: np.ndarray):
 
 
 def gpu_run(w: W.Workload, x: np.ndarray, variant: int = 0, host_path: bool = False, in_layout: int = 0,
-            ascending: bool = False):
+            ascending: bool = False, tuning=None):
     """CUDA path through the C ABI.  Returns (plan, flat float32 numpy output).  `x` is always given as
     [beam][channel][time] with channel 0 the highest frequency (the oracle's order); for the other input
     conventions of the ABI it is re-laid out here (channel order reversed / spectra contiguous) before the call."""
     import torch
     from paper_2605_03531_b200 import binding as B
 
-    plan = B.Plan.from_workload(w, in_layout=in_layout, ascending=ascending)
+    plan = B.Plan.from_workload(w, in_layout=in_layout, ascending=ascending, tuning=tuning)
     if ascending:
         x = x[:, ::-1, :]
     if in_layout == B.DD_LAYOUT_SPECTRUM_MAJOR:

@@ -181,39 +181,37 @@ def test_host_path_and_caller_workspace():
 # ---- kernel v2: table modes, tile shapes, two-level packed accumulators ---------------------------------
 
 @pytest.mark.parametrize("mode", [0, 1, 2])
-def test_table_modes_agree_on_fine_dm_grid(mode, monkeypatch):
+def test_table_modes_agree_on_fine_dm_grid(mode):
     """A fine DM grid (every delay step 0 or 1) run through each table form of the tiled kernel:
     0 = one load per trial, 1 = load skipped on equal offsets, 2 = delta bits + uniform skip branch."""
-    monkeypatch.setenv("DD_MODE", str(mode))
-    monkeypatch.setenv("DD_BYTES", "0")   # keep the undecimated range on 16-bit lanes (else: 8-bit lanes, next test)
+    # byte_lanes 0: keep the undecimated range on 16-bit lanes (else: 8-bit lanes, next test)
     w = W.scaled(W.CONFIGS[3], nchans=260, nsamps=2 ** 14 + 5,
                  ranges=[W.DMRange(0.0, 0.1, 150, 1), W.DMRange(600.0, 0.5, 75, 4)])
     x = W.generate(w)
-    plan, flat = gpu_run(w, x, TILED)
+    plan, flat = gpu_run(w, x, TILED, tuning=dict(mode=mode, byte_lanes=0))
     assert plan.tile_info(0)["mode"] == mode
     check_full(w, x, plan, flat)
 
 
-def test_delta_mode_is_refused_for_coarse_dm_grid(monkeypatch):
+def test_delta_mode_is_refused_for_coarse_dm_grid():
     """Delay steps above 1 cannot be delta coded: the plan falls back to the offsets table."""
-    monkeypatch.setenv("DD_MODE", "2")
     w = W.scaled(W.CONFIGS[2], nchans=64, nsamps=2 ** 14, ranges=[W.DMRange(0.0, 2.0, 40, 1)])
     x = W.generate(w)
-    plan, flat = gpu_run(w, x, TILED)
+    plan, flat = gpu_run(w, x, TILED, tuning=dict(mode=2))
     assert plan.tile_info(0)["mode"] == 0
     check_full(w, x, plan, flat)
 
 
 @pytest.mark.parametrize("tile", ["16,32,32,3", "16,32,4,6", "8,64,16,4", "4,128,8,3", "2,256,8,2", "1,512,4,2",
                                   "8,32,16,4", "4,64,8,5", "1,256,8,2"])
-def test_tile_shapes(tile, monkeypatch):
+def test_tile_shapes(tile):
     """Every CTA shape (trial groups x superwords, channels per stage, ring depth) gives the same bits."""
-    monkeypatch.setenv("DD_TILE", tile)
+    g, t, cc, st = (int(v) for v in tile.split(","))
     w = W.scaled(W.CONFIGS[3], nchans=100, nsamps=2 ** 15 + 77,
                  ranges=[W.DMRange(0.0, 0.1, 77, 1), W.DMRange(50.0, 1.5, 19, 2)])   # delta + offsets tables
     x = W.generate(w)
-    plan, flat = gpu_run(w, x, TILED)
-    g, t = (int(v) for v in tile.split(",")[:2])
+    plan, flat = gpu_run(w, x, TILED, tuning=dict(trial_groups=g, words_per_cta=t, chans_per_stage=cc, stages=st))
+    assert plan.tile_shape(0)["tiled"] == 1 and plan.tile_shape(0)["chans_per_stage"] == cc
     assert plan.tile_info(0)["dm_per_cta"] == 8 * g and plan.tile_info(0)["words_per_cta"] == t
     check_full(w, x, plan, flat)
 
@@ -248,7 +246,7 @@ def test_many_flushes_and_wide_fallback():
 
 
 @pytest.mark.parametrize("bits", [8, 16])
-def test_byte_lanes_coarse_dm_grid(bits, monkeypatch):
+def test_byte_lanes_coarse_dm_grid(bits):
     """Undecimated range with delay steps of several samples: 8-bit lanes (uint16: low and high byte planes,
     S = S_lo + 256 S_hi, one rounding).  Saturated rows next to random ones reach the lane bounds; 600 channels
     cross two flushes."""
@@ -262,8 +260,7 @@ def test_byte_lanes_coarse_dm_grid(bits, monkeypatch):
     assert plan.tile_info(0)["lanes"] == 16 and plan.tile_info(0)["mode"] == 0
     assert plan.launches() == 1 + bits // 8
     check_full(w, x, plan, flat)
-    monkeypatch.setenv("DD_BYTES", "0")
-    plan2, flat2 = gpu_run(w, x, TILED)
+    plan2, flat2 = gpu_run(w, x, TILED, tuning=dict(byte_lanes=0))
     assert plan2.tile_info(0)["lanes"] == (8 if bits == 8 else 4)
     assert np.array_equal(flat.view(np.uint32)[flat != -1.0], flat2.view(np.uint32)[flat2 != -1.0])
 
@@ -376,3 +373,17 @@ def test_streaming_blocks_join_exactly(layout):
             assert ref.shape[1] == got.shape[1] - maxd
             assert np.array_equal(got[:, maxd:].view(np.uint32), ref.view(np.uint32)), (b, r)
     st.destroy()
+
+
+def test_row_pitch_regression_gpu():
+    """a staged row wider than the last channel's (per-channel rounding) overran the next row of
+    the shared-memory stage.  The reported plan, plus a few hundred-trial fine grids of the same band."""
+    nch, ns = 128, 4096
+    rng = np.random.default_rng(5)
+    x = rng.integers(0, 256, size=(1, nch, ns), dtype=np.uint8)
+    for lo, step, ndm in [(23.979060551005045, 0.01977691285836024, 16), (3.0, 0.0213, 333), (11.7, 0.0171, 400)]:
+        w = W.Workload("rowpitch", 1399.6529111929856, -2.664227517042692, nch, 327.68e-6, ns, 1, 8,
+                       (W.DMRange(lo, step, ndm, 1),), 1, 0, 0)
+        plan, flat = gpu_run(w, x, TILED)
+        assert plan.tile_shape(0)["tiled"] == 1
+        check_full(w, x, plan, flat)

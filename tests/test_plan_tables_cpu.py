@@ -127,3 +127,79 @@ def test_host_only_plans_cannot_execute_and_edge_shapes_build():
         else:                                       # undecimated, coarse steps: byte lanes (uint16: two planes)
             assert info["lanes"] == (16 if nch <= 30720 else 4)
         p.destroy()
+
+
+def _row_invariant(plan, r):
+    """Every staged row (time tile + span of the block's delays) fits the row pitch of the shared-memory stage."""
+    info, shape = plan.tile_info(r), plan.tile_shape(r)
+    if not shape["tiled"]:
+        return True
+    span = plan.table(r, 2).astype(np.int64)
+    return bool((span + info["words_per_cta"] <= shape["row_superwords"]).all())
+
+
+def test_row_pitch_covers_every_channels_span_regression():
+    """the row pitch was sized from the LAST channel's delay spread only; delays are rounded per
+    channel, so another channel's staged row could be 8 superwords longer and its bulk copy overran the next row.
+    The reported case: span 16 where the last channel gave 8."""
+    p = B.Plan(1399.6529111929856, -2.664227517042692, 128, 327.68e-6, 4096,
+               [(23.979060551005045, 0.01977691285836024, 16, 1)], host_only=True)
+    assert p.tile_shape(0)["tiled"] == 1 and _row_invariant(p, 0)
+    got, rd, shape = _decode(p, 0)
+    assert np.array_equal(got, _padded_delays(p, 0, shape, rd))
+    p.destroy()
+
+
+def test_row_pitch_property_random_plans():
+    """Host-only property test over random small plans and multi-block fine-grid (delta) plans."""
+    rng = np.random.default_rng(20261104)
+    checked = delta_plans = 0
+    for i in range(400):
+        nch = int(rng.integers(4, 200))
+        f_top = float(rng.uniform(300.0, 1500.0))
+        cw = -float(rng.uniform(0.2, 0.6)) * f_top / nch
+        tsamp = float(rng.choice([81.92e-6, 327.68e-6, 655.36e-6, 1.31072e-3]))
+        decim = int(rng.choice([1, 2, 4, 8]))
+        fine = i % 2 == 0
+        ndm = int(rng.integers(200, 1000)) if fine else int(rng.integers(1, 80))
+        # fine: steps of at most ~1 sample at the lowest channel (delta mode); coarse: a few samples per trial
+        f_lo = f_top + (nch - 1) * cw
+        sweep_per_dm = 4.148808e3 * (f_lo ** -2 - f_top ** -2) / (tsamp * decim)
+        step = float(rng.uniform(0.2, 0.999) if fine else rng.uniform(1.0, 6.0)) / sweep_per_dm
+        lo = float(rng.uniform(0.0, 50.0)) * step
+        maxd = int(sweep_per_dm * (lo + ndm * step)) + 2
+        try:
+            p = B.Plan(f_top, cw, nch, tsamp, (maxd + 600) * decim, [(lo, step, ndm, decim)], host_only=True)
+        except B.DDError:
+            continue
+        assert _row_invariant(p, 0), (i, f_top, cw, nch, tsamp, decim, lo, step, ndm)
+        delta_plans += p.tile_info(0)["mode"] == 2
+        checked += 1
+        p.destroy()
+    assert checked > 300 and delta_plans > 100
+
+
+def test_tuned_plan_goes_through_the_same_checks():
+    """dd_plan_create_tuned: forced modes / shapes are validated like the automatic choice (no environment variables)."""
+    w = W.scaled(W.CONFIGS[3], nchans=100, nsamps=2 ** 15, ranges=[W.DMRange(0.0, 0.1, 77, 1)])
+    p = B.Plan.from_workload(w, host_only=True, tuning=dict(trial_groups=8, words_per_cta=64, chans_per_stage=16, stages=4))
+    assert p.tile_info(0)["dm_per_cta"] == 64 and p.tile_shape(0)["tiled"] == 1 and _row_invariant(p, 0)
+    p.destroy()
+    # a shape the kernels are not built for is refused: the range falls back to the direct kernel, never a bad launch
+    p = B.Plan.from_workload(w, host_only=True, tuning=dict(trial_groups=3, words_per_cta=100, chans_per_stage=5, stages=2))
+    assert p.tile_shape(0)["tiled"] == 0
+    p.destroy()
+    # delta rows above 64 KB per stage cannot be addressed with 16-bit byte offsets: refused as well
+    p = B.Plan.from_workload(w, host_only=True, tuning=dict(mode=2, trial_groups=1, words_per_cta=512, chans_per_stage=32, stages=2))
+    assert p.tile_shape(0)["tiled"] == 0
+    p.destroy()
+    with pytest.raises(B.DDError):
+        B.Plan.from_workload(w, host_only=True, tuning=dict(mode=7))
+    import os
+    os.environ["DD_MODE"] = "0"      # the library reads no environment variables
+    try:
+        p = B.Plan.from_workload(w, host_only=True)
+        assert p.tile_info(0)["mode"] == 2
+        p.destroy()
+    finally:
+        del os.environ["DD_MODE"]
