@@ -16,8 +16,11 @@ _SRC = os.path.join(_HERE, "oracle_dedisp.c")
 _LIB = os.path.join(_HERE, "liboracle_dedisp.so")
 _SRC_SPS = os.path.join(_HERE, "oracle_sps.c")
 _LIB_SPS = os.path.join(_HERE, "liboracle_sps.so")
+_SRC_POST = os.path.join(_HERE, "oracle_post.c")
+_LIB_POST = os.path.join(_HERE, "liboracle_post.so")
 _lib = None
 _lib_sps = None
+_lib_post = None
 
 _ERRORS = {-1: "invalid argument", -2: "window exceeds the valid span (too short)", -3: "out of memory"}
 
@@ -38,6 +41,13 @@ def build(force: bool = False) -> str:
             check=True,
         )
         os.replace(tmp, _LIB_SPS)
+    if force or not os.path.exists(_LIB_POST) or os.path.getmtime(_LIB_POST) < os.path.getmtime(_SRC_POST):
+        tmp = _LIB_POST + ".tmp.%d" % os.getpid()
+        subprocess.run(  # no FMA contraction: the operation order of oracle_post.c is part of its definition
+            ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC_POST, "-lm"],
+            check=True,
+        )
+        os.replace(tmp, _LIB_POST)
     return _LIB
 
 
@@ -157,3 +167,68 @@ def sps(rows: np.ndarray, n: int, nwidths: int, threshold: float):
                              _ptr(mean), _ptr(sigma))
     _check(rc, "sps")
     return {"snr": snr, "tmax": tmax, "count": count, "mean": mean, "sigma": sigma}
+
+
+# ---- pulsar-side post-processing of dedispersed series (oracle_post.c) ----------------
+def _post():
+    global _lib_post
+    if _lib_post is None:
+        build()
+        lib = ctypes.CDLL(_LIB_POST)
+        vp, i64, i32, f64 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+        lib.oracle_downsample.argtypes = [vp, i64, i64, i64, i32, vp, i64]
+        lib.oracle_running_median.argtypes = [vp, i64, i64, i64, i32, vp, vp, i64]
+        lib.oracle_resample_edges.argtypes = [f64, f64, f64, f64, i64, vp, i64, vp, vp]
+        lib.oracle_resample.argtypes = [vp, i64, i64, i64, f64, f64, f64, f64, vp, i64]
+        for fn in (lib.oracle_downsample, lib.oracle_running_median, lib.oracle_resample_edges, lib.oracle_resample):
+            fn.restype = ctypes.c_int
+        _lib_post = lib
+    return _lib_post
+
+
+def _rows(x: np.ndarray) -> np.ndarray:
+    if x.ndim != 2 or x.dtype != np.float32:
+        raise ValueError("oracle post: rows must be a 2-D float32 array")
+    return np.ascontiguousarray(x)
+
+
+def downsample(rows: np.ndarray, factor: int) -> np.ndarray:
+    """C1 (PAPER.md:421): y[k] = sum_{i<F} x[k*F+i], k < n//F; float32 [nrows][n//F]."""
+    rows = _rows(rows)
+    nrows, n = rows.shape
+    out = np.empty((nrows, n // factor), dtype=np.float32)
+    _check(_post().oracle_downsample(_ptr(rows), nrows, n, n, factor, _ptr(out), max(1, n // factor)), "downsample")
+    return out
+
+
+def running_median(rows: np.ndarray, window: int):
+    """C2: (median, x - median) with the centred odd window held at the first / last full window
+    near the ends; both float32 [nrows][n]."""
+    rows = _rows(rows)
+    nrows, n = rows.shape
+    med = np.empty((nrows, n), dtype=np.float32)
+    out = np.empty((nrows, n), dtype=np.float32)
+    _check(_post().oracle_running_median(_ptr(rows), nrows, n, n, window, _ptr(med), _ptr(out), n), "running_median")
+    return med, out
+
+
+def resample_edges(f0: float, f1: float, f2: float, tsamp: float, n: int):
+    """C3-C4 (Eq. 3.3): (edges float64 [M+1] in input-sample units, reversed flag)."""
+    m = ctypes.c_int64()
+    rev = ctypes.c_int32()
+    _check(_post().oracle_resample_edges(f0, f1, f2, tsamp, n, None, 0, ctypes.byref(m), ctypes.byref(rev)), "resample_edges")
+    u = np.empty(m.value + 1, dtype=np.float64)
+    _check(_post().oracle_resample_edges(f0, f1, f2, tsamp, n, _ptr(u), m.value + 1, ctypes.byref(m), ctypes.byref(rev)),
+           "resample_edges")
+    return u, bool(rev.value)
+
+
+def resample(rows: np.ndarray, f0: float, f1: float, f2: float, tsamp: float) -> np.ndarray:
+    """C5-C7 (Eqs 3.1-3.6): fractional-overlap re-sampling of every row; float32 [nrows][M]."""
+    rows = _rows(rows)
+    nrows, n = rows.shape
+    u, _ = resample_edges(f0, f1, f2, tsamp, n)
+    m = len(u) - 1
+    out = np.empty((nrows, max(1, m)), dtype=np.float32)
+    _check(_post().oracle_resample(_ptr(rows), nrows, n, n, f0, f1, f2, tsamp, _ptr(out), max(1, m)), "resample")
+    return out[:, :m]
