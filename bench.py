@@ -37,9 +37,21 @@ METRIC = "dedispersed DM-trial x samples per second"
 UNIT = "DM-trial*samples/s"
 WORKLOAD_KEY = 3  # BASELINE.json configs[2]
 FP32_LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum per dd_tiled_kernel launch (mean of the 3 ranges) from the
-# committed `ncu --set full` capture (profiles/); None until one exists for the current kernel.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.55e9  # profiles/r1_dd_tiled_kernel_ncu_full.md: (4.440 GB range 0 + 2.657 GB range 2) / 2
+# dram__bytes_read.sum + dram__bytes_write.sum of every dd_tiled_kernel launch of one step, from the committed ncu
+# capture (one launch per ncu run, so no counter is lost to multi-pass replay); see the .md beside it for the command
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_dd_tiled_kernel_traffic.csv")
+
+
+def ncu_traffic_per_launch(workload_name: str):
+    """Mean DRAM bytes (read + write) per dd_tiled_kernel launch of `workload_name` from TRAFFIC_CSV, or None."""
+    try:
+        import csv
+        with open(TRAFFIC_CSV) as fh:
+            rows = [r for r in csv.DictReader(l for l in fh if not l.startswith("#")) if r["workload"] == workload_name]
+        vals = [float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows]
+        return sum(vals) / len(vals) if vals else None
+    except Exception:
+        return None
 
 
 def _measured_peaks():
@@ -172,7 +184,89 @@ def aggregate(total_units: float, elapsed_ms_local: float, dist=None, device=Non
     return float(total_units), float(elapsed_ms_local)
 
 
+def run_stub(args, w):
+    """--stub-body (tests only): the N-rank plumbing of run_ours -- rendezvous, one seeded beam per rank, barrier,
+    max-over-ranks time, summed units, rank 0 prints -- over gloo on CPU with the timed GPU body replaced by a
+    sleep.  Lets `bench.py --gpus 2` be run as a command where there is no GPU.  Never a bench value."""
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    small = W.scaled(w, nchans=32, nsamps=2048, ranges=[W.DMRange(0.0, 1.0, 4, 1)])
+    x = W.generate_beam(small, beam=rank)                      # every rank its own seeded beam
+    units_local = 1000.0 * args.steps
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    time.sleep(0.01 * (rank + 1) * args.steps)                 # stands in for the timed dd_execute loop
+    ms_local = (time.perf_counter() - t0) * 1e3
+    if world > 1:
+        dist.barrier()
+    units, ms_total = aggregate(units_local, ms_local, dist if world > 1 else None, None)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": units / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+                          "stub": True, "units": units, "beam_checksum_rank0": int(x.sum()),
+                          "config": {"workload": w.name, "parallelism": "replicas: one beam per GPU, no collective"}}),
+              flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def self_launch(args, argv):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: start the N ranks ourselves (one process per GPU),
+    exactly as the driver would: torch.distributed.run --nnodes=1 --nproc-per-node N on 127.0.0.1."""
+    import socket
+    import subprocess
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd, env=dict(os.environ, MASTER_ADDR="127.0.0.1"))
+
+
+def time_config(B, torch, key, steps, warmup, dev, sms, f_max):
+    """One line of `other_configs`: ms per dd_execute, DM-samples/s and fraction of the FP32-add roofline of BASELINE
+    config `key`, same event timing as the headline.  Kernel timing does not depend on the sample values, so the
+    input is seeded random bytes drawn on the device (the parity tests use the real generators)."""
+    w = W.CONFIGS[key]
+    plan = B.Plan.from_workload(w)
+    dm_samples, adds = plan.work()
+    g = torch.Generator(device=dev)
+    g.manual_seed(w.seed)
+    x = torch.randint(0, 256, (w.in_bytes,), dtype=torch.uint8, device=dev, generator=g)
+    out = torch.empty(plan.out_elems(), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        plan.execute(x, out, stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        plan.execute(x, out, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    tiles = [plan.tile_info(r) for r in range(plan.nranges)]
+    res = {"workload": w.name, "ms_per_execute": ms, "dm_samples_per_s": dm_samples / (ms * 1e-3), "adds": adds,
+           "frac_of_fp32_add_roofline": adds / (ms * 1e-3) / (sms * FP32_LANES_PER_SM * f_max),
+           "input_gb_per_s": w.in_bytes / (ms * 1e-3) / 1e9, "dtype": "u%d" % w.in_bits, "nbeams": w.nbeams,
+           "lanes_mode_per_range": [[t["lanes"], t["mode"]] for t in tiles], "steps": steps,
+           "input": "seeded random bytes drawn on the device (timing only)"}
+    plan.destroy()
+    del x, out
+    torch.cuda.empty_cache()
+    return res
+
+
 def run_ours(args, w):
+    if args.stub_body:
+        return run_stub(args, w)
     import torch
     import torch.distributed as dist
 
@@ -238,7 +332,8 @@ def run_ours(args, w):
     achieved = adds * args.steps / (tiled_ms * 1e-3)
     roofline = {
         "bound": "alu", "achieved": achieved / 1e12, "peak": peak_adds / 1e12, "unit": "Tadd/s",
-        "frac": achieved / peak_adds, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+        "frac": achieved / peak_adds, "traffic": ncu_traffic_per_launch(w.name),
+        "traffic_source": "profiles/r2_dd_tiled_kernel_traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean over the launches of one step)",
         "kernel": "dd_tiled_kernel", "launches_timed": n_tiled,
         "adds_per_launch": adds / max(1, n_tiled // max(1, args.steps)),
         "avg_launch_ms": tiled_ms / max(1, n_tiled),
@@ -258,7 +353,7 @@ def run_ours(args, w):
         hout = torch.empty(plan.out_elems(), dtype=torch.float32).pin_memory()
         plan.set_profiling(0)
         plan.execute_host(hin, hout, stream)  # allocates the staging buffers, warms up
-        n_e2e = max(1, min(args.steps, args.e2e_steps))
+        n_e2e = max(1, min(args.steps, args.e2e_steps or args.steps))
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
@@ -301,6 +396,20 @@ def run_ours(args, w):
                "candidates_above_threshold": int(cnt.sum().item())}
         del snr, tmx, cnt
 
+    # the other BASELINE configs (1, 2, 4, 5), reported beside the headline: `value` stays on config 3
+    other = None
+    if rank == 0 and world == 1 and not args.no_other_configs:
+        del x, out
+        torch.cuda.empty_cache()
+        other = []
+        for key in (1, 2, 4, 5):
+            if key == args.workload:
+                continue
+            try:
+                other.append(time_config(B, torch, key, 5 if key != 5 else 3, 3, dev, sms, f_max))
+            except Exception as e:  # e.g. a smaller GPU: say so instead of dropping the line
+                other.append({"workload": W.CONFIGS[key].name, "skipped": repr(e)})
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, done, threads, desc = oracle_sample_run(w, x_host, args.ref_trials)
@@ -317,7 +426,7 @@ def run_ours(args, w):
                        "l2": "inputs larger than L2 (1.07 GB input, 4.0 GB packed copy, 3.8 GB output per step)",
                        "parallelism": "replicas: one beam per GPU, no collective"},
             "input_gb_per_s": world * w.nchans * w.nsamps * (w.in_bits // 8) / (ms_total / args.steps * 1e-3) / 1e9,
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps, "other_configs": other,
             "gpu_launches": plan.launches() * args.steps, "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
@@ -334,11 +443,17 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=WORKLOAD_KEY, help="BASELINE config number (1-5); default 3")
     ap.add_argument("--ref-trials", type=int, default=48, help="oracle sample: trials per range")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=0, help="end-to-end steps (0 = as many as --steps)")
+    ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--stub-body", action="store_true", help=argparse.SUPPRESS)  # tests: N-rank plumbing on CPU / gloo
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sps", action="store_true")
     args = ap.parse_args(argv)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        return self_launch(args, sys.argv[1:] if argv is None else argv)
+    if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%s" % (args.gpus, os.environ.get("WORLD_SIZE")))
     w = W.CONFIGS[args.workload]
     if w.nbeams > 1:
         w = W.scaled(w, nbeams=1, name=w.name + "_1beam_per_gpu")

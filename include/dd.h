@@ -269,6 +269,51 @@ int dd_sps_rows(const dd_plan_t* plan, int64_t* rows);
 int dd_sps_execute(const dd_plan_t* plan, const float* plane_dev, int32_t nwidths, double threshold, float* snr_dev,
                    int32_t* tmax_dev, int32_t* count_dev, void* cuda_stream);
 
+/* ---- pulsar-side post-processing of dedispersed series ------------------------------ */
+
+/*
+ * The thesis's pulsar pipeline continues from the dedispersed series with downsampling, running-
+ * median de-reddening and re-sampling that removes the frequency derivatives f1, f2
+ * (Eqs 3.1-3.6).  These calls apply one such step to `nrows` independent series stored as rows
+ * of floats: row r at in_dev + r*in_pitch, the first n floats valid -- e.g. the rows of one range of the DM-time
+ * plane (in_dev = out_dev of dd_execute + offset_r, nrows = ndm_r, in_pitch = pitch_r, n = nout_r).  Device
+ * pointers, 4-byte aligned; out rows at out_dev + r*out_pitch; all work is enqueued on `cuda_stream`, nothing
+ * synchronises.  Readings where the thesis is silent: DESIGN.md C1-C7.
+ *
+ * dd_post_downsample  (C1)  out[k] = sum_{i<factor} in[k*factor + i], k < n/factor (a SUM, as the input decimation;
+ *     tail dropped), accumulated in double in index order and rounded once.  out_pitch >= n/factor.
+ *
+ * dd_post_dered       (C2)  window odd, 1 <= window <= min(n, DD_POST_MAX_WINDOW), h = (window-1)/2:
+ *         median[t] = the (h+1)-th smallest of in[s .. s+window),  s = min(max(t-h, 0), n-window)
+ *     (centred on t; held at the first / last full window near the ends -- no padding), out[t] = in[t] - median[t].
+ *     Exact order statistics of the floats (finite values; any sign).  median_dev or out_dev may be NULL (not
+ *     wanted), not both; both have pitch out_pitch >= n.
+ *
+ * dd_resample_*       (C3-C7)  Eq 3.3 laid end to end: bin edges in input samples u_0 = 0, u_{k+1} = u_k + w_k,
+ *         t = u_k*tsamp,  w_k = (1 + (f'*t)/F0) + (f''*(t*t))/(2*F0)          (IEEE double, this order)
+ *     with (F0, f', f'') = (f0, -f1, -f2) if f1 <= 0, else the series is reversed and (Eqs 3.5, 3.6)
+ *     F0 = (f0 + f1*T) + (f2*(T*T))/2, f' = f1 + f2*T, f'' = -f2, T = n*tsamp; M = number of complete bins
+ *     (u_{k+1} <= n); w_k < 1/2 is refused (DD_ERR_INVALID).
+ *         out[k] = fl32( sum_i in[i] * |[u_k,u_{k+1}) n [i,i+1)| )   left to right in double, no fused multiply-add;
+ *     the reversed case reads the row backwards and writes it backwards.
+ *     dd_resample_create builds and uploads the edges for series of n samples (current device);
+ *     dd_resample_create_host builds them only (queries, no execute); dd_resample_info: M and the reversed flag;
+ *     dd_resample_get_edges copies the M+1 edges (test hook); dd_resample_execute: out_pitch >= M.
+ */
+#define DD_POST_MAX_WINDOW 8191
+int dd_post_downsample(const float* in_dev, int64_t nrows, int64_t in_pitch, int64_t n, int32_t factor, float* out_dev,
+                       int64_t out_pitch, void* cuda_stream);
+int dd_post_dered(const float* in_dev, int64_t nrows, int64_t in_pitch, int64_t n, int32_t window, float* median_dev,
+                  float* out_dev, int64_t out_pitch, void* cuda_stream);
+typedef struct dd_resample dd_resample_t; /* opaque */
+int dd_resample_create(double f0_hz, double f1_hz_s, double f2_hz_s2, double tsamp_s, int64_t n, dd_resample_t** out);
+int dd_resample_create_host(double f0_hz, double f1_hz_s, double f2_hz_s2, double tsamp_s, int64_t n, dd_resample_t** out);
+int dd_resample_info(const dd_resample_t* r, int64_t* out_len, int32_t* reversed);
+int dd_resample_get_edges(const dd_resample_t* r, double* host_buf);
+int dd_resample_execute(const dd_resample_t* r, const float* in_dev, int64_t nrows, int64_t in_pitch, float* out_dev,
+                        int64_t out_pitch, void* cuda_stream);
+int dd_resample_destroy(dd_resample_t* r);
+
 /* ---- errors ---------------------------------------------------------------------------------- */
 const char* dd_strerror(int code);       /* static string for a dd_status */
 const char* dd_last_cuda_error(void);    /* text of the last CUDA failure seen by this thread ("" if none) */

@@ -25,7 +25,10 @@ SYMBOLS = [
     "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_create_tuned", "dd_plan_tile_shape", "dd_plan_table",
     "dd_sps_rows", "dd_sps_execute", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
+    "dd_post_downsample", "dd_post_dered", "dd_resample_create", "dd_resample_create_host", "dd_resample_info",
+    "dd_resample_get_edges", "dd_resample_execute", "dd_resample_destroy",
 ]
+DD_POST_MAX_WINDOW = 8191
 
 
 class dd_range_t(ctypes.Structure):
@@ -95,6 +98,15 @@ def _load():
         lib.dd_plan_table.argtypes = [vp, i32, i32, vp, ctypes.c_int64, P(ctypes.c_int64)]
         lib.dd_plan_set_profiling.argtypes = [vp, i32]
         lib.dd_plan_kernel_times.argtypes = [vp, i32, i32, P(ctypes.c_float), P(i32), P(i32), P(i32)]
+        f64 = ctypes.c_double
+        lib.dd_post_downsample.argtypes = [vp, i64, i64, i64, i32, vp, i64, vp]
+        lib.dd_post_dered.argtypes = [vp, i64, i64, i64, i32, vp, vp, i64, vp]
+        lib.dd_resample_create.argtypes = [f64, f64, f64, f64, i64, P(vp)]
+        lib.dd_resample_create_host.argtypes = [f64, f64, f64, f64, i64, P(vp)]
+        lib.dd_resample_info.argtypes = [vp, P(i64), P(i32)]
+        lib.dd_resample_get_edges.argtypes = [vp, vp]
+        lib.dd_resample_execute.argtypes = [vp, vp, i64, i64, vp, i64, vp]
+        lib.dd_resample_destroy.argtypes = [vp]
         lib.dd_strerror.argtypes = [ctypes.c_int]
         lib.dd_strerror.restype = ctypes.c_char_p
         lib.dd_last_cuda_error.restype = ctypes.c_char_p
@@ -342,6 +354,56 @@ class Stream:
         if getattr(self, "_h", None):
             self.plan._h = None
             _load().dd_stream_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# ---- pulsar-side post-processing of dedispersed series (dd_post_* / dd_resample_* of include/dd.h) -------------------
+def _p(a):
+    return None if a is None else (a if isinstance(a, int) else a.data_ptr())
+
+
+def post_downsample(in_dev, nrows: int, in_pitch: int, n: int, factor: int, out_dev, out_pitch: int, stream=None) -> None:
+    _chk(_load().dd_post_downsample(_p(in_dev), nrows, in_pitch, n, factor, _p(out_dev), out_pitch, _stream_ptr(stream)),
+         "dd_post_downsample")
+
+
+def post_dered(in_dev, nrows: int, in_pitch: int, n: int, window: int, median_dev, out_dev, out_pitch: int, stream=None) -> None:
+    _chk(_load().dd_post_dered(_p(in_dev), nrows, in_pitch, n, window, _p(median_dev), _p(out_dev), out_pitch,
+                               _stream_ptr(stream)), "dd_post_dered")
+
+
+class Resample:
+    """Owns a dd_resample_t*: re-sampling of series of n samples for one (f0, f1, f2) (Eqs 3.1-3.6)."""
+
+    def __init__(self, f0: float, f1: float, f2: float, tsamp_s: float, n: int, host_only: bool = False):
+        lib = _load()
+        h = ctypes.c_void_p()
+        fn = lib.dd_resample_create_host if host_only else lib.dd_resample_create
+        _chk(fn(float(f0), float(f1), float(f2), float(tsamp_s), int(n), ctypes.byref(h)), "dd_resample_create")
+        self._h = h
+        m, rev = ctypes.c_int64(), ctypes.c_int32()
+        _chk(lib.dd_resample_info(h, ctypes.byref(m), ctypes.byref(rev)), "dd_resample_info")
+        self.n, self.out_len, self.reversed = int(n), m.value, bool(rev.value)
+
+    def edges(self):
+        import numpy as np
+        u = np.empty(self.out_len + 1, dtype=np.float64)
+        _chk(_load().dd_resample_get_edges(self._h, u.ctypes.data), "dd_resample_get_edges")
+        return u
+
+    def execute(self, in_dev, nrows: int, in_pitch: int, out_dev, out_pitch: int, stream=None) -> None:
+        _chk(_load().dd_resample_execute(self._h, _p(in_dev), nrows, in_pitch, _p(out_dev), out_pitch, _stream_ptr(stream)),
+             "dd_resample_execute")
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None):
+            _load().dd_resample_destroy(self._h)
             self._h = None
 
     def __del__(self):

@@ -8,10 +8,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libdd.so")
-SOURCES = ["dd_plan.cu", "dd_kernels.cu", "dd_tiled.cu", "dd_stream.cu", "dd_sps.cu"]
+SOURCES = ["dd_plan.cu", "dd_kernels.cu", "dd_tiled.cu", "dd_stream.cu", "dd_sps.cu", "dd_post.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off", "-shared", "-Xptxas", "-v",
 ]
 
 

@@ -121,3 +121,27 @@ def test_reference_arm_prints_contract_line():
     line = json.loads(res.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "DM-trial*samples/s"
+
+
+def test_bench_gpus_2_as_a_command_launches_two_ranks():
+    """`python bench.py --gpus 2` outside torchrun starts two ranks itself (torch.distributed.run on 127.0.0.1).
+    The timed GPU body is replaced by a stub (--stub-body, gloo, CPU) -- everything else is the real N > 1 path:
+    rendezvous, one seeded beam per rank, barrier, max-over-ranks time, summed units, one JSON line from rank 0."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "2", "--warmup", "1",
+                          "--stub-body"], capture_output=True, text=True, env=env, timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, res.stdout                      # rank 0 alone prints
+    line = lines[0]
+    assert line["n_gpus"] == 2 and line["stub"] is True
+    assert line["units"] == 2 * 1000.0 * 2                  # summed over both ranks
+    assert line["ms_per_step"] >= 20.0 * 0.9                # the slower rank (rank 1 sleeps 20 ms per step) sets the time
+    # the same command under torchrun (the driver's form) gives the same line shape
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29741", os.path.join(ROOT, "bench.py"),
+                          "--gpus", "2", "--steps", "1", "--warmup", "1", "--stub-body"],
+                         capture_output=True, text=True, env=dict(env, MASTER_ADDR="127.0.0.1"), timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
+    assert sum(1 for l in res.stdout.splitlines() if l.startswith("{")) == 1
