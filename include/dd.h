@@ -89,6 +89,14 @@ typedef struct dd_plan dd_plan_t; /* opaque */
                               coincide over a channel quad (delta-coded ranges; other ranges as DD_KERNEL_TILED):
                               an exact shortcut that executes fewer adds than the brute-force count of
                               PAPER.md:421.  Same bits. */
+#define DD_KERNEL_SUBBAND 4 /* exact two-channel sub-bands (the thesis uses redundancy the same way
+                              for the FFA).  In a delta-coded range neighbouring channels 2v, 2v+1 differ in
+                              delay by delta_v or delta_v + 1 for every trial, so S[j][t] = sum_v U_{p(v,j)}[v][t + d(2v,j)]
+                              with the two pre-summed rows U_p[v][i] = y_2v[i] + y_2v+1[i + delta_v + p] (one extra streaming
+                              kernel per range and execute).  Half the adds of the brute-force count, same bits.  Ranges
+                              where some pair needs a third row run as DD_KERNEL_SHARED.  Needs twice the workspace:
+                              dd_plan_set_kernel re-allocates a plan-owned workspace; a caller-owned one must be set again
+                              (dd_plan_workspace_bytes reports the new size). */
 
 /*
  * dd_plan_create: host work (delay tables, per-range sizes, tile shapes) plus device allocations and
@@ -184,6 +192,13 @@ int dd_plan_get_delays(const dd_plan_t* plan, int32_t r, int32_t* host_buf);
 int dd_plan_work(const dd_plan_t* plan, int64_t* dm_samples, int64_t* adds);
 /* Kernel launches one dd_execute enqueues (pack + dedispersion) with the current kernel variant. */
 int dd_plan_launches(const dd_plan_t* plan, int32_t* n_launches);
+/* Sample additions one dd_execute actually performs with the current kernel variant, all beams (pre-sums of
+ * DD_KERNEL_SUBBAND included).  Equals the brute-force count of dd_plan_work for DD_KERNEL_AUTO / TILED / DIRECT. */
+int dd_plan_executed_adds(const dd_plan_t* plan, int64_t* adds);
+/* DD_KERNEL_SUBBAND, range r (any pointer may be NULL): whether the range runs on two-channel sub-bands, pairs per
+ * pipeline stage, superwords per staged pair row (two per time index), number of pair rows incl. padding. */
+int dd_plan_pair_info(const dd_plan_t* plan, int32_t r, int32_t* enabled, int32_t* pairs_per_stage,
+                      int32_t* row_superwords, int32_t* npairs);
 
 /* ---- workspace and variants ------------------------------------------------------------------ */
 
@@ -209,8 +224,10 @@ int dd_plan_tile_shape(const dd_plan_t* plan, int32_t r, int32_t* trial_groups, 
                        int32_t* stages, int32_t* row_superwords, int32_t* cpad, int32_t* nblocks, int32_t* tiled);
 /* Test hook: the tables of the tiled kernel for range r as they are uploaded.  which = 0: the per-trial table
  * (uint32 words; layout per mode in DESIGN.md "Data layout"), 1: start of the staged row per (trial block,
- * channel) (int32 superwords, multiple of 8), 2: its length beyond the time tile (int32).  *bytes = size; the
- * table is copied when host_buf != NULL (DD_ERR_NOMEM if cap_bytes is too small). */
+ * channel) (int32 superwords, multiple of 8), 2: its length beyond the time tile (int32).  After
+ * dd_plan_set_kernel(DD_KERNEL_SUBBAND): 3, 4, 5 = the same three tables of the pair mode (per pair row, delays of
+ * channel 2v), 6 = delta_v per pair (int32).  *bytes = size; the table is copied when host_buf != NULL
+ * (DD_ERR_NOMEM if cap_bytes is too small). */
 int dd_plan_table(const dd_plan_t* plan, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes);
 
 /* ---- per-kernel timing (measurement hook) ------------------------------------------------------- */

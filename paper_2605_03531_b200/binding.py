@@ -14,13 +14,14 @@ from .build import LIB, build
 
 DD_OK = 0
 DD_ERR_INVALID, DD_ERR_TOO_SHORT, DD_ERR_OVERFLOW, DD_ERR_ALIGN, DD_ERR_CUDA, DD_ERR_NOMEM, DD_ERR_DEVICE = -1, -2, -3, -4, -5, -6, -7
-DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED, DD_KERNEL_SHARED = 0, 1, 2, 3
+DD_KERNEL_AUTO, DD_KERNEL_DIRECT, DD_KERNEL_TILED, DD_KERNEL_SHARED, DD_KERNEL_SUBBAND = 0, 1, 2, 3, 4
 DD_LAYOUT_CHANNEL_MAJOR, DD_LAYOUT_SPECTRUM_MAJOR = 0, 1
 
 # every symbol include/dd.h declares
 SYMBOLS = [
     "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
+    "dd_plan_executed_adds", "dd_plan_pair_info",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
     "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_create_tuned", "dd_plan_tile_shape", "dd_plan_table",
     "dd_sps_rows", "dd_sps_execute", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
@@ -79,6 +80,8 @@ def _load():
         lib.dd_plan_get_delays.argtypes = [vp, i32, vp]
         lib.dd_plan_work.argtypes = [vp, P(i64), P(i64)]
         lib.dd_plan_launches.argtypes = [vp, P(i32)]
+        lib.dd_plan_executed_adds.argtypes = [vp, P(i64)]
+        lib.dd_plan_pair_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32)]
         lib.dd_plan_workspace_bytes.argtypes = [vp, P(i64)]
         lib.dd_plan_set_workspace.argtypes = [vp, vp, i64]
         lib.dd_plan_set_kernel.argtypes = [vp, i32]
@@ -248,6 +251,16 @@ class Plan:
         _chk(_load().dd_plan_launches(self._h, ctypes.byref(v)), "dd_plan_launches")
         return v.value
 
+    def executed_adds(self) -> int:
+        v = ctypes.c_int64()
+        _chk(_load().dd_plan_executed_adds(self._h, ctypes.byref(v)), "dd_plan_executed_adds")
+        return v.value
+
+    def pair_info(self, r: int) -> dict:
+        vals = [ctypes.c_int32() for _ in range(4)]
+        _chk(_load().dd_plan_pair_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_pair_info")
+        return {k: v.value for k, v in zip(["enabled", "pairs_per_stage", "row_superwords", "npairs"], vals)}
+
     def workspace_bytes(self) -> int:
         v = ctypes.c_int64()
         _chk(_load().dd_plan_workspace_bytes(self._h, ctypes.byref(v)), "dd_plan_workspace_bytes")
@@ -275,11 +288,12 @@ class Plan:
         return {k: v.value for k, v in zip(keys, vals)}
 
     def table(self, r: int, which: int):
-        """Tables of the tiled kernel (test hook): which = 0 per-trial table (uint32), 1 row starts, 2 row spans."""
+        """Tables of the tiled kernel (test hook): which = 0 per-trial table (uint32), 1 row starts, 2 row spans;
+        3, 4, 5 the same of the pair mode, 6 delta_v per pair (after set_kernel(DD_KERNEL_SUBBAND))."""
         import numpy as np
         n = ctypes.c_int64()
         _chk(_load().dd_plan_table(self._h, r, which, None, 0, ctypes.byref(n)), "dd_plan_table")
-        buf = np.empty(n.value // 4, dtype=np.uint32 if which == 0 else np.int32)
+        buf = np.empty(n.value // 4, dtype=np.uint32 if which in (0, 3) else np.int32)
         _chk(_load().dd_plan_table(self._h, r, which, buf.ctypes.data, n.value, ctypes.byref(n)), "dd_plan_table")
         return buf
 
@@ -299,13 +313,13 @@ class Plan:
         _chk(_load().dd_plan_set_profiling(self._h, int(max_executes)), "dd_plan_set_profiling")
 
     def kernel_times(self, slot: int) -> List[dict]:
-        cap = 2 * self.nranges
+        cap = 3 * self.nranges
         ms = (ctypes.c_float * cap)()
         kind = (ctypes.c_int32 * cap)()
         rng = (ctypes.c_int32 * cap)()
         n = ctypes.c_int32()
         _chk(_load().dd_plan_kernel_times(self._h, slot, cap, ms, kind, rng, ctypes.byref(n)), "dd_plan_kernel_times")
-        names = {0: "pack", 1: "tiled", 2: "direct"}
+        names = {0: "pack", 1: "tiled", 2: "direct", 3: "pairs"}
         return [{"ms": float(ms[i]), "kind": names[kind[i]], "range": int(rng[i])} for i in range(n.value)]
 
     # -- convenience for callers holding torch tensors

@@ -34,8 +34,16 @@ __host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? 
 //   kModeDeltaShare    kModeDelta plus sharing of partial sums (variant DD_KERNEL_SHARED): while
 //                      no channel of a quad changes its delay, the quad's sum wa+wb+wc+wd is the same for
 //                      consecutive trials and is added as ONE term.  Same table, same bits, fewer executed adds.
-enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3 };
-__host__ __device__ constexpr bool is_delta(int mode) { return mode == kModeDelta || mode == kModeDeltaShare; }
+//   kModeDeltaPair     exact two-channel sub-bands (variant DD_KERNEL_SUBBAND): neighbouring channels
+//                      2v, 2v+1 differ in delay by delta_v or delta_v + 1 for EVERY trial of the range, so the two
+//                      pre-summed rows U_p[i] = y_2v[i] + y_2v+1[i + delta_v + p], p = 0, 1 (built once per execute,
+//                      interleaved: superword 2i + p) replace both channels: one load and one add per trial and PAIR.
+//                      Table as kModeDelta per quad of pairs, with two bits per trial step and pair: "delay of
+//                      channel 2v changed" (address += 32) and "p flipped" (address ^= 16).
+enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3, kModeDeltaPair = 4 };
+__host__ __device__ constexpr bool is_delta(int mode) {
+  return mode == kModeDelta || mode == kModeDeltaShare || mode == kModeDeltaPair;
+}
 
 // kModeDelta processes channels in quads A,B,C,D.  The changed bits of a quad share one 32-bit word laid
 // out so that each byte feeds one R2P (register -> 7 predicates): bit n%7 of byte n/7, n = (j-1)*4 + q
@@ -90,6 +98,18 @@ struct RangePlan {
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
   int32_t* d_delays = nullptr;  // [ndm][nchans], only for the direct kernel (lazy)
+  // two-channel sub-bands (kModeDeltaPair), built by dd_plan_set_kernel(DD_KERNEL_SUBBAND): rows are pairs
+  int pair_ok = 0;        // 1: this range runs in pair mode under DD_KERNEL_SUBBAND
+  int Cc2 = 0;            // pairs per pipeline stage (= Cc / 2)
+  int Smax2 = 0;          // largest staged span of a pair row (time superwords; the row holds 2 per time index)
+  int stages2 = 0;
+  int64_t ws2_offset = 0, ws2_bytes = 0;  // pair array [nbeams][Cpad/2][2*Wp] superwords in the workspace
+  std::vector<uint32_t> h_meta2;          // [nblocks][Cpad/8][G] {Pd bits | any 1..4, Pf bits | any 5..7, offA|offB<<16, offC|offD<<16}
+  std::vector<int32_t> h_dmin2, h_span2;  // [nblocks][Cpad/2] of channel 2v (time superwords)
+  std::vector<int32_t> h_delta;           // [Cpad/2] delta_v
+  uint4* d_meta2 = nullptr;
+  int32_t *d_dmin2 = nullptr, *d_span2 = nullptr, *d_delta = nullptr;
+  int64_t adds_pair = 0;  // adds executed per beam in pair mode (pre-sums included)
 };
 
 }  // namespace dd
@@ -108,8 +128,10 @@ struct dd_plan {
   int device = 0;
   int variant = DD_KERNEL_AUTO;
   // workspace
-  int64_t ws_bytes = 0;
+  int64_t ws_bytes = 0;      // packed copies of every range
+  int64_t ws_pair_bytes = 0; // + the pair arrays of DD_KERNEL_SUBBAND (0 until that variant is selected)
   void* ws = nullptr;
+  int64_t ws_have = 0;       // bytes behind ws
   bool ws_owned = false;
   // per-kernel timing hook (dd_plan_set_profiling): events[slot][2*launch + {0,1}]
   int prof_slots = 0;
@@ -136,6 +158,9 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
                          int nblk = 0);
 cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_dev, float* out_dev,
                           cudaStream_t stream);
+// kModeDeltaPair: pre-sum the packed rows of a range into its pair array (reads P, writes P2)
+cudaError_t launch_pairs(const dd_plan* p, const RangePlan& r, cudaStream_t stream);
+inline bool use_pairs(const dd_plan* p, const RangePlan& r) { return p->variant == DD_KERNEL_SUBBAND && r.pair_ok; }
 cudaError_t configure_kernels(const dd_plan* p);  // opt in to the dynamic shared memory sizes
 size_t tiled_smem_bytes(const RangePlan& r);
 

@@ -308,6 +308,49 @@ cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev
 }
 
 // ------------------------------------------------------------------------------------------------
+// DD_KERNEL_SUBBAND: pair rows.  P2[beam][v][2i + p] = P[beam][2v][i] + P[beam][2v+1][i + delta_v + p], lane by lane
+// (16-bit lanes: 2 * maxval < 65536, no carry between lanes).  A delay is a shift by whole superwords, so both
+// terms are aligned 16-byte loads.  Thread = 4 consecutive time indices of one pair row: 4 + 5 loads, 8 stores.
+// Elements past the end of the packed row (never needed by a valid output) read as zero.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 add4(const uint4& a, const uint4& b) {
+  return make_uint4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w);
+}
+__global__ void __launch_bounds__(256) dd_pair_kernel(const uint4* __restrict__ P, uint4* __restrict__ P2,
+                                                      const int32_t* __restrict__ delta, int npairs, int64_t Wp) {
+  const int64_t i0 = 4 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+  if (i0 >= Wp) return;
+  const int v = blockIdx.y;
+  const int beam = blockIdx.z;
+  const uint4* ra = P + ((int64_t)beam * 2 * npairs + 2 * v) * Wp;
+  const uint4* rb = ra + Wp;
+  const int64_t d = delta[v];
+  const uint4 z = make_uint4(0, 0, 0, 0);
+  uint4 b[5];
+#pragma unroll
+  for (int e = 0; e < 5; ++e) {
+    const int64_t k = i0 + d + e;
+    b[e] = (k >= 0 && k < Wp) ? __ldg(rb + k) : z;
+  }
+  uint4* dst = P2 + ((int64_t)beam * npairs + v) * (2 * Wp) + 2 * i0;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) {
+    if (i0 + e >= Wp) break;  // Wp is a multiple of 8: never taken, kept for clarity
+    const uint4 a = __ldg(ra + i0 + e);
+    store2(dst + 2 * e, add4(a, b[e]), add4(a, b[e + 1]));
+  }
+}
+
+cudaError_t launch_pairs(const dd_plan* p, const RangePlan& r, cudaStream_t stream) {
+  const uint4* P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset);
+  uint4* P2 = reinterpret_cast<uint4*>(static_cast<char*>(p->ws) + r.ws2_offset);
+  const int npairs = r.Cpad / 2;
+  dim3 grid((unsigned)((r.Wp / 4 + 255) / 256), (unsigned)npairs, (unsigned)p->nbeams);
+  dd_pair_kernel<<<grid, 256, 0, stream>>>(P, P2, r.d_delta, npairs, r.Wp);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
 // the simple variant
 // ------------------------------------------------------------------------------------------------
 template <typename Tin>

@@ -7,6 +7,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <limits.h>
 
 #include <algorithm>
 #include <new>
@@ -297,6 +298,96 @@ int upload_tables(dd::RangePlan& r) {
   return DD_OK;
 }
 
+// ---- two-channel sub-bands (kModeDeltaPair, variant DD_KERNEL_SUBBAND) ---------------------------------------------
+// Delay of internal channel row c for the pair tables: rows past nchans are zero rows, so any delay is correct for
+// them; the pad partner of the last real channel copies it (delta = 0), all-pad pairs stay at 0.
+inline int32_t pair_delay(const dd_plan& p, const dd::RangePlan& r, int j, int c) {
+  j = std::min(r.ndm - 1, j);
+  if (c < p.nchans) return r.delays[(size_t)j * p.nchans + c];
+  if ((c & 1) && c - 1 < p.nchans) return r.delays[(size_t)j * p.nchans + c - 1];
+  return 0;
+}
+
+// Decide whether range r can run on pair rows and build its tables (host).  Conditions: delta-coded 16-bit-lane
+// range, an even number of channel rows per stage quad, every pair's delay difference takes at most two
+// neighbouring values over ALL trials of the range, and the doubled rows fit the 16-bit byte offsets and shared memory.
+void build_pair_tables(const dd_plan& p, dd::RangePlan& r) {
+  r.pair_ok = 0;
+  if (!r.tiled_ok || r.mode != dd::kModeDelta || r.NL != 8 || r.Cc % 8 != 0 || r.planes != 1) return;
+  const int nvc = r.Cpad / 2;
+  r.Cc2 = r.Cc / 2;
+  r.h_delta.assign(nvc, 0);
+  for (int v = 0; v < nvc; ++v) {
+    int32_t lo = INT32_MAX, hi = INT32_MIN;
+    for (int j = 0; j < r.ndm; ++j) {
+      const int32_t d = pair_delay(p, r, j, 2 * v + 1) - pair_delay(p, r, j, 2 * v);
+      lo = std::min(lo, d);
+      hi = std::max(hi, d);
+    }
+    if (hi - lo > 1) return;  // a third row would be needed: not this range
+    r.h_delta[v] = lo;
+  }
+  const size_t nbv = (size_t)r.nblocks * nvc;
+  r.h_dmin2.assign(nbv, 0);
+  r.h_span2.assign(nbv, 0);
+  r.Smax2 = 0;
+  for (int b = 0; b < r.nblocks; ++b)
+    for (int v = 0; v < nvc; ++v) {
+      const int j0 = b * r.Dcta;
+      const int32_t d0 = pair_delay(p, r, j0, 2 * v) & ~7;
+      const int32_t sp = (int32_t)round_up(pair_delay(p, r, j0 + r.Dcta - 1, 2 * v) - d0, 8);
+      r.h_dmin2[(size_t)b * nvc + v] = d0;
+      r.h_span2[(size_t)b * nvc + v] = sp;
+      r.Smax2 = std::max(r.Smax2, (int)sp);
+    }
+  const size_t rowbytes = (size_t)2 * (r.T + r.Smax2) * 16;
+  if ((size_t)r.Cc2 * rowbytes > 65536) return;  // 16-bit byte offsets inside a stage
+  const size_t stage = (r.Cc2 * rowbytes + dd::tiled_meta_bytes(dd::kModeDeltaPair, r.NL, r.Cc2, r.G) + 127) / 128 * 128;
+  r.stages2 = (int)std::min<size_t>(6, ((size_t)227 * 1024 - 128 - 512) / stage);
+  if (r.stages2 < 2) return;
+  // table: one 16-byte entry per quad of pairs and trial group
+  r.h_meta2.assign((size_t)r.nblocks * (nvc / 4) * r.G * 4, 0);
+  for (int b = 0; b < r.nblocks; ++b)
+    for (int v = 0; v < nvc; ++v) {
+      const int32_t d0 = r.h_dmin2[(size_t)b * nvc + v];
+      const int q = v % 4;
+      for (int g = 0; g < r.G; ++g) {
+        const int jg = b * r.Dcta + g * r.RD;
+        uint32_t* e = &r.h_meta2[(((size_t)b * (nvc / 4) + v / 4) * r.G + g) * 4];
+        auto D = [&](int j) { return pair_delay(p, r, j, 2 * v); };
+        auto P = [&](int j) { return pair_delay(p, r, j, 2 * v + 1) - D(j) - r.h_delta[v]; };
+        const uint32_t off = (uint32_t)(v % r.Cc2) * (uint32_t)rowbytes + (uint32_t)((D(jg) - d0) * 2 + P(jg)) * 16u;
+        e[2 + q / 2] |= off << (16 * (q % 2));
+        for (int j = 1; j < r.RD; ++j) {
+          const bool cd = D(jg + j) != D(jg + j - 1), cf = P(jg + j) != P(jg + j - 1);
+          if (cd) e[0] |= 1u << dd::delta_bit(j, q);
+          if (cf) e[1] |= 1u << dd::delta_bit(j, q);
+          if (cd || cf) {  // "some pair of the quad changes at step j": bit 7 of byte j-1 (steps 1..4: word 0, 5..7: word 1)
+            if (j <= 4) e[0] |= 0x80u << (8 * (j - 1));
+            else e[1] |= 0x80u << (8 * (j - 5));
+          }
+        }
+      }
+    }
+  r.ws2_bytes = round_up((int64_t)p.nbeams * nvc * 2 * r.Wp * dd::kSuperwordBytes, 256);
+  // executed adds per beam: one per (trial, sample, pair) + two pre-sums per packed pair-row element
+  r.adds_pair = (int64_t)r.ndm * r.nout * (p.nchans + 1) / 2 + (int64_t)2 * ((p.nchans + 1) / 2) * r.ns;
+  r.pair_ok = 1;
+}
+
+int upload_pair_tables(dd::RangePlan& r) {
+  if (r.d_meta2) return DD_OK;
+  DD_CUDA(cudaMalloc(&r.d_meta2, r.h_meta2.size() * sizeof(uint32_t)));
+  DD_CUDA(cudaMalloc(&r.d_dmin2, r.h_dmin2.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMalloc(&r.d_span2, r.h_span2.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMalloc(&r.d_delta, r.h_delta.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMemcpy(r.d_meta2, r.h_meta2.data(), r.h_meta2.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_dmin2, r.h_dmin2.data(), r.h_dmin2.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_span2, r.h_span2.data(), r.h_span2.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMemcpy(r.d_delta, r.h_delta.data(), r.h_delta.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  return DD_OK;
+}
+
 int ensure_direct_tables(dd_plan* p, bool only_untiled) {
   for (auto& r : p->ranges) {
     if (r.d_delays || (only_untiled && r.tiled_ok)) continue;
@@ -307,14 +398,20 @@ int ensure_direct_tables(dd_plan* p, bool only_untiled) {
 }
 
 int ensure_workspace(dd_plan* p) {
-  if (p->ws || p->ws_bytes == 0) return DD_OK;
-  cudaError_t e = cudaMalloc(&p->ws, (size_t)p->ws_bytes);
+  const int64_t need = p->ws_bytes + p->ws_pair_bytes;
+  if (need == 0 || (p->ws && p->ws_have >= need)) return DD_OK;
+  if (p->ws && !p->ws_owned) return DD_ERR_NOMEM;  // a caller-owned workspace that is too small: set a larger one
+  if (p->ws) cudaFree(p->ws);
+  p->ws = nullptr;
+  p->ws_have = 0;
+  cudaError_t e = cudaMalloc(&p->ws, (size_t)need);
   if (e != cudaSuccess) {
     cuda_fail(e, "cudaMalloc(workspace)");
     p->ws = nullptr;
     return DD_ERR_NOMEM;
   }
   p->ws_owned = true;
+  p->ws_have = need;
   return DD_OK;
 }
 
@@ -487,6 +584,10 @@ int dd_plan_destroy(dd_plan_t* p) {
     if (r.d_dmin) cudaFree(r.d_dmin);
     if (r.d_span) cudaFree(r.d_span);
     if (r.d_delays) cudaFree(r.d_delays);
+    if (r.d_meta2) cudaFree(r.d_meta2);
+    if (r.d_dmin2) cudaFree(r.d_dmin2);
+    if (r.d_span2) cudaFree(r.d_span2);
+    if (r.d_delta) cudaFree(r.d_delta);
   }
   for (cudaEvent_t e : p->prof_events) cudaEventDestroy(e);
   if (p->ws && p->ws_owned) cudaFree(p->ws);
@@ -509,7 +610,7 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
   // optional per-launch events (measurement hook)
-  const int max_launch = 2 * (int)plan->ranges.size();
+  const int max_launch = 3 * (int)plan->ranges.size();
   const int slot = plan->prof_slots > 0 ? (int)(plan->prof_calls++ % plan->prof_slots) : -1;
   int nl = 0;
   auto ev_before = [&](int kind, int range) -> cudaError_t {
@@ -528,10 +629,15 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
   // other on the stream without a pack kernel draining the machine in between.
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) continue;
-    if (!plan->ws) return DD_ERR_NOMEM;
+    if (!plan->ws || plan->ws_have < plan->ws_bytes + plan->ws_pair_bytes) return DD_ERR_NOMEM;
     DD_CUDA(ev_before(0, (int)(&r - plan->ranges.data())));
     DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
     DD_CUDA(ev_after());
+    if (dd::use_pairs(plan, r)) {  // DD_KERNEL_SUBBAND: pre-sum the packed rows into the pair rows
+      DD_CUDA(ev_before(3, (int)(&r - plan->ranges.data())));
+      DD_CUDA(dd::launch_pairs(plan, r, stream));
+      DD_CUDA(ev_after());
+    }
   }
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) {
@@ -586,6 +692,7 @@ static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) continue;
     DD_CUDA(dd::launch_pack(plan, r, plan->h_in_dev, stream));
+    if (dd::use_pairs(plan, r)) DD_CUDA(dd::launch_pairs(plan, r, stream));
   }
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) {
@@ -623,7 +730,7 @@ int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void*
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) {
       if (!r.d_delays) return DD_ERR_INVALID;  // uploaded by dd_plan_create / dd_plan_set_kernel
-    } else if (!plan->ws) {
+    } else if (!plan->ws || plan->ws_have < plan->ws_bytes + plan->ws_pair_bytes) {
       return DD_ERR_NOMEM;
     }
   }
@@ -685,14 +792,54 @@ int dd_plan_work(const dd_plan_t* p, int64_t* dm_samples, int64_t* adds) {
 int dd_plan_launches(const dd_plan_t* p, int32_t* n) {
   if (!p || !n) return DD_ERR_INVALID;
   int k = 0;
-  for (const auto& r : p->ranges) k += (p->variant == DD_KERNEL_DIRECT || !r.tiled_ok) ? 1 : 1 + r.planes;
+  for (const auto& r : p->ranges)
+    k += (p->variant == DD_KERNEL_DIRECT || !r.tiled_ok) ? 1 : 1 + r.planes + (dd::use_pairs(p, r) ? 1 : 0);
   *n = k;
+  return DD_OK;
+}
+
+int dd_plan_executed_adds(const dd_plan_t* p, int64_t* adds) {
+  if (!p || !adds) return DD_ERR_INVALID;
+  int64_t total = 0;
+  for (const auto& r : p->ranges) {
+    const int64_t brute = (int64_t)r.ndm * r.nout * p->nchans;
+    if (dd::use_pairs(p, r)) {
+      total += r.adds_pair;
+    } else if ((p->variant == DD_KERNEL_SHARED || p->variant == DD_KERNEL_SUBBAND) && r.tiled_ok && r.mode == dd::kModeDelta) {
+      // quad sums shared while no channel of the quad changes: a trial step costs 1 add per sample if unchanged,
+      // else 3 (the new quad sum) + 1; the first trial of a group always 3 + 1.  Counted from the table.
+      int64_t units = 0;  // adds per (time sample) summed over (block, quad, group, trial)
+      const size_t nent = r.h_meta.size() / 4;
+      for (size_t i = 0; i < nent; ++i) {
+        const uint32_t any = r.h_meta[i * 4 + 3];
+        units += 4;
+        for (int j = 1; j < r.RD; ++j) units += ((any >> j) & 1u) ? 4 : 1;
+      }
+      // the table covers padded trials and channel rows; scale to the real (trial, channel) count
+      const double scale = (double)brute / ((double)r.nblocks * r.Dcta * r.Cpad * (double)r.nout);
+      total += (int64_t)((double)units * (double)r.nout * scale);
+    } else {
+      total += brute;
+    }
+  }
+  *adds = total * p->nbeams;
+  return DD_OK;
+}
+
+int dd_plan_pair_info(const dd_plan_t* p, int32_t r, int32_t* enabled, int32_t* pairs_per_stage, int32_t* row_superwords,
+                      int32_t* npairs) {
+  if (!p || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  if (enabled) *enabled = dd::use_pairs(p, q) ? 1 : 0;
+  if (pairs_per_stage) *pairs_per_stage = q.Cc2;
+  if (row_superwords) *row_superwords = 2 * (q.T + q.Smax2);
+  if (npairs) *npairs = q.Cpad / 2;
   return DD_OK;
 }
 
 int dd_plan_workspace_bytes(const dd_plan_t* p, int64_t* bytes) {
   if (!p || !bytes) return DD_ERR_INVALID;
-  *bytes = p->ws_bytes;
+  *bytes = p->ws_bytes + p->ws_pair_bytes;
   return DD_OK;
 }
 
@@ -700,24 +847,51 @@ int dd_plan_set_workspace(dd_plan_t* p, void* dev, int64_t bytes) {
   if (!p) return DD_ERR_INVALID;
   if (dev) {
     if (!aligned16(dev)) return DD_ERR_ALIGN;
-    if (bytes < p->ws_bytes) return DD_ERR_NOMEM;
+    if (bytes < p->ws_bytes + p->ws_pair_bytes) return DD_ERR_NOMEM;
     if (p->ws && p->ws_owned) cudaFree(p->ws);
     p->ws = dev;
     p->ws_owned = false;
+    p->ws_have = bytes;
     return DD_OK;
   }
-  if (p->ws && !p->ws_owned) p->ws = nullptr;
+  if (p->ws && !p->ws_owned) p->ws = nullptr, p->ws_have = 0;
   return ensure_workspace(p);
 }
 
 int dd_plan_set_kernel(dd_plan_t* p, int32_t variant) {
   if (!p) return DD_ERR_INVALID;
   if (variant != DD_KERNEL_AUTO && variant != DD_KERNEL_DIRECT && variant != DD_KERNEL_TILED &&
-      variant != DD_KERNEL_SHARED)
+      variant != DD_KERNEL_SHARED && variant != DD_KERNEL_SUBBAND)
     return DD_ERR_INVALID;
-  if (variant == DD_KERNEL_DIRECT) {
+  if (variant == DD_KERNEL_DIRECT && p->device >= 0) {
     int rc = ensure_direct_tables(p, false);
     if (rc != DD_OK) return rc;
+  }
+  if (variant == DD_KERNEL_SUBBAND && p->ws_pair_bytes == 0) {
+    // first use: pair tables of every range that qualifies, their device copies, and room for the pair arrays
+    try {
+      int64_t off = p->ws_bytes;
+      for (auto& r : p->ranges) {
+        build_pair_tables(*p, r);
+        if (!r.pair_ok) continue;
+        r.ws2_offset = off;
+        off += r.ws2_bytes;
+      }
+      p->ws_pair_bytes = off - p->ws_bytes;
+    } catch (const std::bad_alloc&) {
+      return DD_ERR_NOMEM;
+    }
+    if (p->device >= 0) {
+      for (auto& r : p->ranges)
+        if (r.pair_ok) {
+          int rc = upload_pair_tables(r);
+          if (rc != DD_OK) return rc;
+        }
+      if (p->ws_owned || !p->ws) {
+        int rc = ensure_workspace(p);
+        if (rc != DD_OK) return rc;
+      }
+    }
   }
   p->variant = variant;
   return DD_OK;
@@ -729,7 +903,7 @@ int dd_plan_set_profiling(dd_plan_t* p, int32_t max_executes) {
   p->prof_events.clear();
   p->prof_slots = 0;
   p->prof_calls = 0;
-  const size_t max_launch = 2 * p->ranges.size();
+  const size_t max_launch = 3 * p->ranges.size();
   try {
     p->prof_kind.assign(max_launch * max_executes, 0);
     p->prof_range.assign(max_launch * max_executes, 0);
@@ -750,7 +924,7 @@ int dd_plan_set_profiling(dd_plan_t* p, int32_t max_executes) {
 int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* ms, int32_t* kind, int32_t* range,
                          int32_t* n) {
   if (!p || !ms || !n || slot < 0 || slot >= p->prof_slots || cap < 0) return DD_ERR_INVALID;
-  const size_t max_launch = 2 * p->ranges.size();
+  const size_t max_launch = 3 * p->ranges.size();
   const int cnt = std::min<int>(cap, p->prof_count[slot]);
   for (int i = 0; i < cnt; ++i) {
     const size_t k = (size_t)slot * max_launch + i;
@@ -763,10 +937,15 @@ int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* m
 }
 
 int dd_plan_table(const dd_plan_t* p, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes) {
-  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 2) return DD_ERR_INVALID;
+  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 6) return DD_ERR_INVALID;
   const auto& q = p->ranges[r];
-  const void* src = which == 0 ? (const void*)q.h_meta.data() : which == 1 ? (const void*)q.h_dmin.data() : (const void*)q.h_span.data();
-  const size_t n = which == 0 ? q.h_meta.size() * 4 : which == 1 ? q.h_dmin.size() * 4 : q.h_span.size() * 4;
+  const void* srcs[7] = {q.h_meta.data(), q.h_dmin.data(), q.h_span.data(), q.h_meta2.data(), q.h_dmin2.data(),
+                         q.h_span2.data(), q.h_delta.data()};
+  const size_t sizes[7] = {q.h_meta.size(), q.h_dmin.size(), q.h_span.size(), q.h_meta2.size(), q.h_dmin2.size(),
+                           q.h_span2.size(), q.h_delta.size()};
+  if (which >= 3 && !q.pair_ok) return DD_ERR_INVALID;
+  const void* src = srcs[which];
+  const size_t n = sizes[which] * 4;
   *bytes = (int64_t)n;
   if (host_buf) {
     if (cap_bytes < (int64_t)n) return DD_ERR_NOMEM;

@@ -81,6 +81,20 @@ __device__ __forceinline__ void lds_if_bit(uint4& w, uint32_t& addr, uint32_t m)
       : "r"(m), "n"(1u << BIT));
 }
 
+// pair mode: bit BIT of md = the delay of channel 2v stepped (address += 32: two superwords per time index), bit BIT of
+// mf = the row selector p flipped (address ^= 16); reload in place if either is set
+template <int BIT>
+__device__ __forceinline__ void lds_pair_if(uint4& w, uint32_t& addr, uint32_t md, uint32_t mf) {
+  asm volatile(
+      "{\n .reg .pred p, q, r;\n .reg .b32 t;\n and.b32 t, %5, %7;\n setp.ne.u32 p, t, 0;\n"
+      " and.b32 t, %6, %7;\n setp.ne.u32 q, t, 0;\n or.pred r, p, q;\n"
+      " @p add.u32 %4, %4, 32;\n"
+      " @q xor.b32 %4, %4, 16;\n"
+      " @r ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n}"
+      : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w), "+r"(addr)
+      : "r"(md), "r"(mf), "n"(1u << BIT));
+}
+
 __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4& b) {
   // one IADD3 per 32-bit word: two channels, and (NL == 8) two 16-bit time lanes, per instruction
   acc.x = acc.x + a.x + b.x;
@@ -100,6 +114,7 @@ struct TiledParams {
   int rowpitch;      // superwords per staged row = T + Smax
   int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
   float accum_scale;  // 0: store; else out = value * accum_scale + out (high byte plane of uint16 input)
+  int wmul;           // superwords per time index in the packed rows: 1, or 2 for the interleaved pair rows (kModeDeltaPair)
 };
 
 __host__ __device__ inline size_t tiled_stage_bytes(int mode, int NL, int Cc, int rowpitch, int G) {
@@ -180,12 +195,23 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4&
     // by ONE branch on its "any channel changed" bit: neighbouring channels have nearly the same delay
     // curve and often change at the same trial.  `any` sits in a uniform register (stage_delta),
     // which makes this a branch without reconvergence bookkeeping.
-    if (any & (1u << J)) {
-      lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
-      lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
-      lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
-      lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
-      if constexpr (SHARE) sum4(t4, wa, wb, wc, wd);
+    if constexpr (SHARE) {
+      if (any & (1u << J)) {
+        lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
+        lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
+        lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
+        lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
+        sum4(t4, wa, wb, wc, wd);
+      }
+    } else {
+      // (measured: one uniform branch per channel PAIR instead of per quad skips more predicated-off loads but
+      // costs more than it saves: 116.2 vs 111.7 ms on config 3; 109.7 vs 107.0 ms in the SHARE variant)
+      if (any & (1u << J)) {
+        lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
+        lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
+        lds_if_bit<delta_bit(J, 2)>(wc, ac, bits);
+        lds_if_bit<delta_bit(J, 3)>(wd, ad, bits);
+      }
     }
     if constexpr (SHARE) {
       add1(acc[J], t4);  // the quad's sum is unchanged since the last taken step: one term per word
@@ -230,6 +256,50 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
       add_pair(acc[0], wc, wd);
     }
     delta_steps<1, SHARE>(acc, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
+  }
+}
+
+// pair mode (kModeDeltaPair): rows are two-channel sub-bands, quads A..D of them; one table entry per quad =
+//   {delay-step bits | any(1..4) in bit 7 of each byte, flip bits | any(5..7), offA | offB<<16, offC | offD<<16}
+template <int J>
+__device__ __forceinline__ void pair_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t& aa,
+                                           uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bd, uint32_t bf, uint32_t u0,
+                                           uint32_t u1) {
+  if constexpr (J < kRD) {
+    constexpr uint32_t anymask = J <= 4 ? (0x80u << (8 * (J - 1))) : (0x80u << (8 * (J - 5)));
+    if ((J <= 4 ? u0 : u1) & anymask) {  // uniform: some pair of the quad changes at this trial step
+      lds_pair_if<delta_bit(J, 0)>(wa, aa, bd, bf);
+      lds_pair_if<delta_bit(J, 1)>(wb, ab, bd, bf);
+      lds_pair_if<delta_bit(J, 2)>(wc, ac, bd, bf);
+      lds_pair_if<delta_bit(J, 3)>(wd, ad, bd, bf);
+    }
+    add_pair(acc[J], wa, wb);
+    add_pair(acc[J], wc, wd);
+    pair_steps<J + 1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bd, bf, u0, u1);
+  }
+}
+
+__device__ __forceinline__ void stage_pairs(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {
+  uint4 m;
+  lds_sw(m, smeta);
+#pragma unroll 1
+  for (int cc = 0; cc < Cc; cc += 4) {
+    uint32_t aa = sdata + (m.z & 0xffffu);
+    uint32_t ab = sdata + (m.z >> 16);
+    uint32_t ac = sdata + (m.w & 0xffffu);
+    uint32_t ad = sdata + (m.w >> 16);
+    const uint32_t bd = m.x, bf = m.y;
+    const uint32_t u0 = __reduce_or_sync(0xffffffffu, m.x), u1 = __reduce_or_sync(0xffffffffu, m.y);
+    uint4 wa, wb, wc, wd;
+    lds_sw(wa, aa);
+    lds_sw(wb, ab);
+    lds_sw(wc, ac);
+    lds_sw(wd, ad);
+    smeta += meta_row;
+    lds_sw(m, smeta);  // next quad's entry (see stage_delta)
+    add_pair(acc[0], wa, wb);
+    add_pair(acc[0], wc, wd);
+    pair_steps<1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bd, bf, u0, u1);
   }
 }
 
@@ -314,7 +384,9 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
   }
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
-    if constexpr (is_delta(MODE))
+    if constexpr (MODE == kModeDeltaPair)
+      stage_pairs(acc, sdata, smeta, Cc, meta_row);
+    else if constexpr (is_delta(MODE))
       stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
     else
       stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
@@ -412,7 +484,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   // byte count.  A warp issues chunk k when it starts iteration k - ahead (ahead = nstages - 2): the
   // stage it refills was consumed two iterations ago, so the wait on its empty barrier is normally
   // already satisfied.  Row start and length of the warp's NEXT chunk are fetched one turn early.
-  const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T;
+  const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T * p.wmul;
   const long long tab = (long long)blk * p.Cpad;
   const char* meta_blk = reinterpret_cast<const char*>(p.meta) + (size_t)blk * (size_t)nchunks * meta_bytes;
   const int lane = tid & 31;
@@ -425,8 +497,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     pf_bytes = 0;
     if (k < nchunks && lane < p.Cc) {
       const int c = k * p.Cc + lane;
-      pf_d0 = __ldg(p.dmin + tab + c);
-      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
+      pf_d0 = __ldg(p.dmin + tab + c) * p.wmul;
+      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes * p.wmul;
     }
   };
   // stage and wrap count of a chunk index are tracked incrementally (no divisions in the main loop)
@@ -473,7 +545,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const int ti = tid - g * p.T;  // superword inside the time tile
   Lanes<NL> lanes;
   lanes.init();
-  const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
+  const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes * p.wmul;
   const uint32_t entry_bytes = 16u;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
   const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
@@ -546,6 +618,7 @@ static cudaError_t set_smem_t() {
   X(8, kModeGeneral, 256) X(8, kModeGeneralReuse, 256) X(8, kModeDelta, 256)                   \
   X(8, kModeGeneral, 512) X(8, kModeGeneralReuse, 512) X(8, kModeDelta, 512)                   \
   X(8, kModeDeltaShare, 256) X(8, kModeDeltaShare, 512) X(4, kModeDeltaShare, 256) X(4, kModeDeltaShare, 512) \
+  X(8, kModeDeltaPair, 256) X(8, kModeDeltaPair, 512)                                           \
   X(4, kModeGeneral, 256) X(4, kModeGeneralReuse, 256) X(4, kModeDelta, 256)                   \
   X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)                   \
   X(16, kModeGeneral, 256) X(16, kModeGeneral, 512)
@@ -562,35 +635,41 @@ cudaError_t configure_kernels(const dd_plan*) {
 cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, cudaStream_t stream, int blk0, int nblk) {
   if (nblk <= 0) nblk = r.nblocks - blk0;
   if (blk0 < 0 || nblk <= 0 || blk0 + nblk > r.nblocks) return cudaErrorInvalidValue;
+  const bool pairs = use_pairs(p, r);
   TiledParams tp;
-  tp.meta = r.d_meta;
-  tp.dmin = r.d_dmin;
-  tp.span = r.d_span;
+  tp.meta = pairs ? r.d_meta2 : r.d_meta;
+  tp.dmin = pairs ? r.d_dmin2 : r.d_dmin;
+  tp.span = pairs ? r.d_span2 : r.d_span;
+  tp.wmul = pairs ? 2 : 1;
   tp.out = out_dev + r.offset;
   tp.out_beam_stride = p->beam_stride;
   tp.pitch = r.pitch;
-  tp.Wp = r.Wp;
+  tp.Wp = pairs ? 2 * r.Wp : r.Wp;
   tp.H = r.H;
   tp.nout = r.nout;
   tp.ntau = r.ntau;
   tp.ndm = r.ndm;
-  tp.Cpad = r.Cpad;
+  tp.Cpad = pairs ? r.Cpad / 2 : r.Cpad;  // rows of the packed array the kernel walks (pairs: sub-band rows)
   tp.G = r.G;
   tp.T = r.T;
-  tp.Cc = r.Cc;
-  tp.nstages = r.stages;
+  tp.Cc = pairs ? r.Cc2 : r.Cc;
+  tp.nstages = pairs ? r.stages2 : r.stages;
   tp.blk0 = blk0;
   tp.nblk = nblk;
-  tp.rowpitch = r.T + r.Smax;
-  tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;
+  tp.rowpitch = pairs ? 2 * (r.T + r.Smax2) : r.T + r.Smax;
+  tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;  // pairs: flush/2 sub-band rows = the same number of stages
   const long long nctas = (long long)nblk * r.ntau * p->nbeams;
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  const size_t smem = tiled_smem_bytes(r);
+  const size_t smem = pairs ? kBarRegion + (size_t)r.stages2 * tiled_stage_bytes(kModeDeltaPair, r.NL, r.Cc2, tp.rowpitch, r.G) + 512
+                            : tiled_smem_bytes(r);
   const int nt = r.G * r.T;
-  const int mode = (r.mode == kModeDelta && p->variant == DD_KERNEL_SHARED) ? (int)kModeDeltaShare : r.mode;
+  const int mode = pairs ? (int)kModeDeltaPair
+                   : (r.mode == kModeDelta && (p->variant == DD_KERNEL_SHARED || p->variant == DD_KERNEL_SUBBAND))
+                       ? (int)kModeDeltaShare
+                       : r.mode;
   // one launch per byte plane: low bytes stored, high bytes added with weight 256
   for (int plane = 0; plane < r.planes; ++plane) {
-    tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + r.ws_offset + plane * r.plane_bytes);
+    tp.P = reinterpret_cast<const uint4*>(static_cast<const char*>(p->ws) + (pairs ? r.ws2_offset : r.ws_offset + plane * r.plane_bytes));
     tp.accum_scale = plane == 0 ? 0.0f : 256.0f;
     cudaError_t e = cudaErrorInvalidConfiguration;
 #define DD_GO(NL_, MODE_, NT_) \

@@ -160,3 +160,25 @@ def test_full_cfg4_uint16_ulp_histogram():
 @gpu
 def test_full_cfg5_32beams():
     _run_full(5, [0, 4, 9, 13, 18, 22, 27, 31], max(_STRIDE, 1) * (1 if _STRIDE == 1 else 2))
+
+
+@gpu
+def test_full_cfg3_subband_variant_equals_default_everywhere():
+    """NEXT-3 at full size: the two-channel sub-band variant (half the brute-force adds) writes the same bits as the
+    default kernel for EVERY element of the config-3 plane (the default is compared with the oracle above)."""
+    import torch
+    from paper_2605_03531_b200 import binding as B
+
+    w = W.CONFIGS[3]
+    x = torch.from_numpy(W.generate(w)).cuda()
+    plan = B.Plan.from_workload(w)
+    a = torch.full((plan.out_elems(),), -1.0, dtype=torch.float32, device="cuda")
+    plan.execute(x, a, torch.cuda.current_stream())
+    plan.set_kernel(B.DD_KERNEL_SUBBAND)
+    assert all(plan.pair_info(r)["enabled"] == 1 for r in range(3))
+    assert plan.executed_adds() < 0.51 * plan.work()[1]
+    b = torch.full((plan.out_elems(),), -1.0, dtype=torch.float32, device="cuda")
+    plan.execute(x, b, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert bool(torch.equal(a.view(torch.int32), b.view(torch.int32)))
+    plan.destroy()

@@ -387,3 +387,49 @@ def test_row_pitch_regression_gpu():
         plan, flat = gpu_run(w, x, TILED)
         assert plan.tile_shape(0)["tiled"] == 1
         check_full(w, x, plan, flat)
+
+
+SUBBAND = 4
+_CW = -200.0 / 4096   # SPOTLIGHT's channel width: neighbouring channels differ by less than a sample in delay
+
+
+@pytest.mark.parametrize("nchans", [272, 271, 64])
+def test_subband_pairs_variant(nchans):
+    """DD_KERNEL_SUBBAND: two-channel sub-band rows pre-summed once per execute, one load and
+    one add per trial and PAIR -- half the brute-force adds, identical bits.  Odd channel counts pair the last channel
+    with a zero row; a coarse range in the same plan keeps its own kernel."""
+    w = W.Workload("pairs", 600.0, _CW, nchans, 1.31072e-3, 2 ** 15 + 3, 1, 8,
+                   (W.DMRange(0.0, 0.1, 203, 1), W.DMRange(200.0, 0.2, 150, 2), W.DMRange(600.0, 3.0, 41, 4),
+                    W.DMRange(900.0, 0.9, 90, 1), W.DMRange(100.0, 300.0, 12, 2)), 353103, 128, 12)
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, SUBBAND)
+    en = [plan.pair_info(r)["enabled"] for r in range(5)]
+    assert en == [1, 1, 1, 1, 0]
+    assert plan.executed_adds() < 0.56 * plan.work()[1]
+    assert plan.launches() == 5 + 5 + 4
+    check_full(w, x, plan, flat)
+
+
+def test_subband_saturated_input_and_flushes():
+    """Pair rows hold up to 2 * 255 * decim per 16-bit lane and the packed accumulators are flushed every flush/2 pair
+    rows: saturated input over 1024 channels crosses several flushes at the exact lane bound."""
+    nch, ns = 1024, 2 ** 14
+    x = np.full((1, nch, ns), 255, dtype=np.uint8)
+    x[0, 7::13, :] = 254
+    x[0, :, 5000:5003] = 0
+    for decim, step in ((1, 0.3), (4, 1.2), (8, 2.4)):
+        w = W.Workload("pairsat", 750.0, _CW, nch, 1.31072e-3, ns, 1, 8, (W.DMRange(0.0, step, 90, decim),), 1, 0, 0)
+        plan, flat = gpu_run(w, x, SUBBAND)
+        assert plan.pair_info(0)["enabled"] == 1
+        check_full(w, x, plan, flat)
+
+
+def test_subband_host_path_and_two_beams():
+    nch, ns = 128, 2 ** 14
+    rng = np.random.default_rng(4242)
+    x = rng.integers(0, 256, size=(2, nch, ns), dtype=np.uint8)
+    w = W.Workload("pairhost", 700.0, _CW, nch, 1.31072e-3, ns, 2, 8,
+                   (W.DMRange(0.0, 1.0, 300, 1), W.DMRange(300.0, 2.0, 100, 2)), 1, 0, 0)
+    plan, flat = gpu_run(w, x, SUBBAND, host_path=True)
+    assert plan.pair_info(0)["enabled"] == 1 and plan.pair_info(1)["enabled"] == 1
+    check_full(w, x, plan, flat, check_pad=False)

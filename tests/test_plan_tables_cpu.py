@@ -203,3 +203,82 @@ def test_tuned_plan_goes_through_the_same_checks():
         p.destroy()
     finally:
         del os.environ["DD_MODE"]
+
+
+def _decode_pairs(plan, r):
+    """DD_KERNEL_SUBBAND tables -> delays of both channels of every pair row: [nblocks*Dcta][Cpad]."""
+    info, shape, pi = plan.tile_info(r), plan.tile_shape(r), plan.pair_info(r)
+    g, cpad, nb = shape["trial_groups"], shape["cpad"], shape["nblocks"]
+    nvc, cc2, rowsw = pi["npairs"], pi["pairs_per_stage"], pi["row_superwords"]
+    assert nvc == cpad // 2 and cc2 * 2 == shape["chans_per_stage"]
+    e = plan.table(r, 3).reshape(nb, nvc // 4, g, 4).astype(np.int64)
+    dmin = plan.table(r, 4).astype(np.int64).reshape(nb, nvc)
+    span = plan.table(r, 5).astype(np.int64).reshape(nb, nvc)
+    delta = plan.table(r, 6).astype(np.int64)
+    assert (dmin % 8 == 0).all() and (span % 8 == 0).all() and (2 * (span + info["words_per_cta"]) <= rowsw).all()
+    out = np.zeros((nb, g, 8, cpad), dtype=np.int64)
+    anyb = np.zeros((nb, nvc // 4, g), dtype=np.int64)
+    for q in range(4):
+        field = (e[..., 2 + q // 2] >> (16 * (q % 2))) & 0xFFFF                  # [nb][quad][g] byte offset in the stage
+        assert (field % 16 == 0).all()
+        vrow = (np.arange(q, nvc, 4) % cc2) * rowsw                                # superwords, row of the pair in its stage
+        rel = field // 16 - vrow[None, :, None]
+        assert (rel >= 0).all()
+        D = rel // 2 + dmin[:, q::4][:, :, None]
+        P = rel % 2
+        for j in range(8):
+            if j > 0:
+                n = (j - 1) * 4 + q
+                bit = 1 << ((n // 7) * 8 + n % 7)
+                cd = (e[..., 0] & bit) != 0
+                cf = (e[..., 1] & bit) != 0
+                anyb |= (cd | cf).astype(np.int64) << j
+                D = D + cd
+                P = P ^ cf
+            assert (D - dmin[:, q::4][:, :, None] <= span[:, q::4][:, :, None]).all(), "loads stay inside the staged row"
+            out[:, :, j, 2 * q::8] = D.transpose(0, 2, 1)
+            out[:, :, j, 2 * q + 1::8] = (D + delta[None, q::4, None] + P).transpose(0, 2, 1)
+    stored = np.zeros_like(anyb)
+    for j in range(1, 8):
+        word, byte = (0, j - 1) if j <= 4 else (1, j - 5)
+        stored |= ((e[..., word] >> (8 * byte + 7)) & 1) << j
+    assert np.array_equal(stored, anyb), "any-changed bits (bit 7 of each table byte) are the OR of the quad's bits"
+    return out.reshape(nb * g * 8, cpad)
+
+
+@pytest.mark.parametrize("cfg,nchans", [(3, 4096), (3, 4095), (3, 1001), (1, 128)])
+def test_pair_tables_reproduce_the_delay_table(cfg, nchans):
+    """DD_KERNEL_SUBBAND (NEXT-3): the pair-row tables, decoded independently of the kernel, give back the oracle's
+    delay of BOTH channels of every pair for every trial; padded rows follow their partner."""
+    w = W.CONFIGS[cfg]
+    if nchans != w.nchans:
+        w = W.scaled(w, nchans=nchans, nsamps=2 ** 16)
+    plan = _host_plan(w)
+    plan.set_kernel(B.DD_KERNEL_SUBBAND)
+    for r, rg in enumerate(w.ranges):
+        pi = plan.pair_info(r)
+        if plan.tile_info(r)["mode"] != 2:
+            assert pi["enabled"] == 0                       # coarse grids are not delta coded: no pair mode
+            continue
+        want = oracle.delay_table(w.f_top_mhz, w.chan_width_mhz, w.nchans, w.tsamp_s, rg.decim, rg.dm_lo, rg.dm_step, rg.ndm)
+        npair = w.nchans // 2
+        diff = want[:, 1:2 * npair:2] - want[:, 0:2 * npair:2]
+        valid = bool(((diff.max(axis=0) - diff.min(axis=0)) <= 1).all())   # two neighbouring values per pair over ALL trials
+        assert pi["enabled"] == int(valid), (cfg, r)
+        if cfg == 3 and nchans >= 4095:
+            assert valid                                      # the SPOTLIGHT-shaped beam qualifies in all three ranges
+        if not valid:
+            continue
+        shape = plan.tile_shape(r)
+        got = _decode_pairs(plan, r)
+        rows = np.minimum(np.arange(got.shape[0]), rg.ndm - 1)
+        assert np.array_equal(got[:, : w.nchans], want[rows]), (cfg, r)
+        if w.nchans % 2:                                     # the pad partner of the last channel copies its delay
+            assert np.array_equal(got[:, w.nchans], want[rows][:, -1])
+        stage = -(-(pi["pairs_per_stage"] * pi["row_superwords"] * 16 + pi["pairs_per_stage"] // 4 * shape["trial_groups"] * 16) // 128) * 128
+        assert pi["pairs_per_stage"] * pi["row_superwords"] * 16 <= 65536 and 128 + 2 * stage + 512 <= 227 * 1024
+    brute = plan.work()[1]
+    assert plan.executed_adds() < 0.52 * brute if cfg == 3 and nchans == 4096 else plan.executed_adds() <= brute
+    plan.set_kernel(B.DD_KERNEL_TILED)
+    assert plan.executed_adds() == brute
+    plan.destroy()
