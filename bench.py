@@ -285,6 +285,8 @@ def run_ours(args, w):
     # one beam per rank, a different seeded beam each (weak scaling over independent beams)
     x_host = W.generate_beam(w, beam=rank)
     plan = B.Plan.from_workload(w)
+    if args.variant:
+        plan.set_kernel(args.variant)
     dm_samples, adds = plan.work()
     x = torch.from_numpy(x_host.view(np.int16) if x_host.dtype == np.uint16 else x_host).to(dev)
     out = torch.empty(plan.out_elems(), dtype=torch.float32, device=dev)
@@ -396,6 +398,34 @@ def run_ours(args, w):
                "candidates_above_threshold": int(cnt.sum().item())}
         del snr, tmx, cnt
 
+    # NEXT-3: the exact two-channel sub-band variant, an opt-in shortcut that performs about half the
+    # adds of the brute-force count the roofline divides by -- reported beside the metric, never inside `value`
+    subband = None
+    if rank == 0 and world == 1 and not args.no_subband and not args.variant:
+        try:
+            plan.set_profiling(0)
+            plan.set_kernel(B.DD_KERNEL_SUBBAND)
+            for _ in range(2):
+                plan.execute(x, out, stream)
+            b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            b0.record(stream)
+            for _ in range(5):
+                plan.execute(x, out, stream)
+            b1.record(stream)
+            torch.cuda.synchronize()
+            sb_ms = b0.elapsed_time(b1) / 5
+            executed = plan.executed_adds()
+            subband = {"variant": "DD_KERNEL_SUBBAND (exact two-channel sub-bands)", "ms_per_execute": sb_ms,
+                       "dm_samples_per_s": dm_samples / (sb_ms * 1e-3), "executed_adds": executed, "brute_force_adds": adds,
+                       "executed_over_brute_force": executed / adds,
+                       "brute_force_add_bound_ms": adds / peak_adds * 1e3,
+                       "ranges_on_pair_rows": [bool(plan.pair_info(r)["enabled"]) for r in range(plan.nranges)],
+                       "launches_per_execute": plan.launches(), "workspace_bytes": plan.workspace_bytes()}
+            plan.set_kernel(B.DD_KERNEL_AUTO)
+        except Exception as e:
+            subband = {"skipped": repr(e)}
+
     # the other BASELINE configs (1, 2, 4, 5), reported beside the headline: `value` stays on config 3
     other = None
     if rank == 0 and world == 1 and not args.no_other_configs:
@@ -426,7 +456,7 @@ def run_ours(args, w):
                        "l2": "inputs larger than L2 (1.07 GB input, 4.0 GB packed copy, 3.8 GB output per step)",
                        "parallelism": "replicas: one beam per GPU, no collective"},
             "input_gb_per_s": world * w.nchans * w.nsamps * (w.in_bits // 8) / (ms_total / args.steps * 1e-3) / 1e9,
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps, "other_configs": other,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps, "subband": subband, "other_configs": other,
             "gpu_launches": plan.launches() * args.steps, "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
@@ -445,6 +475,8 @@ def main(argv=None):
     ap.add_argument("--ref-trials", type=int, default=48, help="oracle sample: trials per range")
     ap.add_argument("--e2e-steps", type=int, default=0, help="end-to-end steps (0 = as many as --steps)")
     ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--no-subband", action="store_true")
+    ap.add_argument("--variant", type=int, default=0, help="dd_plan_set_kernel variant of the timed plan (measurements)")
     ap.add_argument("--stub-body", action="store_true", help=argparse.SUPPRESS)  # tests: N-rank plumbing on CPU / gloo
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

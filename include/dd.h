@@ -196,7 +196,7 @@ int dd_plan_launches(const dd_plan_t* plan, int32_t* n_launches);
  * DD_KERNEL_SUBBAND included).  Equals the brute-force count of dd_plan_work for DD_KERNEL_AUTO / TILED / DIRECT. */
 int dd_plan_executed_adds(const dd_plan_t* plan, int64_t* adds);
 /* DD_KERNEL_SUBBAND, range r (any pointer may be NULL): whether the range runs on two-channel sub-bands, pairs per
- * pipeline stage, superwords per staged pair row (two per time index), number of pair rows incl. padding. */
+ * pipeline stage (each with its two pre-summed rows), superwords per staged row, number of pairs incl. padding. */
 int dd_plan_pair_info(const dd_plan_t* plan, int32_t r, int32_t* enabled, int32_t* pairs_per_stage,
                       int32_t* row_superwords, int32_t* npairs);
 
@@ -225,8 +225,9 @@ int dd_plan_tile_shape(const dd_plan_t* plan, int32_t r, int32_t* trial_groups, 
 /* Test hook: the tables of the tiled kernel for range r as they are uploaded.  which = 0: the per-trial table
  * (uint32 words; layout per mode in DESIGN.md "Data layout"), 1: start of the staged row per (trial block,
  * channel) (int32 superwords, multiple of 8), 2: its length beyond the time tile (int32).  After
- * dd_plan_set_kernel(DD_KERNEL_SUBBAND): 3, 4, 5 = the same three tables of the pair mode (per pair row, delays of
- * channel 2v), 6 = delta_v per pair (int32).  *bytes = size; the table is copied when host_buf != NULL
+ * dd_plan_set_kernel(DD_KERNEL_SUBBAND): 3 = the pair-mode table (per trial block, quad of pairs and trial group 20
+ * words: changed bits, any bits, 0, 0, then eight 16-bit byte offsets per pair), 4, 5 = start / span per staged row
+ * (rows 2v, 2v+1 = the two pre-summed rows of pair v), 6 = delta_v per pair (int32).  *bytes = size; the table is copied when host_buf != NULL
  * (DD_ERR_NOMEM if cap_bytes is too small). */
 int dd_plan_table(const dd_plan_t* plan, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes);
 

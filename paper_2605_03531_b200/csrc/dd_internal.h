@@ -38,8 +38,8 @@ __host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? 
 //                      2v, 2v+1 differ in delay by delta_v or delta_v + 1 for EVERY trial of the range, so the two
 //                      pre-summed rows U_p[i] = y_2v[i] + y_2v+1[i + delta_v + p], p = 0, 1 (built once per execute,
 //                      interleaved: superword 2i + p) replace both channels: one load and one add per trial and PAIR.
-//                      Table as kModeDelta per quad of pairs, with two bits per trial step and pair: "delay of
-//                      channel 2v changed" (address += 32) and "p flipped" (address ^= 16).
+//                      Table per quad of pairs: one "changed" bit per trial step and pair as in kModeDelta, plus a byte
+//                      offset per trial and pair that selects the row (U_0 or U_1) and the delay.
 enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3, kModeDeltaPair = 4 };
 __host__ __device__ constexpr bool is_delta(int mode) {
   return mode == kModeDelta || mode == kModeDeltaShare || mode == kModeDeltaPair;
@@ -58,6 +58,7 @@ __host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 
 // group) -- eight 16-bit superword offsets, or (NL = 16) four 32-bit byte offsets inside the stage, row
 // included -- or one 16-byte entry per channel quad in delta mode.
 __host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int NL, int Cc, int G) {
+  if (mode == 4) return (size_t)(Cc / 8) * (size_t)G * 80;  // kModeDeltaPair: 5 entries per quad of pairs (8 rows)
   return (size_t)(is_delta(mode) ? Cc / 4 : Cc) * (size_t)G * 16;
 }
 
@@ -100,12 +101,12 @@ struct RangePlan {
   int32_t* d_delays = nullptr;  // [ndm][nchans], only for the direct kernel (lazy)
   // two-channel sub-bands (kModeDeltaPair), built by dd_plan_set_kernel(DD_KERNEL_SUBBAND): rows are pairs
   int pair_ok = 0;        // 1: this range runs in pair mode under DD_KERNEL_SUBBAND
-  int Cc2 = 0;            // pairs per pipeline stage (= Cc / 2)
-  int Smax2 = 0;          // largest staged span of a pair row (time superwords; the row holds 2 per time index)
+  int Cc2 = 0;            // pairs per pipeline stage (= Cc / 2; a stage holds Cc rows: U_0 and U_1 of each pair)
+  int Smax2 = 0;          // largest staged span of a pair row (superwords)
   int stages2 = 0;
-  int64_t ws2_offset = 0, ws2_bytes = 0;  // pair array [nbeams][Cpad/2][2*Wp] superwords in the workspace
-  std::vector<uint32_t> h_meta2;          // [nblocks][Cpad/8][G] {Pd bits | any 1..4, Pf bits | any 5..7, offA|offB<<16, offC|offD<<16}
-  std::vector<int32_t> h_dmin2, h_span2;  // [nblocks][Cpad/2] of channel 2v (time superwords)
+  int64_t ws2_offset = 0, ws2_bytes = 0;  // pair array [nbeams][Cpad][Wp] superwords in the workspace: rows 2v, 2v+1 = U_0, U_1 of pair v
+  std::vector<uint32_t> h_meta2;          // [nblocks][Cpad/8][G][5 entries of 4 words]: {changed bits, any bits, 0, 0}, then 8 16-bit offsets per pair
+  std::vector<int32_t> h_dmin2, h_span2;  // [nblocks][Cpad]: start / span of the staged row (both rows of a pair: those of channel 2v)
   std::vector<int32_t> h_delta;           // [Cpad/2] delta_v
   uint4* d_meta2 = nullptr;
   int32_t *d_dmin2 = nullptr, *d_span2 = nullptr, *d_delta = nullptr;
@@ -158,7 +159,7 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
                          int nblk = 0);
 cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_dev, float* out_dev,
                           cudaStream_t stream);
-// kModeDeltaPair: pre-sum the packed rows of a range into its pair array (reads P, writes P2)
+// kModeDeltaPair: pre-sum the packed rows of a range into its pair rows (reads P, writes P2)
 cudaError_t launch_pairs(const dd_plan* p, const RangePlan& r, cudaStream_t stream);
 inline bool use_pairs(const dd_plan* p, const RangePlan& r) { return p->variant == DD_KERNEL_SUBBAND && r.pair_ok; }
 cudaError_t configure_kernels(const dd_plan* p);  // opt in to the dynamic shared memory sizes

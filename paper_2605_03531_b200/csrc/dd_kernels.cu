@@ -308,7 +308,7 @@ cudaError_t launch_pack(const dd_plan* p, const RangePlan& r, const void* in_dev
 }
 
 // ------------------------------------------------------------------------------------------------
-// DD_KERNEL_SUBBAND: pair rows.  P2[beam][v][2i + p] = P[beam][2v][i] + P[beam][2v+1][i + delta_v + p], lane by lane
+// DD_KERNEL_SUBBAND: pair rows.  P2[beam][2v + p][i] = P[beam][2v][i] + P[beam][2v+1][i + delta_v + p], lane by lane
 // (16-bit lanes: 2 * maxval < 65536, no carry between lanes).  A delay is a shift by whole superwords, so both
 // terms are aligned 16-byte loads.  Thread = 4 consecutive time indices of one pair row: 4 + 5 loads, 8 stores.
 // Elements past the end of the packed row (never needed by a valid output) read as zero.
@@ -332,13 +332,15 @@ __global__ void __launch_bounds__(256) dd_pair_kernel(const uint4* __restrict__ 
     const int64_t k = i0 + d + e;
     b[e] = (k >= 0 && k < Wp) ? __ldg(rb + k) : z;
   }
-  uint4* dst = P2 + ((int64_t)beam * npairs + v) * (2 * Wp) + 2 * i0;
+  uint4* dst0 = P2 + ((int64_t)beam * 2 * npairs + 2 * v) * Wp + i0;  // i0 is a multiple of 4 and Wp of 8: all four in range
+  uint4* dst1 = dst0 + Wp;
+  uint4 a[4];
 #pragma unroll
-  for (int e = 0; e < 4; ++e) {
-    if (i0 + e >= Wp) break;  // Wp is a multiple of 8: never taken, kept for clarity
-    const uint4 a = __ldg(ra + i0 + e);
-    store2(dst + 2 * e, add4(a, b[e]), add4(a, b[e + 1]));
-  }
+  for (int e = 0; e < 4; ++e) a[e] = __ldg(ra + i0 + e);
+  store2(dst0, add4(a[0], b[0]), add4(a[1], b[1]));
+  store2(dst0 + 2, add4(a[2], b[2]), add4(a[3], b[3]));
+  store2(dst1, add4(a[0], b[1]), add4(a[1], b[2]));
+  store2(dst1 + 2, add4(a[2], b[3]), add4(a[3], b[4]));
 }
 
 cudaError_t launch_pairs(const dd_plan* p, const RangePlan& r, cudaStream_t stream) {

@@ -327,49 +327,48 @@ void build_pair_tables(const dd_plan& p, dd::RangePlan& r) {
     if (hi - lo > 1) return;  // a third row would be needed: not this range
     r.h_delta[v] = lo;
   }
-  const size_t nbv = (size_t)r.nblocks * nvc;
-  r.h_dmin2.assign(nbv, 0);
-  r.h_span2.assign(nbv, 0);
+  const size_t nbc = (size_t)r.nblocks * r.Cpad;
+  r.h_dmin2.assign(nbc, 0);
+  r.h_span2.assign(nbc, 0);
   r.Smax2 = 0;
   for (int b = 0; b < r.nblocks; ++b)
     for (int v = 0; v < nvc; ++v) {
       const int j0 = b * r.Dcta;
       const int32_t d0 = pair_delay(p, r, j0, 2 * v) & ~7;
       const int32_t sp = (int32_t)round_up(pair_delay(p, r, j0 + r.Dcta - 1, 2 * v) - d0, 8);
-      r.h_dmin2[(size_t)b * nvc + v] = d0;
-      r.h_span2[(size_t)b * nvc + v] = sp;
+      for (int q = 0; q < 2; ++q) {  // both pre-summed rows of the pair are staged over the span of channel 2v
+        r.h_dmin2[(size_t)b * r.Cpad + 2 * v + q] = d0;
+        r.h_span2[(size_t)b * r.Cpad + 2 * v + q] = sp;
+      }
       r.Smax2 = std::max(r.Smax2, (int)sp);
     }
-  const size_t rowbytes = (size_t)2 * (r.T + r.Smax2) * 16;
-  if ((size_t)r.Cc2 * rowbytes > 65536) return;  // 16-bit byte offsets inside a stage
-  const size_t stage = (r.Cc2 * rowbytes + dd::tiled_meta_bytes(dd::kModeDeltaPair, r.NL, r.Cc2, r.G) + 127) / 128 * 128;
+  const size_t rowbytes = (size_t)(r.T + r.Smax2) * 16;
+  if ((size_t)r.Cc * rowbytes > 65536) return;  // 16-bit byte offsets inside a stage
+  const size_t stage = (r.Cc * rowbytes + dd::tiled_meta_bytes(dd::kModeDeltaPair, r.NL, r.Cc, r.G) + 127) / 128 * 128;
   r.stages2 = (int)std::min<size_t>(6, ((size_t)227 * 1024 - 128 - 512) / stage);
   if (r.stages2 < 2) return;
-  // table: one 16-byte entry per quad of pairs and trial group
-  r.h_meta2.assign((size_t)r.nblocks * (nvc / 4) * r.G * 4, 0);
+  // table: five 16-byte entries per quad of pairs and trial group (dd_tiled.cu stage_pairs)
+  r.h_meta2.assign((size_t)r.nblocks * (nvc / 4) * r.G * 20, 0);
   for (int b = 0; b < r.nblocks; ++b)
     for (int v = 0; v < nvc; ++v) {
-      const int32_t d0 = r.h_dmin2[(size_t)b * nvc + v];
+      const int32_t d0 = r.h_dmin2[(size_t)b * r.Cpad + 2 * v];
       const int q = v % 4;
       for (int g = 0; g < r.G; ++g) {
         const int jg = b * r.Dcta + g * r.RD;
-        uint32_t* e = &r.h_meta2[(((size_t)b * (nvc / 4) + v / 4) * r.G + g) * 4];
+        uint32_t* e = &r.h_meta2[(((size_t)b * (nvc / 4) + v / 4) * r.G + g) * 20];
         auto D = [&](int j) { return pair_delay(p, r, j, 2 * v); };
         auto P = [&](int j) { return pair_delay(p, r, j, 2 * v + 1) - D(j) - r.h_delta[v]; };
-        const uint32_t off = (uint32_t)(v % r.Cc2) * (uint32_t)rowbytes + (uint32_t)((D(jg) - d0) * 2 + P(jg)) * 16u;
-        e[2 + q / 2] |= off << (16 * (q % 2));
-        for (int j = 1; j < r.RD; ++j) {
-          const bool cd = D(jg + j) != D(jg + j - 1), cf = P(jg + j) != P(jg + j - 1);
-          if (cd) e[0] |= 1u << dd::delta_bit(j, q);
-          if (cf) e[1] |= 1u << dd::delta_bit(j, q);
-          if (cd || cf) {  // "some pair of the quad changes at step j": bit 7 of byte j-1 (steps 1..4: word 0, 5..7: word 1)
-            if (j <= 4) e[0] |= 0x80u << (8 * (j - 1));
-            else e[1] |= 0x80u << (8 * (j - 5));
+        for (int j = 0; j < r.RD; ++j) {
+          const uint32_t off = ((uint32_t)((2 * v + P(jg + j)) % r.Cc) * (uint32_t)(r.T + r.Smax2) + (uint32_t)(D(jg + j) - d0)) * 16u;
+          e[4 + 4 * q + j / 2] |= off << (16 * (j % 2));
+          if (j > 0 && (D(jg + j) != D(jg + j - 1) || P(jg + j) != P(jg + j - 1))) {
+            e[0] |= 1u << dd::delta_bit(j, q);
+            e[1] |= 1u << j;  // some pair of the quad changes at this trial step
           }
         }
       }
     }
-  r.ws2_bytes = round_up((int64_t)p.nbeams * nvc * 2 * r.Wp * dd::kSuperwordBytes, 256);
+  r.ws2_bytes = round_up((int64_t)p.nbeams * r.Cpad * r.Wp * dd::kSuperwordBytes, 256);
   // executed adds per beam: one per (trial, sample, pair) + two pre-sums per packed pair-row element
   r.adds_pair = (int64_t)r.ndm * r.nout * (p.nchans + 1) / 2 + (int64_t)2 * ((p.nchans + 1) / 2) * r.ns;
   r.pair_ok = 1;
@@ -832,7 +831,7 @@ int dd_plan_pair_info(const dd_plan_t* p, int32_t r, int32_t* enabled, int32_t* 
   const auto& q = p->ranges[r];
   if (enabled) *enabled = dd::use_pairs(p, q) ? 1 : 0;
   if (pairs_per_stage) *pairs_per_stage = q.Cc2;
-  if (row_superwords) *row_superwords = 2 * (q.T + q.Smax2);
+  if (row_superwords) *row_superwords = q.T + q.Smax2;
   if (npairs) *npairs = q.Cpad / 2;
   return DD_OK;
 }

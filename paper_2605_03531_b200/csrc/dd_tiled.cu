@@ -81,18 +81,16 @@ __device__ __forceinline__ void lds_if_bit(uint4& w, uint32_t& addr, uint32_t m)
       : "r"(m), "n"(1u << BIT));
 }
 
-// pair mode: bit BIT of md = the delay of channel 2v stepped (address += 32: two superwords per time index), bit BIT of
-// mf = the row selector p flipped (address ^= 16); reload in place if either is set
+// pair mode: if bit BIT of m is set (the pair row of this trial differs from the previous trial's: its delay
+// stepped or the other pre-summed row is needed), reload from the byte offset the table gives for this trial
 template <int BIT>
-__device__ __forceinline__ void lds_pair_if(uint4& w, uint32_t& addr, uint32_t md, uint32_t mf) {
+__device__ __forceinline__ void lds_pair_if(uint4& w, uint32_t sdata, uint32_t off, uint32_t m) {
   asm volatile(
-      "{\n .reg .pred p, q, r;\n .reg .b32 t;\n and.b32 t, %5, %7;\n setp.ne.u32 p, t, 0;\n"
-      " and.b32 t, %6, %7;\n setp.ne.u32 q, t, 0;\n or.pred r, p, q;\n"
-      " @p add.u32 %4, %4, 32;\n"
-      " @q xor.b32 %4, %4, 16;\n"
-      " @r ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n}"
-      : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w), "+r"(addr)
-      : "r"(md), "r"(mf), "n"(1u << BIT));
+      "{\n .reg .pred p;\n .reg .b32 t;\n and.b32 t, %6, %7;\n setp.ne.u32 p, t, 0;\n"
+      " add.u32 t, %4, %5;\n"
+      " @p ld.shared.v4.u32 {%0,%1,%2,%3}, [t];\n}"
+      : "+r"(w.x), "+r"(w.y), "+r"(w.z), "+r"(w.w)
+      : "r"(sdata), "r"(off), "r"(m), "n"(1u << BIT));
 }
 
 __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4& b) {
@@ -114,7 +112,6 @@ struct TiledParams {
   int rowpitch;      // superwords per staged row = T + Smax
   int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
   float accum_scale;  // 0: store; else out = value * accum_scale + out (high byte plane of uint16 input)
-  int wmul;           // superwords per time index in the packed rows: 1, or 2 for the interleaved pair rows (kModeDeltaPair)
 };
 
 __host__ __device__ inline size_t tiled_stage_bytes(int mode, int NL, int Cc, int rowpitch, int G) {
@@ -259,47 +256,48 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
   }
 }
 
-// pair mode (kModeDeltaPair): rows are two-channel sub-bands, quads A..D of them; one table entry per quad =
-//   {delay-step bits | any(1..4) in bit 7 of each byte, flip bits | any(5..7), offA | offB<<16, offC | offD<<16}
+// pair mode (kModeDeltaPair): the packed array holds, per pair v of channels, the two pre-summed rows U_0, U_1 (rows
+// 2v, 2v+1).  Per quad A..D of pairs and trial group the table has five 16-byte entries:
+//   {changed bits (delta_bit layout), any bits (bit j: some pair of the quad changes at trial step j), 0, 0}
+//   then for each pair of the quad eight 16-bit byte offsets (inside the stage, row and U_p selection included), one
+//   per trial.  A trial whose bit is clear reuses the registers of the previous trial.
 template <int J>
-__device__ __forceinline__ void pair_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t& aa,
-                                           uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bd, uint32_t bf, uint32_t u0,
-                                           uint32_t u1) {
+__device__ __forceinline__ void pair_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint32_t sdata,
+                                           const uint4& oa, const uint4& ob, const uint4& oc, const uint4& od, uint32_t bits,
+                                           uint32_t any) {
   if constexpr (J < kRD) {
-    constexpr uint32_t anymask = J <= 4 ? (0x80u << (8 * (J - 1))) : (0x80u << (8 * (J - 5)));
-    if ((J <= 4 ? u0 : u1) & anymask) {  // uniform: some pair of the quad changes at this trial step
-      lds_pair_if<delta_bit(J, 0)>(wa, aa, bd, bf);
-      lds_pair_if<delta_bit(J, 1)>(wb, ab, bd, bf);
-      lds_pair_if<delta_bit(J, 2)>(wc, ac, bd, bf);
-      lds_pair_if<delta_bit(J, 3)>(wd, ad, bd, bf);
+    if (any & (1u << J)) {  // uniform (stage_pairs)
+      lds_pair_if<delta_bit(J, 0)>(wa, sdata, off16(oa, J), bits);
+      lds_pair_if<delta_bit(J, 1)>(wb, sdata, off16(ob, J), bits);
+      lds_pair_if<delta_bit(J, 2)>(wc, sdata, off16(oc, J), bits);
+      lds_pair_if<delta_bit(J, 3)>(wd, sdata, off16(od, J), bits);
     }
     add_pair(acc[J], wa, wb);
     add_pair(acc[J], wc, wd);
-    pair_steps<J + 1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bd, bf, u0, u1);
+    pair_steps<J + 1>(acc, wa, wb, wc, wd, sdata, oa, ob, oc, od, bits, any);
   }
 }
 
 __device__ __forceinline__ void stage_pairs(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {
-  uint4 m;
-  lds_sw(m, smeta);
+  // Cc = rows of the stage = 2 per pair; a quad of pairs = 8 rows
 #pragma unroll 1
-  for (int cc = 0; cc < Cc; cc += 4) {
-    uint32_t aa = sdata + (m.z & 0xffffu);
-    uint32_t ab = sdata + (m.z >> 16);
-    uint32_t ac = sdata + (m.w & 0xffffu);
-    uint32_t ad = sdata + (m.w >> 16);
-    const uint32_t bd = m.x, bf = m.y;
-    const uint32_t u0 = __reduce_or_sync(0xffffffffu, m.x), u1 = __reduce_or_sync(0xffffffffu, m.y);
-    uint4 wa, wb, wc, wd;
-    lds_sw(wa, aa);
-    lds_sw(wb, ab);
-    lds_sw(wc, ac);
-    lds_sw(wd, ad);
+  for (int cc = 0; cc < Cc; cc += 8) {
+    uint4 m, oa, ob, oc, od;
+    lds_sw(m, smeta);
+    lds_sw(oa, smeta + 16);
+    lds_sw(ob, smeta + 32);
+    lds_sw(oc, smeta + 48);
+    lds_sw(od, smeta + 64);
     smeta += meta_row;
-    lds_sw(m, smeta);  // next quad's entry (see stage_delta)
+    const uint32_t any = __reduce_or_sync(0xffffffffu, m.y);
+    uint4 wa, wb, wc, wd;
+    lds_sw(wa, sdata + off16(oa, 0));
+    lds_sw(wb, sdata + off16(ob, 0));
+    lds_sw(wc, sdata + off16(oc, 0));
+    lds_sw(wd, sdata + off16(od, 0));
     add_pair(acc[0], wa, wb);
     add_pair(acc[0], wc, wd);
-    pair_steps<1>(acc, wa, wb, wc, wd, aa, ab, ac, ad, bd, bf, u0, u1);
+    pair_steps<1>(acc, wa, wb, wc, wd, sdata, oa, ob, oc, od, m.x, any);
   }
 }
 
@@ -484,7 +482,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   // byte count.  A warp issues chunk k when it starts iteration k - ahead (ahead = nstages - 2): the
   // stage it refills was consumed two iterations ago, so the wait on its empty barrier is normally
   // already satisfied.  Row start and length of the warp's NEXT chunk are fetched one turn early.
-  const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T * p.wmul;
+  const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T;
   const long long tab = (long long)blk * p.Cpad;
   const char* meta_blk = reinterpret_cast<const char*>(p.meta) + (size_t)blk * (size_t)nchunks * meta_bytes;
   const int lane = tid & 31;
@@ -497,8 +495,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     pf_bytes = 0;
     if (k < nchunks && lane < p.Cc) {
       const int c = k * p.Cc + lane;
-      pf_d0 = __ldg(p.dmin + tab + c) * p.wmul;
-      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes * p.wmul;
+      pf_d0 = __ldg(p.dmin + tab + c);
+      pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
     }
   };
   // stage and wrap count of a chunk index are tracked incrementally (no divisions in the main loop)
@@ -545,8 +543,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const int ti = tid - g * p.T;  // superword inside the time tile
   Lanes<NL> lanes;
   lanes.init();
-  const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes * p.wmul;
-  const uint32_t entry_bytes = 16u;  // table bytes per (channel | quad, trial group)
+  const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
+  const uint32_t entry_bytes = MODE == kModeDeltaPair ? 80u : 16u;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
   const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
@@ -640,27 +638,26 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.meta = pairs ? r.d_meta2 : r.d_meta;
   tp.dmin = pairs ? r.d_dmin2 : r.d_dmin;
   tp.span = pairs ? r.d_span2 : r.d_span;
-  tp.wmul = pairs ? 2 : 1;
   tp.out = out_dev + r.offset;
   tp.out_beam_stride = p->beam_stride;
   tp.pitch = r.pitch;
-  tp.Wp = pairs ? 2 * r.Wp : r.Wp;
+  tp.Wp = r.Wp;
   tp.H = r.H;
   tp.nout = r.nout;
   tp.ntau = r.ntau;
   tp.ndm = r.ndm;
-  tp.Cpad = pairs ? r.Cpad / 2 : r.Cpad;  // rows of the packed array the kernel walks (pairs: sub-band rows)
+  tp.Cpad = r.Cpad;  // rows of the packed array the kernel walks (pairs: the two pre-summed rows of each pair)
   tp.G = r.G;
   tp.T = r.T;
-  tp.Cc = pairs ? r.Cc2 : r.Cc;
+  tp.Cc = r.Cc;
   tp.nstages = pairs ? r.stages2 : r.stages;
   tp.blk0 = blk0;
   tp.nblk = nblk;
-  tp.rowpitch = pairs ? 2 * (r.T + r.Smax2) : r.T + r.Smax;
-  tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;  // pairs: flush/2 sub-band rows = the same number of stages
+  tp.rowpitch = pairs ? r.T + r.Smax2 : r.T + r.Smax;
+  tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;  // pairs: a stage holds Cc/2 pair sums of twice the size: same interval
   const long long nctas = (long long)nblk * r.ntau * p->nbeams;
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  const size_t smem = pairs ? kBarRegion + (size_t)r.stages2 * tiled_stage_bytes(kModeDeltaPair, r.NL, r.Cc2, tp.rowpitch, r.G) + 512
+  const size_t smem = pairs ? kBarRegion + (size_t)r.stages2 * tiled_stage_bytes(kModeDeltaPair, r.NL, r.Cc, tp.rowpitch, r.G) + 512
                             : tiled_smem_bytes(r);
   const int nt = r.G * r.T;
   const int mode = pairs ? (int)kModeDeltaPair

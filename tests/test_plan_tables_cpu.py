@@ -206,43 +206,41 @@ def test_tuned_plan_goes_through_the_same_checks():
 
 
 def _decode_pairs(plan, r):
-    """DD_KERNEL_SUBBAND tables -> delays of both channels of every pair row: [nblocks*Dcta][Cpad]."""
+    """DD_KERNEL_SUBBAND tables -> delays of both channels of every pair: [nblocks*Dcta][Cpad]."""
     info, shape, pi = plan.tile_info(r), plan.tile_shape(r), plan.pair_info(r)
-    g, cpad, nb = shape["trial_groups"], shape["cpad"], shape["nblocks"]
-    nvc, cc2, rowsw = pi["npairs"], pi["pairs_per_stage"], pi["row_superwords"]
-    assert nvc == cpad // 2 and cc2 * 2 == shape["chans_per_stage"]
-    e = plan.table(r, 3).reshape(nb, nvc // 4, g, 4).astype(np.int64)
-    dmin = plan.table(r, 4).astype(np.int64).reshape(nb, nvc)
-    span = plan.table(r, 5).astype(np.int64).reshape(nb, nvc)
+    g, cpad, nb, cc = shape["trial_groups"], shape["cpad"], shape["nblocks"], shape["chans_per_stage"]
+    nvc, rowsw = pi["npairs"], pi["row_superwords"]
+    assert nvc == cpad // 2 and pi["pairs_per_stage"] * 2 == cc
+    e = plan.table(r, 3).reshape(nb, nvc // 4, g, 20).astype(np.int64)
+    dmin = plan.table(r, 4).astype(np.int64).reshape(nb, cpad)
+    span = plan.table(r, 5).astype(np.int64).reshape(nb, cpad)
     delta = plan.table(r, 6).astype(np.int64)
-    assert (dmin % 8 == 0).all() and (span % 8 == 0).all() and (2 * (span + info["words_per_cta"]) <= rowsw).all()
+    assert (dmin % 8 == 0).all() and (span % 8 == 0).all() and (span + info["words_per_cta"] <= rowsw).all()
+    assert np.array_equal(dmin[:, 0::2], dmin[:, 1::2]) and np.array_equal(span[:, 0::2], span[:, 1::2])
     out = np.zeros((nb, g, 8, cpad), dtype=np.int64)
     anyb = np.zeros((nb, nvc // 4, g), dtype=np.int64)
+    assert (e[..., 2:4] == 0).all()
     for q in range(4):
-        field = (e[..., 2 + q // 2] >> (16 * (q % 2))) & 0xFFFF                  # [nb][quad][g] byte offset in the stage
-        assert (field % 16 == 0).all()
-        vrow = (np.arange(q, nvc, 4) % cc2) * rowsw                                # superwords, row of the pair in its stage
-        rel = field // 16 - vrow[None, :, None]
-        assert (rel >= 0).all()
-        D = rel // 2 + dmin[:, q::4][:, :, None]
-        P = rel % 2
+        v = np.arange(q, nvc, 4)                                                    # the pairs in position q of their quad
+        prev = None
         for j in range(8):
+            off = (e[..., 4 + 4 * q + j // 2] >> (16 * (j % 2))) & 0xFFFF             # [nb][quad][g] byte offset in the stage
+            assert (off % 16 == 0).all()
+            sw = off // 16
+            row, rel = sw // rowsw, sw % rowsw                                       # row inside the stage, superword inside the row
+            pbit = row - ((2 * v) % cc)[None, :, None]                               # which pre-summed row: U_0 or U_1
+            assert ((pbit == 0) | (pbit == 1)).all()
+            assert (rel <= span[:, 2 * v][:, :, None]).all(), "loads stay inside the staged row"
+            D = rel + dmin[:, 2 * v][:, :, None]
             if j > 0:
                 n = (j - 1) * 4 + q
-                bit = 1 << ((n // 7) * 8 + n % 7)
-                cd = (e[..., 0] & bit) != 0
-                cf = (e[..., 1] & bit) != 0
-                anyb |= (cd | cf).astype(np.int64) << j
-                D = D + cd
-                P = P ^ cf
-            assert (D - dmin[:, q::4][:, :, None] <= span[:, q::4][:, :, None]).all(), "loads stay inside the staged row"
+                chg = (e[..., 0] >> ((n // 7) * 8 + n % 7)) & 1
+                assert np.array_equal(chg, (off != prev).astype(np.int64)), "changed bit <=> the offset differs from the previous trial's"
+                anyb |= chg << j
+            prev = off
             out[:, :, j, 2 * q::8] = D.transpose(0, 2, 1)
-            out[:, :, j, 2 * q + 1::8] = (D + delta[None, q::4, None] + P).transpose(0, 2, 1)
-    stored = np.zeros_like(anyb)
-    for j in range(1, 8):
-        word, byte = (0, j - 1) if j <= 4 else (1, j - 5)
-        stored |= ((e[..., word] >> (8 * byte + 7)) & 1) << j
-    assert np.array_equal(stored, anyb), "any-changed bits (bit 7 of each table byte) are the OR of the quad's bits"
+            out[:, :, j, 2 * q + 1::8] = (D + delta[None, v, None] + pbit).transpose(0, 2, 1)
+    assert np.array_equal(anyb, e[..., 1]), "any bits are the OR of the quad's changed bits"
     return out.reshape(nb * g * 8, cpad)
 
 
@@ -275,8 +273,9 @@ def test_pair_tables_reproduce_the_delay_table(cfg, nchans):
         assert np.array_equal(got[:, : w.nchans], want[rows]), (cfg, r)
         if w.nchans % 2:                                     # the pad partner of the last channel copies its delay
             assert np.array_equal(got[:, w.nchans], want[rows][:, -1])
-        stage = -(-(pi["pairs_per_stage"] * pi["row_superwords"] * 16 + pi["pairs_per_stage"] // 4 * shape["trial_groups"] * 16) // 128) * 128
-        assert pi["pairs_per_stage"] * pi["row_superwords"] * 16 <= 65536 and 128 + 2 * stage + 512 <= 227 * 1024
+        rows = shape["chans_per_stage"]
+        stage = -(-(rows * pi["row_superwords"] * 16 + rows // 8 * shape["trial_groups"] * 80) // 128) * 128
+        assert rows * pi["row_superwords"] * 16 <= 65536 and 128 + 2 * stage + 512 <= 227 * 1024
     brute = plan.work()[1]
     assert plan.executed_adds() < 0.52 * brute if cfg == 3 and nchans == 4096 else plan.executed_adds() <= brute
     plan.set_kernel(B.DD_KERNEL_TILED)
