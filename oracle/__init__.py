@@ -20,4 +20,5 @@ from .oracle import (  # noqa: F401
     resample_edges,
     running_median,
     sps,
+    sps_candidates,
 )

@@ -169,6 +169,28 @@ def sps(rows: np.ndarray, n: int, nwidths: int, threshold: float):
     return {"snr": snr, "tmax": tmax, "count": count, "mean": mean, "sigma": sigma}
 
 
+def sps_candidates(rows: np.ndarray, n: int, nwidths: int, threshold: float, cap: int = 1 << 20):
+    """The candidate list of the boxcar search (oracle_sps.c): structured array of (row, k, t, snr)
+    ordered by row, k, t, and the total count (which may exceed `cap`)."""
+    sps(rows[:1], n, 1, 0.0)  # loads the library
+    lib = _lib_sps
+    vp, i64 = ctypes.c_void_p, ctypes.c_int64
+    lib.oracle_sps_candidates.argtypes = [vp, i64, i64, i64, ctypes.c_int, ctypes.c_double, vp, vp, vp, vp, i64, vp]
+    lib.oracle_sps_candidates.restype = ctypes.c_int
+    rows = np.ascontiguousarray(rows)
+    nrows, pitch = rows.shape
+    cr, ck, ct = (np.empty(cap, dtype=np.int32) for _ in range(3))
+    cs = np.empty(cap, dtype=np.float32)
+    total = ctypes.c_int64()
+    rc = lib.oracle_sps_candidates(_ptr(rows), nrows, pitch, n, nwidths, float(threshold), _ptr(cr), _ptr(ck), _ptr(ct),
+                                   _ptr(cs), cap, ctypes.byref(total))
+    _check(rc, "sps_candidates")
+    m = min(cap, total.value)
+    out = np.empty(m, dtype=[("row", np.int32), ("k", np.int32), ("t", np.int32), ("snr", np.float32)])
+    out["row"], out["k"], out["t"], out["snr"] = cr[:m], ck[:m], ct[:m], cs[:m]
+    return out, total.value
+
+
 # ---- pulsar-side post-processing of dedispersed series (oracle_post.c; PAPER.md:421, :425, :441-484) ----------------
 def _post():
     global _lib_post

@@ -21,6 +21,11 @@
  * No FMA contraction (compile with -ffp-contract=off), so a device implementation that uses the same
  * round-to-nearest operations in the same order gets the same bits.
  *
+ * "The list of candidates thus generated is filtered ..." -- the search hands a LIST on to the next
+ * stage.  Reading B5: the list holds every (row, width index k, t) with B[t] > thr, each with
+ * snr = (float)((B[t] - w*mean)/den) (0 when sigma = 0), ordered by row, then k, then t.  Its length per (row, k) is the
+ * count above.  oracle_sps_candidates writes it (first `cap` entries) and returns the total through *total.
+ *
  * Pins (tests/test_oracle_sps_pins.py): constant row, single impulse and boxcar pulse closed forms, a linear
  * ramp's mean and variance, count limits for extreme thresholds, a pure-Python brute force on random rows,
  * invariance of tmax under a constant offset.
@@ -81,4 +86,48 @@ int oracle_sps(const float* rows, int64_t nrows, int64_t pitch, int64_t n, int K
     }
   }
   return rc;
+}
+
+/* The candidate list (reading B5): entries (row, k, t, snr) in the order row, k, t.  cand_* hold `cap` entries; *total =
+ * number of candidates found (may exceed cap: the rest is counted, not written). */
+int oracle_sps_candidates(const float* rows, int64_t nrows, int64_t pitch, int64_t n, int K, double threshold,
+                          int32_t* cand_row, int32_t* cand_k, int32_t* cand_t, float* cand_snr, int64_t cap, int64_t* total) {
+  if (!rows || !total || nrows < 0 || n < 1 || pitch < n || K < 1 || K > 20 || cap < 0) return ORACLE_ERR_INVALID;
+  if (cap > 0 && (!cand_row || !cand_k || !cand_t || !cand_snr)) return ORACLE_ERR_INVALID;
+  int64_t nc = 0;
+  for (int64_t r = 0; r < nrows; ++r) {
+    const float* x = rows + r * pitch;
+    uint64_t s1 = 0, s2 = 0;
+    for (int64_t t = 0; t < n; ++t) {
+      const uint64_t v = (uint64_t)x[t];
+      s1 += v;
+      s2 += v * v;
+    }
+    const double mean = (double)s1 / (double)n;
+    double var = (double)s2 / (double)n - mean * mean;
+    if (var < 0.0) var = 0.0;
+    const double sigma = sqrt(var);
+    for (int k = 0; k < K; ++k) {
+      const int64_t w = (int64_t)1 << k;
+      if (w > n) continue;
+      const double den = sigma * sqrt((double)w);
+      const double wmean = (double)w * mean;
+      const double thr = wmean + threshold * den;
+      for (int64_t t = 0; t + w <= n; ++t) {
+        uint64_t b = 0;
+        for (int64_t i = 0; i < w; ++i) b += (uint64_t)x[t + i]; /* the boxcar by its definition */
+        if ((double)b > thr) {
+          if (nc < cap) {
+            cand_row[nc] = (int32_t)r;
+            cand_k[nc] = k;
+            cand_t[nc] = (int32_t)t;
+            cand_snr[nc] = sigma > 0.0 ? (float)(((double)b - wmean) / den) : 0.0f;
+          }
+          ++nc;
+        }
+      }
+    }
+  }
+  *total = nc;
+  return ORACLE_OK;
 }

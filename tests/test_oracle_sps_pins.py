@@ -114,3 +114,67 @@ def test_offset_invariance_of_position_and_near_invariance_of_snr():
     b = oracle.sps((x + 1000)[None, :], n, 8, 3.0)
     assert np.array_equal(a["tmax"], b["tmax"]) and np.array_equal(a["count"], b["count"])
     assert np.allclose(a["snr"], b["snr"], rtol=1e-5)
+
+
+# ---- the candidate list ("The list of candidates thus generated is filtered ...") ---------------------
+def test_candidate_list_single_impulse_closed_form():
+    """One impulse of height h at t0 over a constant level c: for width w the windows that contain it are
+    t0-w+1 .. t0, each with B = w*c + h and snr = (B - w*mean)/(sigma*sqrt(w)); they are the only candidates and come
+    in the order (row, width index, t)."""
+    n, c, h, t0, K, thr = 2000, 50.0, 400.0, 700, 6, 4.0
+    x = np.full(n, c, dtype=np.float32)
+    x[t0] += h
+    mean = (n * c + h) / n
+    sigma = math.sqrt((((n - 1) * c * c + (c + h) ** 2) / n) - mean * mean)
+    cand, total = oracle.sps_candidates(x[None, :], n, K, thr)
+    want = []
+    for k in range(K):
+        w = 2 ** k
+        snr = (w * c + h - w * mean) / (sigma * math.sqrt(w))
+        if snr > thr:
+            want += [(0, k, t, snr) for t in range(t0 - w + 1, t0 + 1)]
+    assert total == len(want) == len(cand) and total > 0
+    assert [(int(a["row"]), int(a["k"]), int(a["t"])) for a in cand] == [(r, k, t) for r, k, t, _ in want]
+    assert np.allclose(cand["snr"], [s for *_, s in want], rtol=1e-6, atol=0)
+
+
+def test_candidate_list_agrees_with_counts_order_and_brute_force():
+    rng = np.random.default_rng(99)
+    rows = rng.integers(900, 1100, size=(5, 700)).astype(np.float32)
+    rows[1, 100:108] += 300.0
+    rows[3, 650:700] += 120.0
+    rows[4, :] = 1000.0                      # sigma = 0: nothing can exceed the mean
+    K, thr = 7, 3.5
+    res = oracle.sps(rows, 700, K, thr)
+    cand, total = oracle.sps_candidates(rows, 700, K, thr)
+    assert total == len(cand) == int(res["count"].sum()) and total > 20
+    key = cand["row"].astype(np.int64) * 10 ** 9 + cand["k"].astype(np.int64) * 10 ** 6 + cand["t"]
+    assert (np.diff(key) > 0).all()          # strictly increasing in (row, k, t)
+    for r in range(5):                       # count per (row, k) == list length per (row, k)
+        for k in range(K):
+            assert int(((cand["row"] == r) & (cand["k"] == k)).sum()) == res["count"][r, k]
+    # brute force in Python doubles: same membership, snr compared as float32 bits
+    for r in (1, 3):
+        x = [float(v) for v in rows[r]]
+        n = len(x)
+        mean = sum(x) / n
+        var = sum(v * v for v in x) / n - mean * mean
+        sigma = math.sqrt(max(var, 0.0))
+        mine = []
+        for k in range(K):
+            w = 2 ** k
+            den = sigma * math.sqrt(w)
+            for t in range(n - w + 1):
+                b = sum(x[t:t + w])
+                if b > w * mean + thr * den:
+                    mine.append((k, t, np.float32((b - w * mean) / den)))
+        got = cand[cand["row"] == r]
+        assert [(int(a["k"]), int(a["t"])) for a in got] == [(k, t) for k, t, _ in mine]
+        assert np.array_equal(got["snr"].view(np.uint32), np.array([s for *_, s in mine], dtype=np.float32).view(np.uint32))
+    # the best candidate of a (row, k) is the snr / tmax the search reports
+    for r, k in ((1, 3), (3, 5)):
+        sel = cand[(cand["row"] == r) & (cand["k"] == k)]
+        assert sel["snr"].max() == res["snr"][r, k] and int(sel["t"][np.argmax(sel["snr"])]) == res["tmax"][r, k]
+    # a capacity below the total truncates the list but still reports the total
+    few, total2 = oracle.sps_candidates(rows, 700, K, thr, cap=10)
+    assert total2 == total and len(few) == 10 and np.array_equal(few, cand[:10])
