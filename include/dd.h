@@ -282,10 +282,35 @@ int dd_stream_destroy(dd_stream_t* s);
  *     rows*nwidths elements ([row][k]); 1 <= nwidths <= 12; threshold finite.  Enqueues one kernel per range on
  *     `cuda_stream`.  DD_ERR_OVERFLOW if (nchans*(2^in_bits-1)*decim)^2 * nout_r >= 2^63 for some range (sum x^2
  *     would not be exact; uint8 SPOTLIGHT-shaped data is far below).
+ *
+ * The candidate list ("The list of candidates thus generated is filtered ..."): every (row, k, t) with
+ * B[t] > w*mean + threshold*sigma*sqrt(w), with snr = (float)((B[t] - w*mean)/(sigma*sqrt(w))), ordered by row, then k,
+ * then t.  dd_sps_candidates: after dd_sps_execute on the same plane with the same nwidths and threshold, count_dev as
+ *     written by it.  Writes offsets_dev[rows*nwidths + 1] (int64) = exclusive scan of the counts -- the candidates of
+ *     (row, k) are entries offsets[row*nwidths + k] .. offsets[row*nwidths + k + 1] of the list, the last element is the
+ *     total -- and the first max_cands candidates to cand_dev.  Two small kernels plus one CTA per row that leaves at
+ *     once when the row has no candidate; rows with candidates redo their boxcars.
+ *
+ * Row statistics from the dedispersion epilogue: dd_plan_set_row_stats(plan, stats_dev) with stats_dev = rows*2
+ *     uint64 (caller-owned device memory, 8-byte aligned; NULL switches it off; uint8 input only).  From then on
+ *     dd_execute zeroes stats_dev and its dedispersion kernels add sum x and sum x^2 of every row they write (exact
+ *     integers), and dd_sps_execute / dd_sps_candidates take S1, S2 from there instead of reading the plane a first
+ *     time: the plane is then read ONCE.  The plane handed to them must be the one the last dd_execute of this plan
+ *     wrote.  (dd_execute_host does not accumulate statistics.)
  */
+typedef struct dd_sps_cand {
+  int32_t row;         /* as in dd_sps_rows */
+  int32_t width_log2;  /* k: boxcar width 2^k */
+  int32_t t;           /* first sample of the window */
+  float snr;
+} dd_sps_cand_t;
 int dd_sps_rows(const dd_plan_t* plan, int64_t* rows);
 int dd_sps_execute(const dd_plan_t* plan, const float* plane_dev, int32_t nwidths, double threshold, float* snr_dev,
                    int32_t* tmax_dev, int32_t* count_dev, void* cuda_stream);
+int dd_sps_candidates(const dd_plan_t* plan, const float* plane_dev, int32_t nwidths, double threshold,
+                      const int32_t* count_dev, int64_t* offsets_dev, dd_sps_cand_t* cand_dev, int64_t max_cands,
+                      void* cuda_stream);
+int dd_plan_set_row_stats(dd_plan_t* plan, uint64_t* stats_dev);
 
 /* ---- pulsar-side post-processing of dedispersed series ------------------------------ */
 

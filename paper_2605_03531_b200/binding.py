@@ -24,7 +24,7 @@ SYMBOLS = [
     "dd_plan_executed_adds", "dd_plan_pair_info",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
     "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_create_tuned", "dd_plan_tile_shape", "dd_plan_table",
-    "dd_sps_rows", "dd_sps_execute", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
+    "dd_sps_rows", "dd_sps_execute", "dd_sps_candidates", "dd_plan_set_row_stats", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
     "dd_post_downsample", "dd_post_dered", "dd_resample_create", "dd_resample_create_host", "dd_resample_info",
     "dd_resample_get_edges", "dd_resample_execute", "dd_resample_destroy",
@@ -91,6 +91,8 @@ def _load():
         lib.dd_plan_create_tuned.argtypes = [P(dd_config_t), P(dd_tuning_t), i32, P(vp)]
         lib.dd_sps_rows.argtypes = [vp, P(ctypes.c_int64)]
         lib.dd_sps_execute.argtypes = [vp, vp, i32, ctypes.c_double, vp, vp, vp, vp]
+        lib.dd_sps_candidates.argtypes = [vp, vp, i32, ctypes.c_double, vp, vp, vp, i64, vp]
+        lib.dd_plan_set_row_stats.argtypes = [vp, vp]
         lib.dd_stream_create.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_stream_push.argtypes = [vp, vp, vp, vp]
         lib.dd_stream_plan.argtypes = [vp]
@@ -308,6 +310,20 @@ class Plan:
         ptr = lambda a: a if isinstance(a, int) else a.data_ptr()  # noqa: E731
         _chk(_load().dd_sps_execute(self._h, ptr(plane_dev), int(nwidths), float(threshold), ptr(snr_dev), ptr(tmax_dev),
                                     ptr(count_dev), _stream_ptr(stream)), "dd_sps_execute")
+
+    def sps_candidates(self, plane_dev, nwidths: int, threshold: float, count_dev, offsets_dev, cand_dev, max_cands: int,
+                       stream=None) -> None:
+        """offsets_dev: int64 [rows*nwidths + 1]; cand_dev: max_cands entries of dd_sps_cand_t (16 bytes each:
+        int32 row, int32 width_log2, int32 t, float32 snr), e.g. an int32 tensor [max_cands][4]."""
+        ptr = lambda a: None if a is None else (a if isinstance(a, int) else a.data_ptr())  # noqa: E731
+        _chk(_load().dd_sps_candidates(self._h, ptr(plane_dev), int(nwidths), float(threshold), ptr(count_dev),
+                                       ptr(offsets_dev), ptr(cand_dev), int(max_cands), _stream_ptr(stream)), "dd_sps_candidates")
+
+    def set_row_stats(self, stats_dev) -> None:
+        """stats_dev: int64 CUDA tensor of sps_rows()*2 elements (or None to switch the epilogue statistics off)."""
+        ptr = None if stats_dev is None else (stats_dev if isinstance(stats_dev, int) else stats_dev.data_ptr())
+        _chk(_load().dd_plan_set_row_stats(self._h, ptr), "dd_plan_set_row_stats")
+        self._stats_ref = stats_dev
 
     def set_profiling(self, max_executes: int) -> None:
         _chk(_load().dd_plan_set_profiling(self._h, int(max_executes)), "dd_plan_set_profiling")

@@ -67,6 +67,7 @@ struct RangePlan {
   double dm_lo = 0, dm_step = 0;
   int ndm = 0, decim = 1;
   int64_t ns = 0, maxd = 0, nout = 0, pitch = 0, offset = 0;
+  int64_t row0 = 0;    // index of this range's first trial among the rows of one beam (sum of ndm of earlier ranges)
   int64_t in_off = 0;  // first input sample this range reads (0 unless the plan keeps only the tail: dd_plan_create_tail)
   std::vector<int32_t> delays;  // host copy [ndm][nchans]
   // tiled kernel shape
@@ -126,6 +127,10 @@ struct dd_plan {
   std::vector<dd::RangePlan> ranges;
   int64_t beam_stride = 0, out_elems = 0;
   int64_t dm_samples = 0, adds = 0;
+  int64_t rows_per_beam = 0;  // sum of ndm over the ranges
+  // dd_plan_set_row_stats: [nbeams*rows_per_beam][2] = sum x, sum x^2 of every DM-time row, accumulated by the
+  // epilogue of the dedispersion kernels (caller-owned device memory; nullptr = off)
+  unsigned long long* row_stats = nullptr;
   int device = 0;
   int variant = DD_KERNEL_AUTO;
   // workspace

@@ -360,19 +360,34 @@ __global__ void __launch_bounds__(256) dd_direct_kernel(const Tin* __restrict__ 
                                                         float* __restrict__ out, int nchans, long long nsamps, int decim,
                                                         long long nout, long long pitch, long long out_beam_stride,
                                                         long long chan_stride, long long time_stride, int rev,
-                                                        long long off) {
+                                                        long long off, unsigned long long* stats,
+                                                        long long stats_beam_stride) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nout) return;
   const int j = blockIdx.y;
   const int beam = blockIdx.z;
-  const Tin* x = in + (long long)beam * nchans * nsamps;
-  const int32_t* d = delays + (long long)j * nchans;  // internal order: channel 0 = highest frequency
   uint32_t s = 0;
-  for (int c = 0; c < nchans; ++c) {
-    const Tin* src = x + (long long)(rev ? nchans - 1 - c : c) * chan_stride + ((long long)decim * (t + d[c]) + off) * time_stride;
-    for (int q = 0; q < decim; ++q) s += (uint32_t)src[q * time_stride];
+  if (t < nout) {
+    const Tin* x = in + (long long)beam * nchans * nsamps;
+    const int32_t* d = delays + (long long)j * nchans;  // internal order: channel 0 = highest frequency
+    for (int c = 0; c < nchans; ++c) {
+      const Tin* src = x + (long long)(rev ? nchans - 1 - c : c) * chan_stride + ((long long)decim * (t + d[c]) + off) * time_stride;
+      for (int q = 0; q < decim; ++q) s += (uint32_t)src[q * time_stride];
+    }
+    out[(long long)beam * out_beam_stride + (long long)j * pitch + t] = __uint2float_rn(s);
   }
-  out[(long long)beam * out_beam_stride + (long long)j * pitch + t] = __uint2float_rn(s);
+  if (stats) {  // row statistics for the single-pulse search (dd_plan_set_row_stats): one pair of atomics per warp
+    unsigned long long s1 = t < nout ? s : 0, s2 = t < nout ? (unsigned long long)s * s : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      s1 += __shfl_down_sync(0xffffffffu, s1, o);
+      s2 += __shfl_down_sync(0xffffffffu, s2, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      unsigned long long* st = stats + (long long)beam * stats_beam_stride + 2ll * j;
+      atomicAdd(st, s1);
+      atomicAdd(st + 1, s2);
+    }
+  }
 }
 
 cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_dev, float* out_dev,
@@ -381,14 +396,16 @@ cudaError_t launch_direct(const dd_plan* p, const RangePlan& r, const void* in_d
   dim3 grid((unsigned)((r.nout + 255) / 256), (unsigned)r.ndm, (unsigned)p->nbeams);
   const bool tc = p->layout == DD_LAYOUT_SPECTRUM_MAJOR;
   const long long cs = tc ? 1 : p->nsamps, ts = tc ? p->nchans : 1;
+  unsigned long long* stats = p->row_stats ? p->row_stats + 2 * r.row0 : nullptr;
   if (p->in_bits == 8) {
     dd_direct_kernel<uint8_t><<<grid, block, 0, stream>>>(static_cast<const uint8_t*>(in_dev), r.d_delays,
                                                           out_dev + r.offset, p->nchans, p->nsamps, r.decim, r.nout,
-                                                          r.pitch, p->beam_stride, cs, ts, p->ascending, r.in_off);
+                                                          r.pitch, p->beam_stride, cs, ts, p->ascending, r.in_off, stats,
+                                                          2 * p->rows_per_beam);
   } else {
     dd_direct_kernel<uint16_t><<<grid, block, 0, stream>>>(static_cast<const uint16_t*>(in_dev), r.d_delays,
                                                            out_dev + r.offset, p->nchans, p->nsamps, r.decim, r.nout,
-                                                           r.pitch, p->beam_stride, cs, ts, p->ascending, r.in_off);
+                                                           r.pitch, p->beam_stride, cs, ts, p->ascending, r.in_off, nullptr, 0);
   }
   return cudaGetLastError();
 }

@@ -494,6 +494,8 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_
       if (tail_new > 0 && r.nout < tail_new / r.decim) { rc = DD_ERR_TOO_SHORT; break; }
       r.pitch = round_up(r.nout, 32);
       r.offset = offset;
+      r.row0 = p->rows_per_beam;
+      p->rows_per_beam += r.ndm;
       offset += (int64_t)r.ndm * r.pitch;
       p->dm_samples += (int64_t)p->nbeams * r.ndm * r.nout;
       choose_tile(*p, r, tune ? *tune : kAutoTuning);
@@ -624,6 +626,8 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
     plan->prof_count[slot] = ++nl;
     return e;
   };
+  if (plan->row_stats)  // row statistics for the single-pulse search: the kernels' epilogues add into zeroed sums
+    DD_CUDA(cudaMemsetAsync(plan->row_stats, 0, (size_t)plan->nbeams * plan->rows_per_beam * 2 * sizeof(unsigned long long), stream));
   // a2 for every range first, then a3+a4: the dedispersion kernels of consecutive ranges follow each
   // other on the stream without a pack kernel draining the machine in between.
   for (const auto& r : plan->ranges) {
@@ -855,6 +859,13 @@ int dd_plan_set_workspace(dd_plan_t* p, void* dev, int64_t bytes) {
   }
   if (p->ws && !p->ws_owned) p->ws = nullptr, p->ws_have = 0;
   return ensure_workspace(p);
+}
+
+int dd_plan_set_row_stats(dd_plan_t* p, uint64_t* stats_dev) {
+  if (!p) return DD_ERR_INVALID;
+  if (stats_dev && (p->in_bits != 8 || (reinterpret_cast<uintptr_t>(stats_dev) & 7u))) return DD_ERR_INVALID;
+  p->row_stats = reinterpret_cast<unsigned long long*>(stats_dev);
+  return DD_OK;
 }
 
 int dd_plan_set_kernel(dd_plan_t* p, int32_t variant) {

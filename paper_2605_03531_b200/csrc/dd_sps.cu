@@ -1,17 +1,22 @@
 // dd_sps.cu -- boxcar single-pulse search on the rows of the DM-time plane.
 //
 // PAPER.md:317-325 (section 2.1): "The SPS module searches for statistically significant single pulses above a
-// user-specified threshold using time-domain boxcar filtering."  The readings that make this a definition are
-// DESIGN.md B1-B6; per row x[0..n) (integers held in floats):
+// user-specified threshold using time-domain boxcar filtering.  ...  The list of candidates thus generated is
+// filtered ..."  The readings that make this a definition are DESIGN.md B1-B6; per row x[0..n) (integers in floats):
 //   S1 = sum x, S2 = sum x^2 (exact), mean = S1/n, var = S2/n - mean*mean (>= 0), sigma = sqrt(var)   (IEEE double)
 //   for width w = 2^k: B[t] = sum_{i<w} x[t+i]; best = max B, tmax = first t reaching it;
 //   den = sigma*sqrt(w); snr = sigma > 0 ? (best - w*mean)/den : 0; count = #{t: B[t] > w*mean + threshold*den}
+//   candidate list: every (row, k, t) with B[t] > w*mean + threshold*den and its snr, ordered by row, k, t.
 // Everything up to the few double operations per (row, width) is integer arithmetic, and those use explicit
 // round-to-nearest intrinsics in the stated order (no FMA contraction), so the results are bit-exact.
 //
-// One CTA per row.  Phase A: S1, S2 with vector loads and a block reduction.  Phase B: tiles of kTile samples plus
-// a halo of the widest filter are staged in shared memory with coalesced loads and turned into an exclusive prefix
-// sum P (int64); every boxcar of every width is then P[t+w] - P[t].  The plane is read twice (the second pass mostly from L2): HBM-bound.
+// dd_sps_kernel: one CTA per row.  Phase A: S1, S2 (vector loads, block reduction) -- skipped when dd_execute has
+// already accumulated them in its epilogue (dd_plan_set_row_stats), which leaves ONE pass over the plane.  Phase B:
+// tiles of kSpsTile samples plus a halo of the widest filter are staged in shared memory and turned into a prefix sum
+// P; every boxcar of every width is P[t+w] - P[t], four consecutive samples per thread and step.  Samples above the
+// threshold are rare, so the loop tests the maximum of the four against the threshold and counts one by one only then.
+// dd_sps_fill_kernel: the candidate list.  Rows without a candidate leave at once; the others redo their boxcars and
+// write (row, k, t, snr) in order at the offsets an exclusive scan of the counts has fixed (dd_sps_scan_kernel).
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -34,7 +39,15 @@ struct SpsParams {
   int32_t* tmax;
   int32_t* count;
   long long row0, rows_per_beam;  // output row = beam*rows_per_beam + row0 + trial
+  const unsigned long long* stats;  // [rows][2] = S1, S2 per output row, or nullptr (phase A computes them)
+  // candidate list (dd_sps_fill_kernel)
+  const long long* offsets;  // [rows*K + 1] exclusive scan of count
+  dd_sps_cand_t* cand;
+  long long max_cands;
 };
+
+// dynamic shared memory: P[span + 1] prefix sums, then (16-byte aligned) V[span] samples
+__host__ __device__ inline size_t sps_v_offset(size_t span, size_t acc_bytes) { return ((span + 1) * acc_bytes + 15) / 16 * 16; }
 
 __device__ __forceinline__ unsigned long long shfl_down_u64(unsigned long long v, int o) {
   return __shfl_down_sync(0xffffffffu, v, o);
@@ -49,26 +62,39 @@ __device__ __forceinline__ void load4(const unsigned long long* P, unsigned long
   v[0] = a.x, v[1] = a.y, v[2] = b.x, v[3] = b.y;
 }
 
-// K = number of widths; WIDE = boxcar sums may reach 2^32 (64-bit prefix sums), else 32-bit modular prefix sums
-// (a difference of two of them is the exact boxcar because it is below 2^32).
-template <int K, bool WIDE>
-__global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) {
-  using acc_t = typename std::conditional<WIDE, unsigned long long, uint32_t>::type;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  acc_t* P = reinterpret_cast<acc_t*>(smem_raw);  // [kSpsTile + halo + 1]
-  __shared__ unsigned long long red[2][kSpsThreads / 32];
-  __shared__ unsigned long long s_thr[kSpsMaxK];  // B >= s_thr  <=>  B > w*mean + threshold*den
-  __shared__ double s_wmean[kSpsMaxK], s_den[kSpsMaxK];
-  __shared__ double s_sigma;
-  __shared__ unsigned long long s_best[kSpsMaxK][kSpsThreads / 32];
-  __shared__ int s_tb[kSpsMaxK][kSpsThreads / 32], s_cnt[kSpsMaxK][kSpsThreads / 32];
-  __shared__ unsigned long long s_warp_tot[kSpsThreads / 32];
+// Row statistics and the per-width constants, by one thread, in the operation order of the definition.
+struct SpsRowConsts {
+  unsigned long long thr[kSpsMaxK];  // B >= thr  <=>  B > w*mean + threshold*den   (integer B)
+  double wmean[kSpsMaxK], den[kSpsMaxK];
+  double sigma;
+};
+__device__ __forceinline__ void sps_row_consts(unsigned long long t1, unsigned long long t2, int n, int K, double threshold,
+                                               SpsRowConsts& c) {
+  const double dn = (double)n;
+  const double mean = __ddiv_rn(__ull2double_rn(t1), dn);
+  double var = __dsub_rn(__ddiv_rn(__ull2double_rn(t2), dn), __dmul_rn(mean, mean));
+  if (var < 0.0) var = 0.0;
+  const double sigma = __dsqrt_rn(var);
+  c.sigma = sigma;
+  for (int k = 0; k < K; ++k) {
+    const double w = (double)(1 << k);
+    const double den = __dmul_rn(sigma, __dsqrt_rn(w));
+    const double wmean = __dmul_rn(w, mean);
+    const double thr = __dadd_rn(wmean, __dmul_rn(threshold, den));
+    c.den[k] = den;
+    c.wmean[k] = wmean;
+    // integer form of "B > thr" for integer B: B >= floor(thr) + 1 (everything passes below 0, nothing above 2^62)
+    c.thr[k] = thr < 0.0 ? 0ull : thr >= 4.0e18 ? ~0ull : (unsigned long long)floor(thr) + 1ull;
+  }
+}
+__device__ __forceinline__ float sps_snr(unsigned long long b, const SpsRowConsts& c, int k) {
+  return c.sigma > 0.0 ? (float)__ddiv_rn(__dsub_rn(__ull2double_rn(b), c.wmean[k]), c.den[k]) : 0.0f;
+}
 
+// Phase A: exact S1, S2 of the row (all threads call; result valid in thread 0 after the reduction through `red`).
+__device__ __forceinline__ void sps_row_sums(const float* x, int n, unsigned long long (&red)[2][kSpsThreads / 32],
+                                             unsigned long long& t1, unsigned long long& t2) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n = p.n;
-  const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
-
-  // ---------------- phase A: exact sums ---------------------------------------------------------------
   unsigned long long s1 = 0, s2 = 0;
   const int n4 = n / 4;  // rows start on 128-byte lines (pitch and range offsets are multiples of 32 floats)
   for (int q = tid; q < n4; q += kSpsThreads) {
@@ -90,106 +116,179 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
   }
   if (lane == 0) red[0][warp] = s1, red[1][warp] = s2;
   __syncthreads();
-  if (tid == 0) {
-    unsigned long long t1 = 0, t2 = 0;
+  t1 = t2 = 0;
+  if (tid == 0)
     for (int i = 0; i < kSpsThreads / 32; ++i) t1 += red[0][i], t2 += red[1][i];
-    const double dn = (double)n;
-    const double mean = __ddiv_rn(__ull2double_rn(t1), dn);
-    double var = __dsub_rn(__ddiv_rn(__ull2double_rn(t2), dn), __dmul_rn(mean, mean));
-    if (var < 0.0) var = 0.0;
-    const double sigma = __dsqrt_rn(var);
-    s_sigma = sigma;
-    for (int k = 0; k < K; ++k) {
-      const double w = (double)(1 << k);
-      const double den = __dmul_rn(sigma, __dsqrt_rn(w));
-      const double wmean = __dmul_rn(w, mean);
-      const double thr = __dadd_rn(wmean, __dmul_rn(p.threshold, den));
-      s_den[k] = den;
-      s_wmean[k] = wmean;
-      // integer form of "B > thr" for integer B: B >= floor(thr) + 1 (everything passes below 0, nothing above 2^62)
-      s_thr[k] = thr < 0.0 ? 0ull : thr >= 4.0e18 ? ~0ull : (unsigned long long)floor(thr) + 1ull;
+}
+
+// Stage samples [tile0, tile0 + span) of the row (zeros past its end) and build the exclusive prefix sum P[0..span].
+// V: [PER * kSpsThreads] scratch (>= span); PER = odd number of consecutive samples per thread (bank-conflict free),
+// compile-time so that both loops unroll and the samples stay in registers between the two.
+template <typename acc_t, int PER>
+__device__ __forceinline__ void sps_build_prefix(const float* x, int n, int tile0, int span, uint32_t* V, acc_t* P,
+                                                 unsigned long long* warp_tot) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int padded = PER * kSpsThreads;
+  if (tile0 + span <= n && (tile0 & 3) == 0) {  // interior: vector loads
+    for (int q = tid; q < span / 4; q += kSpsThreads) {
+      const float4 v = __ldg(reinterpret_cast<const float4*>(x + tile0) + q);
+      *reinterpret_cast<uint4*>(V + 4 * q) = make_uint4((uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w);
     }
+    for (int i = span / 4 * 4 + tid; i < padded; i += kSpsThreads) V[i] = i < span ? (uint32_t)x[tile0 + i] : 0u;
+  } else {
+    for (int i = tid; i < padded; i += kSpsThreads) {
+      const int t = tile0 + i;
+      V[i] = (i < span && t < n) ? (uint32_t)x[t] : 0u;
+    }
+  }
+  __syncthreads();
+  const int i0 = tid * PER;
+  uint32_t v[PER];
+  acc_t loc = 0;
+#pragma unroll
+  for (int i = 0; i < PER; ++i) {
+    v[i] = V[i0 + i];
+    loc += v[i];
+  }
+  acc_t inc = loc;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const acc_t u = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += u;
+  }
+  if (lane == 31) warp_tot[warp] = inc;
+  __syncthreads();
+  acc_t base = inc - loc;
+  for (int wq = 0; wq < warp; ++wq) base += (acc_t)warp_tot[wq];
+  if (tid == 0) P[0] = 0;
+#pragma unroll
+  for (int i = 0; i < PER; ++i) {
+    base += v[i];
+    if (i0 + i < span) P[i0 + i + 1] = base;
+  }
+  __syncthreads();
+}
+// samples per thread in the prefix build: odd, PER * kSpsThreads >= kSpsTile + 2^(K-1)
+__host__ __device__ constexpr int sps_per(int K) { return ((kSpsTile + (1 << (K - 1)) + kSpsThreads - 1) / kSpsThreads) | 1; }
+
+// K = number of widths; WIDE = boxcar sums may reach 2^32 (64-bit prefix sums), else 32-bit modular prefix sums
+// (a difference of two of them is the exact boxcar because it is below 2^32).
+template <int K, bool WIDE>
+__global__ void __launch_bounds__(kSpsThreads, WIDE ? 2 : 3) dd_sps_kernel(const SpsParams p) {
+  using acc_t = typename std::conditional<WIDE, unsigned long long, uint32_t>::type;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  acc_t* P = reinterpret_cast<acc_t*>(smem_raw);  // [kSpsTile + halo + 1]
+  __shared__ unsigned long long red[2][kSpsThreads / 32];
+  __shared__ SpsRowConsts s_c;
+  __shared__ unsigned long long s_best[kSpsMaxK][kSpsThreads / 32];
+  __shared__ int s_tb[kSpsMaxK][kSpsThreads / 32];
+  __shared__ int s_count[kSpsMaxK];  // boxcars at or above the threshold, whole row (rare: shared-memory atomics)
+  __shared__ unsigned long long s_warp_tot[kSpsThreads / 32];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n = p.n;
+  const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
+  const long long orow = (long long)blockIdx.y * p.rows_per_beam + p.row0 + blockIdx.x;
+
+  // ---------------- phase A: exact sums (or the ones dd_execute left behind) ------------------------------
+  if (tid < kSpsMaxK) s_count[tid] = 0;
+  if (p.stats) {
+    if (tid == 0) sps_row_consts(p.stats[2 * orow], p.stats[2 * orow + 1], n, K, p.threshold, s_c);
+  } else {
+    unsigned long long t1, t2;
+    sps_row_sums(x, n, red, t1, t2);
+    if (tid == 0) sps_row_consts(t1, t2, n, K, p.threshold, s_c);
   }
   __syncthreads();
 
   // ---------------- phase B: boxcars from a prefix sum per tile -------------------------------------------
   constexpr int halo = 1 << (K - 1);
   const int span = kSpsTile + halo;          // prefix entries P[0..span]
-  const int per = ((span + kSpsThreads - 1) / kSpsThreads) | 1;
-  acc_t best[K], thr[K];
-  int tb[K], cnt[K];
+  // per thread and width: best1 = (largest boxcar seen) + 1, 0 = none yet; tq >= 0: start of the group of four samples
+  // that holds it, exact position still to be looked up; tq < 0: -(t + 2) with t where it was first seen (-1: nowhere)
+  acc_t best1[K], thr[K];
+  int tq[K];
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    best[k] = 0, tb[k] = 0x7fffffff, cnt[k] = 0;
-    // thresholds above the reach of acc_t can never be met: 2^32-1 is below 2^32 only for sums that small
-    thr[k] = WIDE ? (acc_t)s_thr[k] : (s_thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_thr[k]);
+    best1[k] = 0, tq[k] = -1;
+    // (narrow sums) boxcars stay below 2^32 - 1 (dd_sps_execute picks WIDE otherwise), so a threshold that does not fit
+    // 32 bits is replaced by 2^32 - 1, which no boxcar reaches
+    thr[k] = WIDE ? (acc_t)s_c.thr[k] : (s_c.thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_c.thr[k]);
   }
-  bool never[K];  // (narrow sums) threshold not representable: count stays 0
-#pragma unroll
-  for (int k = 0; k < K; ++k) never[k] = !WIDE && s_thr[k] > 0xffffffffull;
 
-  uint32_t* V = reinterpret_cast<uint32_t*>(smem_raw + (size_t)(span + 2) / 2 * 2 * sizeof(acc_t));  // the tile's samples, [span]
+  uint32_t* V = reinterpret_cast<uint32_t*>(smem_raw + sps_v_offset(span, sizeof(acc_t)));  // the tile's samples, [span]
+  // the four boxcars of width 2^k that start at tl .. tl+3
+  auto boxcars4 = [&](int k, int tl, const acc_t (&a)[4], const acc_t (&a4)[4], acc_t (&b)[4]) {
+    if (k == 0) {
+      b[0] = a[1] - a[0], b[1] = a[2] - a[1], b[2] = a[3] - a[2], b[3] = a4[0] - a[3];
+    } else if (k == 1) {
+      b[0] = a[2] - a[0], b[1] = a[3] - a[1], b[2] = a4[0] - a[2], b[3] = a4[1] - a[3];
+    } else if (k == 2) {
+      b[0] = a4[0] - a[0], b[1] = a4[1] - a[1], b[2] = a4[2] - a[2], b[3] = a4[3] - a[3];
+    } else {
+      acc_t c[4];
+      load4(P + tl + (1 << k), c);
+      b[0] = c[0] - a[0], b[1] = c[1] - a[1], b[2] = c[2] - a[2], b[3] = c[3] - a[3];
+    }
+  };
   for (int tile0 = 0; tile0 < n; tile0 += kSpsTile) {
-    // stage the tile + halo with coalesced loads (samples past the end of the row count as 0)
-    for (int i = tid; i < span; i += kSpsThreads) {
-      const int t = tile0 + i;
-      V[i] = t < n ? (uint32_t)x[t] : 0u;
-    }
-    __syncthreads();
-    // thread-local sums of `per` consecutive samples (per is odd: conflict-free), then a block-wide exclusive
-    // scan of the thread totals
-    const int i0 = tid * per;
-    acc_t loc = 0;
-    for (int i = i0; i < i0 + per && i < span; ++i) loc += V[i];
-    acc_t inc = loc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const acc_t v = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += v;
-    }
-    if (lane == 31) s_warp_tot[warp] = inc;
-    __syncthreads();
-    acc_t base = inc - loc;
-    for (int wq = 0; wq < warp; ++wq) base += (acc_t)s_warp_tot[wq];
-    if (tid == 0) P[0] = 0;
-    for (int i = i0; i < i0 + per && i < span; ++i) {
-      base += V[i];
-      P[i + 1] = base;
-    }
-    __syncthreads();
-    const bool interior = tile0 + span <= n;  // every window of every width of this tile lies inside the row
-    if (interior) {
-      // four consecutive samples per thread and step: the prefix sums come in vectors, the maximum of the four
-      // boxcars is compared with the running best once, and only a new best looks for its position
-      for (int q = tid; q < kSpsTile / 4; q += kSpsThreads) {
-        const int tl = 4 * q, t = tile0 + tl;
+    sps_build_prefix<acc_t, sps_per(K)>(x, n, tile0, span, V, P, s_warp_tot);
+    // groups of four samples whose windows of every width lie inside the row take the vector path; the last
+    // halo + 3 samples of the row are done one by one below
+    const int nfast = min(kSpsTile, max(0, n - halo - 3 - tile0 + 1)) / 4;  // groups q < nfast: tile0 + 4q + 3 + halo <= n
+    {
+      // Four consecutive samples per thread and step; the prefix sums come in vectors.  Only the maximum m of the four
+      // boxcars is looked at in the loop: "m reaches the threshold" sets a bit (rare: those groups are counted one by
+      // one after the loop) and "m beats the best" records the group (its exact position is looked up after the loop).
+      uint32_t hits = 0;
+      for (int q = tid; q < nfast; q += kSpsThreads) {
+        const int tl = 4 * q;
         acc_t a[4], a4[4];
         load4(P + tl, a);
         load4(P + tl + 4, a4);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
           acc_t b[4];
-          if (k == 0) {
-            b[0] = a[1] - a[0], b[1] = a[2] - a[1], b[2] = a[3] - a[2], b[3] = a4[0] - a[3];
-          } else if (k == 1) {
-            b[0] = a[2] - a[0], b[1] = a[3] - a[1], b[2] = a4[0] - a[2], b[3] = a4[1] - a[3];
-          } else if (k == 2) {
-            b[0] = a4[0] - a[0], b[1] = a4[1] - a[1], b[2] = a4[2] - a[2], b[3] = a4[3] - a[3];
-          } else {
-            acc_t c[4];
-            load4(P + tl + (1 << k), c);
-            b[0] = c[0] - a[0], b[1] = c[1] - a[1], b[2] = c[2] - a[2], b[3] = c[3] - a[3];
-          }
-          if (!never[k]) cnt[k] += (b[0] >= thr[k]) + (b[1] >= thr[k]) + (b[2] >= thr[k]) + (b[3] >= thr[k]);
+          boxcars4(k, tl, a, a4, b);
           const acc_t m01 = b[0] > b[1] ? b[0] : b[1], m23 = b[2] > b[3] ? b[2] : b[3], m = m01 > m23 ? m01 : m23;
-          if (m > best[k] || tb[k] == 0x7fffffff) {  // rare once the row's level is reached; t increases, so the first maximum is kept
-            best[k] = m;
-            tb[k] = t + (b[0] == m ? 0 : b[1] == m ? 1 : b[2] == m ? 2 : 3);
+          if (m >= thr[k]) hits |= 1u << k;
+          if (m >= best1[k]) {  // m > best; t increases, so the first maximum is kept
+            best1[k] = m + 1;
+            tq[k] = tile0 + tl;
           }
         }
       }
-    } else {
-      for (int tl = tid; tl < kSpsTile; tl += kSpsThreads) {
+      if (hits) {  // count the boxcars at or above the threshold in this thread's groups of the widths that had one
+        for (int q = tid; q < nfast; q += kSpsThreads) {
+          const int tl = 4 * q;
+          acc_t a[4], a4[4];
+          load4(P + tl, a);
+          load4(P + tl + 4, a4);
+#pragma unroll
+          for (int k = 0; k < K; ++k) {
+            if (!(hits & (1u << k))) continue;
+            acc_t b[4];
+            boxcars4(k, tl, a, a4, b);
+            const int c = (b[0] >= thr[k]) + (b[1] >= thr[k]) + (b[2] >= thr[k]) + (b[3] >= thr[k]);
+            if (c) atomicAdd(&s_count[k], c);
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < K; ++k) {
+        if (tq[k] >= 0) {  // a new best in this tile: which of the four was it
+          const int tl = tq[k] - tile0;
+          acc_t a[4], a4[4], b[4];
+          load4(P + tl, a);
+          load4(P + tl + 4, a4);
+          boxcars4(k, tl, a, a4, b);
+          const acc_t m = best1[k] - 1;
+          tq[k] = -(tq[k] + (b[0] == m ? 0 : b[1] == m ? 1 : b[2] == m ? 2 : 3) + 2);
+        }
+      }
+    }
+    if (4 * nfast < kSpsTile) {  // the end of the row: windows checked one by one
+      for (int tl = 4 * nfast + tid; tl < kSpsTile; tl += kSpsThreads) {
         const int t = tile0 + tl;
         if (t >= n) break;
         const acc_t p0 = P[tl];
@@ -198,8 +297,8 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
           const int w = 1 << k;
           if (t + w <= n) {
             const acc_t b = P[tl + w] - p0;
-            if (b > best[k] || tb[k] == 0x7fffffff) best[k] = b, tb[k] = t;
-            cnt[k] += (b >= thr[k]) && !never[k];
+            if (b >= best1[k]) best1[k] = b + 1, tq[k] = -(t + 2);
+            if (b >= thr[k]) atomicAdd(&s_count[k], 1);
           }
         }
       }
@@ -210,38 +309,134 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_kernel(const SpsParams p) 
   // ---------------- reduce over the block: larger sum wins, ties go to the smaller t ----------------------
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    {
-      unsigned long long b = best[k];
-      int t = tb[k], c = cnt[k];
+    unsigned long long b = best1[k];  // (best + 1; 0 = this thread saw no window of this width)
+    int t = best1[k] ? -(tq[k] + 2) : 0x7fffffff;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        const unsigned long long ob = shfl_down_u64(b, o);
-        const int ot = __shfl_down_sync(0xffffffffu, t, o);
-        c += __shfl_down_sync(0xffffffffu, c, o);
-        if (ot != 0x7fffffff && (t == 0x7fffffff || ob > b || (ob == b && ot < t))) b = ob, t = ot;
-      }
-      if (lane == 0) s_best[k][warp] = b, s_tb[k][warp] = t, s_cnt[k][warp] = c;
+    for (int o = 16; o > 0; o >>= 1) {
+      const unsigned long long ob = shfl_down_u64(b, o);
+      const int ot = __shfl_down_sync(0xffffffffu, t, o);
+      if (ob > b || (ob == b && ot < t)) b = ob, t = ot;
     }
+    if (lane == 0) s_best[k][warp] = b, s_tb[k][warp] = t;
   }
   __syncthreads();
   if (tid < K) {
     const int k = tid;
     unsigned long long b = 0;
-    int t = 0x7fffffff, c = 0;
+    int t = 0x7fffffff;
+    const int c = s_count[k];
     for (int i = 0; i < kSpsThreads / 32; ++i) {
       const unsigned long long ob = s_best[k][i];
       const int ot = s_tb[k][i];
-      c += s_cnt[k][i];
-      if (ot != 0x7fffffff && (t == 0x7fffffff || ob > b || (ob == b && ot < t))) b = ob, t = ot;
+      if (ob > b || (ob == b && ot < t)) b = ob, t = ot;
     }
-    const long long o = ((long long)blockIdx.y * p.rows_per_beam + p.row0 + blockIdx.x) * K + k;
-    if (t == 0x7fffffff) {  // filter wider than the row
+    const long long o = orow * K + k;
+    if (b == 0) {  // filter wider than the row
       p.snr[o] = 0.0f, p.tmax[o] = -1, p.count[o] = 0;
     } else {
-      const double sigma = s_sigma;
-      p.snr[o] = sigma > 0.0 ? (float)__ddiv_rn(__dsub_rn(__ull2double_rn(b), s_wmean[k]), s_den[k]) : 0.0f;
+      p.snr[o] = sps_snr(b - 1, s_c, k);
       p.tmax[o] = t;
       p.count[o] = c;
+    }
+  }
+}
+
+// Exclusive scan of count[0..m) into offsets[0..m] (int64), one CTA: the list positions of every (row, width).
+__global__ void __launch_bounds__(1024) dd_sps_scan_kernel(const int32_t* __restrict__ count, long long m,
+                                                           long long* __restrict__ offsets) {
+  __shared__ long long wsum[32];
+  __shared__ long long carry;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) carry = 0;
+  __syncthreads();
+  for (long long base = 0; base < m; base += 1024) {
+    const long long i = base + tid;
+    const long long v = i < m ? (long long)count[i] : 0;
+    long long inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const long long u = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += u;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    long long pre = carry;
+    for (int wq = 0; wq < warp; ++wq) pre += wsum[wq];
+    if (i < m) offsets[i] = pre + inc - v;
+    __syncthreads();
+    if (tid == 1023) carry = pre + inc;
+    __syncthreads();
+  }
+  if (tid == 0) offsets[m] = carry;
+}
+
+// The candidate list: (row, k, t, snr) of every boxcar above the threshold, in the order row, k, t, written at
+// offsets[row*K + k] + (rank of t).  One CTA per row; rows without candidates (almost all) return at once.
+template <bool WIDE>
+__global__ void __launch_bounds__(kSpsThreads) dd_sps_fill_kernel(const SpsParams p) {
+  using acc_t = typename std::conditional<WIDE, unsigned long long, uint32_t>::type;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  acc_t* P = reinterpret_cast<acc_t*>(smem_raw);
+  __shared__ unsigned long long red[2][kSpsThreads / 32];
+  __shared__ SpsRowConsts s_c;
+  __shared__ unsigned long long s_warp_tot[kSpsThreads / 32];
+  __shared__ int s_wcnt[kSpsThreads / 32];
+  __shared__ long long s_written;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n = p.n, K = p.K;
+  const long long orow = (long long)blockIdx.y * p.rows_per_beam + p.row0 + blockIdx.x;
+  if (p.offsets[orow * K + K] == p.offsets[orow * K]) return;  // no candidate in this row
+  const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
+  if (p.stats) {
+    if (tid == 0) sps_row_consts(p.stats[2 * orow], p.stats[2 * orow + 1], n, K, p.threshold, s_c);
+  } else {
+    unsigned long long t1, t2;
+    sps_row_sums(x, n, red, t1, t2);
+    if (tid == 0) sps_row_consts(t1, t2, n, K, p.threshold, s_c);
+  }
+  __syncthreads();
+  const int halo = 1 << (K - 1);
+  const int span = kSpsTile + halo;
+  uint32_t* V = reinterpret_cast<uint32_t*>(smem_raw + sps_v_offset(span, sizeof(acc_t)));
+  for (int k = 0; k < K; ++k) {
+    const long long o0 = p.offsets[orow * K + k], o1 = p.offsets[orow * K + k + 1];
+    if (o1 == o0) continue;
+    const int w = 1 << k;
+    const unsigned long long thr = s_c.thr[k];
+    if (tid == 0) s_written = 0;
+    __syncthreads();
+    for (int tile0 = 0; tile0 < n; tile0 += kSpsTile) {
+      if (K <= 9)
+        sps_build_prefix<acc_t, sps_per(9)>(x, n, tile0, span, V, P, s_warp_tot);
+      else
+        sps_build_prefix<acc_t, sps_per(12)>(x, n, tile0, span, V, P, s_warp_tot);
+      for (int c0 = 0; c0 < kSpsTile && tile0 + c0 < n; c0 += kSpsThreads) {  // 256 consecutive t at a time, in order
+        const int tl = c0 + tid, t = tile0 + tl;
+        const bool in = t + w <= n;
+        const unsigned long long b = in ? (unsigned long long)(acc_t)(P[tl + w] - P[tl]) : 0ull;
+        const bool hit = in && b >= thr && (WIDE || thr <= 0xffffffffull);
+        const unsigned bal = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0) s_wcnt[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+        for (int wq = 0; wq < kSpsThreads / 32; ++wq) {
+          before += wq < warp ? s_wcnt[wq] : 0;
+          total += s_wcnt[wq];
+        }
+        if (hit) {
+          const long long pos = o0 + s_written + before + __popc(bal & ((1u << lane) - 1u));
+          if (pos < p.max_cands) {
+            dd_sps_cand_t c;
+            c.row = (int32_t)orow, c.width_log2 = k, c.t = t, c.snr = sps_snr(b, s_c, k);
+            p.cand[pos] = c;
+          }
+        }
+        __syncthreads();
+        if (tid == 0) s_written += total;
+        __syncthreads();
+      }
+      __syncthreads();
     }
   }
 }
@@ -257,6 +452,43 @@ static cudaError_t launch_sps(const SpsParams& sp, dim3 grid, size_t smem, cudaS
 
 }  // namespace dd
 
+namespace {
+
+// validation shared by the entry points; rows_per_beam out
+int sps_check(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, double threshold, int64_t* rows_per_beam) {
+  if (!p || !plane_dev || nwidths < 1 || nwidths > dd::kSpsMaxK || p->device < 0 ||
+      !(threshold >= -1.0e300 && threshold <= 1.0e300))
+    return DD_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(plane_dev) & 15u) != 0) return DD_ERR_ALIGN;  // rows are read with 16-byte loads
+  int cur = -1;
+  cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return dd::cuda_fail(e, "cudaGetDevice");
+  if (cur != p->device) return DD_ERR_DEVICE;
+  *rows_per_beam = 0;
+  for (const auto& r : p->ranges) {
+    // exactness of S2 = sum x^2 in 64 bits: (largest possible sum)^2 * nout < 2^63
+    const double v = (double)p->nchans * (double)((1 << p->in_bits) - 1) * (double)r.decim;
+    if (v * v * (double)r.nout >= 9.2e18 || r.nout > 0x7fffffffLL) return DD_ERR_OVERFLOW;
+    *rows_per_beam += r.ndm;
+  }
+  return DD_OK;
+}
+
+bool sps_wide(const dd_plan_t* p, const dd::RangePlan& r, int nwidths) {
+  // 32-bit prefix sums while the widest boxcar of the largest possible samples stays below 2^32 - 1 (the kernel
+  // keeps "best + 1" and uses 2^32 - 1 as the unreachable threshold)
+  const double vmax = (double)p->nchans * (double)((1 << p->in_bits) - 1) * (double)r.decim;
+  return vmax * (double)(1 << (nwidths - 1)) >= 4294967295.0;
+}
+
+size_t sps_smem(bool wide, int nwidths) {
+  const size_t span = (size_t)dd::kSpsTile + ((size_t)1 << (nwidths - 1));
+  // V is padded to a whole number of samples per thread (the larger of the kernels' choices)
+  return dd::sps_v_offset(span, wide ? 8 : 4) + (size_t)dd::sps_per(nwidths <= 9 ? 9 : 12) * dd::kSpsThreads * 4;
+}
+
+}  // namespace
+
 extern "C" {
 
 int dd_sps_rows(const dd_plan_t* p, int64_t* rows) {
@@ -269,21 +501,14 @@ int dd_sps_rows(const dd_plan_t* p, int64_t* rows) {
 
 int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, double threshold, float* snr_dev,
                    int32_t* tmax_dev, int32_t* count_dev, void* cuda_stream) {
-  if (!p || !plane_dev || !snr_dev || !tmax_dev || !count_dev || nwidths < 1 || nwidths > dd::kSpsMaxK || p->device < 0 ||
-      !(threshold >= -1.0e300 && threshold <= 1.0e300))
-    return DD_ERR_INVALID;
+  if (!snr_dev || !tmax_dev || !count_dev) return DD_ERR_INVALID;
   int64_t rows_per_beam = 0;
-  for (const auto& r : p->ranges) {
-    // exactness of S2 = sum x^2 in 64 bits: (largest possible sum)^2 * nout < 2^63
-    const double v = (double)p->nchans * (double)((1 << p->in_bits) - 1) * (double)r.decim;
-    if (v * v * (double)r.nout >= 9.2e18 || r.nout > 0x7fffffffLL) return DD_ERR_OVERFLOW;
-    rows_per_beam += r.ndm;
-  }
+  int rc = sps_check(p, plane_dev, nwidths, threshold, &rows_per_beam);
+  if (rc != DD_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  const size_t span = (size_t)dd::kSpsTile + ((size_t)1 << (nwidths - 1));
   int64_t row0 = 0;
   for (const auto& r : p->ranges) {
-    dd::SpsParams sp;
+    dd::SpsParams sp = {};
     sp.plane = plane_dev + r.offset;
     sp.beam_stride = p->beam_stride;
     sp.pitch = r.pitch;
@@ -295,10 +520,9 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
     sp.count = count_dev;
     sp.row0 = row0;
     sp.rows_per_beam = rows_per_beam;
-    // 32-bit prefix sums while the widest boxcar of the largest possible samples stays below 2^32
-    const double vmax = (double)p->nchans * (double)((1 << p->in_bits) - 1) * (double)r.decim;
-    const bool wide = vmax * (double)(1 << (nwidths - 1)) >= 4294967296.0;
-    const size_t smem = (span + 2) / 2 * 2 * (wide ? 8 : 4) + span * 4;
+    sp.stats = p->row_stats;
+    const bool wide = sps_wide(p, r, nwidths);
+    const size_t smem = sps_smem(wide, nwidths);
     const dim3 grid((unsigned)r.ndm, (unsigned)p->nbeams);
     cudaError_t e = cudaErrorInvalidValue;
 #define DD_SPS(K_)                                                                                                  \
@@ -311,6 +535,49 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
     }
 #undef DD_SPS
     if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_kernel launch");
+    row0 += r.ndm;
+  }
+  return DD_OK;
+}
+
+int dd_sps_candidates(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, double threshold, const int32_t* count_dev,
+                      int64_t* offsets_dev, dd_sps_cand_t* cand_dev, int64_t max_cands, void* cuda_stream) {
+  if (!count_dev || !offsets_dev || max_cands < 0 || (max_cands > 0 && !cand_dev)) return DD_ERR_INVALID;
+  int64_t rows_per_beam = 0;
+  int rc = sps_check(p, plane_dev, nwidths, threshold, &rows_per_beam);
+  if (rc != DD_OK) return rc;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const int64_t m = rows_per_beam * p->nbeams * nwidths;
+  dd::dd_sps_scan_kernel<<<1, 1024, 0, stream>>>(count_dev, m, reinterpret_cast<long long*>(offsets_dev));
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_scan_kernel launch");
+  int64_t row0 = 0;
+  for (const auto& r : p->ranges) {
+    dd::SpsParams sp = {};
+    sp.plane = plane_dev + r.offset;
+    sp.beam_stride = p->beam_stride;
+    sp.pitch = r.pitch;
+    sp.n = (int)r.nout;
+    sp.K = nwidths;
+    sp.threshold = threshold;
+    sp.row0 = row0;
+    sp.rows_per_beam = rows_per_beam;
+    sp.stats = p->row_stats;
+    sp.offsets = reinterpret_cast<const long long*>(offsets_dev);
+    sp.cand = cand_dev;
+    sp.max_cands = max_cands;
+    const bool wide = sps_wide(p, r, nwidths);
+    const size_t smem = sps_smem(wide, nwidths);
+    const dim3 grid((unsigned)r.ndm, (unsigned)p->nbeams);
+    if (wide) {
+      e = cudaFuncSetAttribute(dd::dd_sps_fill_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+      if (e == cudaSuccess) dd::dd_sps_fill_kernel<true><<<grid, dd::kSpsThreads, smem, stream>>>(sp);
+    } else {
+      e = cudaFuncSetAttribute(dd::dd_sps_fill_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+      if (e == cudaSuccess) dd::dd_sps_fill_kernel<false><<<grid, dd::kSpsThreads, smem, stream>>>(sp);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_fill_kernel launch");
     row0 += r.ndm;
   }
   return DD_OK;

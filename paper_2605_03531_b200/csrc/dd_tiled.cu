@@ -112,6 +112,8 @@ struct TiledParams {
   int rowpitch;      // superwords per staged row = T + Smax
   int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
   float accum_scale;  // 0: store; else out = value * accum_scale + out (high byte plane of uint16 input)
+  unsigned long long* stats;  // nullptr, or [beam][trial of this range][2]: sum x and sum x^2 of the rows written (dd_plan_set_row_stats)
+  long long stats_beam_stride;
 };
 
 __host__ __device__ inline size_t tiled_stage_bytes(int mode, int NL, int Cc, int rowpitch, int G) {
@@ -574,25 +576,41 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
 
   // ---------------- a4: DM-time writer, fp32 (I2F rounds to nearest even) -------------------------
   const long long i = tau * p.T + ti;
-  if (i >= p.H) return;
+  const bool active = i < p.H;  // (threads past the lane segment keep running: the row statistics reduce over whole warps)
+  if (!active && !p.stats) return;
   float* obase = p.out + (long long)beam * p.out_beam_stride;
 #pragma unroll
   for (int j = 0; j < RD; ++j) {
     const int jj = (blk * p.G + g) * RD + j;
-    if (jj >= p.ndm) break;
+    if (jj >= p.ndm) break;  // warp-uniform
     float* orow = obase + (long long)jj * p.pitch;
     uint32_t v[NL];
     lanes.values(j, v);
+    unsigned long long s1 = 0, s2 = 0;
 #pragma unroll
     for (int m = 0; m < NL; ++m) {
       const long long t = i + (long long)m * p.H;  // consecutive threads -> consecutive floats
-      if (t < p.nout) {
+      if (active && t < p.nout) {
         // second byte plane of uint16 input: S = S_lo + 256*S_hi.  Both plane sums are < 2^24, hence exact
         // floats, and the fused multiply-add rounds the exact total once: fl32(S), as the definition asks.
         if (p.accum_scale != 0.0f)
           orow[t] = __fmaf_rn(__uint2float_rn(v[m]), p.accum_scale, orow[t]);
         else
           orow[t] = __uint2float_rn(v[m]);
+        s1 += v[m];
+        s2 += (unsigned long long)v[m] * v[m];
+      }
+    }
+    if (p.stats) {  // sum x, sum x^2 of this row's piece: one pair of atomics per warp and trial (exact integers)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        s1 += __shfl_down_sync(0xffffffffu, s1, o);
+        s2 += __shfl_down_sync(0xffffffffu, s2, o);
+      }
+      if (lane == 0) {
+        unsigned long long* st = p.stats + (long long)beam * p.stats_beam_stride + 2ll * jj;
+        atomicAdd(st, s1);
+        atomicAdd(st + 1, s2);
       }
     }
   }
@@ -654,6 +672,8 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.blk0 = blk0;
   tp.nblk = nblk;
   tp.rowpitch = pairs ? r.T + r.Smax2 : r.T + r.Smax;
+  tp.stats = (p->row_stats && r.planes == 1) ? p->row_stats + 2 * r.row0 : nullptr;
+  tp.stats_beam_stride = 2 * p->rows_per_beam;
   tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;  // pairs: a stage holds Cc/2 pair sums of twice the size: same interval
   const long long nctas = (long long)nblk * r.ntau * p->nbeams;
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;

@@ -96,3 +96,111 @@ def test_sps_all_zero_rows_and_long_rows():
     for k in ("tmax", "count"):
         assert np.array_equal(got[k], ref[k]), k
     assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
+
+
+# ---- the candidate list (dd_sps_candidates) and the row statistics of the dedispersion epilogue -------------------------
+def _candidates_gpu(plan, plane, K, thr, cnt, max_cands):
+    import torch
+    rows = plan.sps_rows()
+    offsets = torch.full((rows * K + 1,), -1, dtype=torch.int64, device="cuda")
+    cand = torch.full((max(1, max_cands), 4), -1, dtype=torch.int32, device="cuda")
+    plan.sps_candidates(plane, K, thr, cnt, offsets, cand, max_cands, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    return offsets.cpu().numpy(), cand.cpu().numpy()
+
+
+def _oracle_candidates(want_planes, w, K, thr):
+    """The oracle's list over the oracle's planes, rows renumbered as in dd_sps_rows (beam-major, ranges in order)."""
+    out, row0 = [], 0
+    for b in range(w.nbeams):
+        for r in range(len(w.ranges)):
+            pl = np.ascontiguousarray(want_planes[b][r])
+            cand, total = oracle.sps_candidates(pl, pl.shape[1], K, thr, cap=1 << 22)
+            assert total == len(cand)
+            c = cand.copy()
+            c["row"] += row0
+            out.append(c)
+            row0 += pl.shape[0]
+    return np.concatenate(out)
+
+
+@pytest.mark.parametrize("K,thr,stats", [(6, 4.0, False), (6, 4.0, True), (12, 3.0, False), (3, -1.0, True)])
+def test_candidate_list_matches_oracle(K, thr, stats):
+    """Every (row, k, t, snr) above the threshold, in the order row, k, t -- bit for bit, with the row statistics
+    either recomputed by the search (two reads of the plane) or taken from the dedispersion epilogue (one read)."""
+    import torch
+    from paper_2605_03531_b200 import binding as B
+    w = W.scaled(W.CONFIGS[3], nchans=64, nsamps=2 ** 13 + 123, nbeams=2,
+                 ranges=[W.DMRange(0.0, 0.2, 21, 1), W.DMRange(40.0, 3.0, 9, 2), W.DMRange(600.0, 2.0, 7, 4)])
+    x = W.generate(w)
+    x[0, :, 3000:3006] = np.minimum(x[0, :, 3000:3006].astype(np.int32) + 25, 255).astype(np.uint8)
+    x[1, :, 7000:7100] = np.minimum(x[1, :, 7000:7100].astype(np.int32) + 6, 255).astype(np.uint8)
+    plan = B.Plan.from_workload(w)
+    rows = plan.sps_rows()
+    out = torch.zeros(plan.out_elems(), dtype=torch.float32, device="cuda")
+    st = None
+    if stats:
+        st = torch.full((rows, 2), -1, dtype=torch.int64, device="cuda")
+        plan.set_row_stats(st)
+    plan.execute(torch.from_numpy(x).cuda(), out, torch.cuda.current_stream())
+    snr = torch.empty((rows, K), dtype=torch.float32, device="cuda")
+    tmax = torch.empty((rows, K), dtype=torch.int32, device="cuda")
+    cnt = torch.empty((rows, K), dtype=torch.int32, device="cuda")
+    plan.sps_execute(out, K, thr, snr, tmax, cnt, torch.cuda.current_stream())
+    want_planes = oracle_full(w, x)
+    want = _oracle_candidates(want_planes, w, K, thr)
+    assert len(want) > 50
+    offsets, cand = _candidates_gpu(plan, out, K, thr, cnt, len(want) + 10)
+    counts = cnt.cpu().numpy().ravel()
+    assert offsets[0] == 0 and offsets[-1] == len(want) and np.array_equal(np.diff(offsets), counts)
+    got = cand[: len(want)]
+    assert np.array_equal(got[:, 0], want["row"]) and np.array_equal(got[:, 1], want["k"]) and np.array_equal(got[:, 2], want["t"])
+    assert np.array_equal(got[:, 3].view(np.uint32), want["snr"].view(np.uint32))
+    assert (cand[len(want):] == -1).all()                              # nothing written past the list
+    if stats:   # the epilogue's sums are the exact row sums
+        sth = st.cpu().numpy()
+        row = 0
+        for b in range(w.nbeams):
+            for r in range(len(w.ranges)):
+                pl = want_planes[b][r].astype(np.float64)
+                assert np.array_equal(sth[row: row + pl.shape[0], 0], pl.sum(axis=1).astype(np.int64))
+                assert np.array_equal(sth[row: row + pl.shape[0], 1], (pl * pl).sum(axis=1).astype(np.int64))
+                row += pl.shape[0]
+        # and the search gives the same results with and without them
+        plan.set_row_stats(None)
+        snr2, tmax2, cnt2 = torch.empty_like(snr), torch.empty_like(tmax), torch.empty_like(cnt)
+        plan.sps_execute(out, K, thr, snr2, tmax2, cnt2, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert torch.equal(snr.view(torch.int32), snr2.view(torch.int32)) and torch.equal(tmax, tmax2) and torch.equal(cnt, cnt2)
+    # a capacity below the total: the first entries, and the total still reported
+    offsets2, few = _candidates_gpu(plan, out, K, thr, cnt, 17)
+    assert offsets2[-1] == len(want) and np.array_equal(few[:17], cand[:17])
+    plan.destroy()
+
+
+def test_row_stats_with_the_direct_kernel_and_subband_variant():
+    import torch
+    from paper_2605_03531_b200 import binding as B
+    w = W.Workload("stats", 600.0, -200.0 / 4096, 96, 1.31072e-3, 2 ** 13, 1, 8,
+                   (W.DMRange(0.0, 0.3, 40, 1), W.DMRange(300.0, 0.9, 24, 2)), 5, 128, 12)
+    x = W.generate(w)
+    want_planes = oracle_full(w, x)
+    for variant in (B.DD_KERNEL_DIRECT, B.DD_KERNEL_TILED, B.DD_KERNEL_SUBBAND):
+        plan = B.Plan.from_workload(w)
+        plan.set_kernel(variant)
+        st = torch.full((plan.sps_rows(), 2), -1, dtype=torch.int64, device="cuda")
+        plan.set_row_stats(st)
+        out = torch.zeros(plan.out_elems(), dtype=torch.float32, device="cuda")
+        for _ in range(2):                                             # twice: the sums are zeroed by every execute
+            plan.execute(torch.from_numpy(x).cuda(), out, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        sth, row = st.cpu().numpy(), 0
+        for r in range(2):
+            pl = want_planes[0][r].astype(np.float64)
+            assert np.array_equal(sth[row: row + pl.shape[0], 0], pl.sum(axis=1).astype(np.int64)), variant
+            assert np.array_equal(sth[row: row + pl.shape[0], 1], (pl * pl).sum(axis=1).astype(np.int64)), variant
+            row += pl.shape[0]
+        plan.destroy()
+    p16 = B.Plan(500.0, -1.0, 16, 1e-3, 4096, [(0.0, 1.0, 2, 1)], in_bits=16)
+    with pytest.raises(B.DDError):
+        p16.set_row_stats(st)
