@@ -23,6 +23,7 @@
 #include <type_traits>
 
 #include "dd_internal.h"
+#include "dd_ptx.cuh"
 
 namespace dd {
 
@@ -47,7 +48,7 @@ struct SpsParams {
 };
 
 // dynamic shared memory: P[span + 1] prefix sums, then (16-byte aligned) V[span] samples
-__host__ __device__ inline size_t sps_v_offset(size_t span, size_t acc_bytes) { return ((span + 1) * acc_bytes + 15) / 16 * 16; }
+__host__ __device__ inline size_t sps_v_offset(size_t span, size_t acc_bytes) { return ((span + 1) * acc_bytes + 127) / 128 * 128; }
 
 __device__ __forceinline__ unsigned long long shfl_down_u64(unsigned long long v, int o) {
   return __shfl_down_sync(0xffffffffu, v, o);
@@ -168,18 +169,50 @@ __device__ __forceinline__ void sps_build_prefix(const float* x, int n, int tile
   }
   __syncthreads();
 }
+// The same from a tile of raw floats already in shared memory (bulk-copied there): X[i] = sample tile0 + i for
+// i < loaded, anything beyond counts as zero.
+template <typename acc_t, int PER>
+__device__ __forceinline__ void sps_build_prefix_raw(const float* X, int valid, int span, acc_t* P, unsigned long long* warp_tot) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int i0 = tid * PER;
+  uint32_t v[PER];
+  acc_t loc = 0;
+#pragma unroll
+  for (int i = 0; i < PER; ++i) {
+    v[i] = i0 + i < valid ? (uint32_t)X[i0 + i] : 0u;  // valid = samples of this tile that exist (row end) and were copied
+    loc += v[i];
+  }
+  acc_t inc = loc;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const acc_t u = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += u;
+  }
+  if (lane == 31) warp_tot[warp] = inc;
+  __syncthreads();
+  acc_t base = inc - loc;
+  for (int wq = 0; wq < warp; ++wq) base += (acc_t)warp_tot[wq];
+  if (tid == 0) P[0] = 0;
+#pragma unroll
+  for (int i = 0; i < PER; ++i) {
+    base += v[i];
+    if (i0 + i < span) P[i0 + i + 1] = base;
+  }
+  __syncthreads();
+}
 // samples per thread in the prefix build: odd, PER * kSpsThreads >= kSpsTile + 2^(K-1)
 __host__ __device__ constexpr int sps_per(int K) { return ((kSpsTile + (1 << (K - 1)) + kSpsThreads - 1) / kSpsThreads) | 1; }
 
 // K = number of widths; WIDE = boxcar sums may reach 2^32 (64-bit prefix sums), else 32-bit modular prefix sums
 // (a difference of two of them is the exact boxcar because it is below 2^32).
 template <int K, bool WIDE>
-__global__ void __launch_bounds__(kSpsThreads, WIDE ? 2 : 3) dd_sps_kernel(const SpsParams p) {
+__global__ void __launch_bounds__(kSpsThreads, WIDE ? 2 : (K <= 8 ? 4 : 3)) dd_sps_kernel(const SpsParams p) {
   using acc_t = typename std::conditional<WIDE, unsigned long long, uint32_t>::type;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   acc_t* P = reinterpret_cast<acc_t*>(smem_raw);  // [kSpsTile + halo + 1]
   __shared__ unsigned long long red[2][kSpsThreads / 32];
   __shared__ SpsRowConsts s_c;
+  __shared__ __align__(8) unsigned long long s_bar[2];  // "tile landed" barriers of the two raw-sample buffers
   __shared__ unsigned long long s_best[kSpsMaxK][kSpsThreads / 32];
   __shared__ int s_tb[kSpsMaxK][kSpsThreads / 32];
   __shared__ int s_count[kSpsMaxK];  // boxcars at or above the threshold, whole row (rare: shared-memory atomics)
@@ -216,7 +249,23 @@ __global__ void __launch_bounds__(kSpsThreads, WIDE ? 2 : 3) dd_sps_kernel(const
     thr[k] = WIDE ? (acc_t)s_c.thr[k] : (s_c.thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_c.thr[k]);
   }
 
-  uint32_t* V = reinterpret_cast<uint32_t*>(smem_raw + sps_v_offset(span, sizeof(acc_t)));  // the tile's samples, [span]
+  // Raw tiles (kSpsTile + halo floats, rounded up to 16 bytes, clipped to the row's pitch) are brought in by 1-D bulk
+  // copies (TMA) into two buffers: the copy of tile i+1 is in flight while tile i is filtered.
+  constexpr int kPer = sps_per(K);
+  float* const X0 = reinterpret_cast<float*>(smem_raw + sps_v_offset(span, sizeof(acc_t)));  // buffer b at X0 + b*kXstride
+  constexpr int kXstride = kPer * kSpsThreads;
+  const uint32_t bar0 = smem_u32(&s_bar[0]);
+  auto tile_floats = [&](int tile0) { return min((span + 3) & ~3, ((n + 3) & ~3) - tile0); };  // rows are padded to 32 floats
+  if (tid == 0) {
+    mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, 1);
+    fence_barrier_init();
+    const uint32_t bytes = (uint32_t)tile_floats(0) * 4u;
+    mbar_arrive_expect_tx(bar0, bytes);
+    bulk_copy_g2s(smem_u32(X0), x, bytes, bar0);
+  }
+  __syncthreads();
+  uint32_t phase = 0;  // bit b: parity to wait for on buffer b
   // the four boxcars of width 2^k that start at tl .. tl+3
   auto boxcars4 = [&](int k, int tl, const acc_t (&a)[4], const acc_t (&a4)[4], acc_t (&b)[4]) {
     if (k == 0) {
@@ -231,8 +280,16 @@ __global__ void __launch_bounds__(kSpsThreads, WIDE ? 2 : 3) dd_sps_kernel(const
       b[0] = c[0] - a[0], b[1] = c[1] - a[1], b[2] = c[2] - a[2], b[3] = c[3] - a[3];
     }
   };
-  for (int tile0 = 0; tile0 < n; tile0 += kSpsTile) {
-    sps_build_prefix<acc_t, sps_per(K)>(x, n, tile0, span, V, P, s_warp_tot);
+  int buf = 0;
+  for (int tile0 = 0; tile0 < n; tile0 += kSpsTile, buf ^= 1) {
+    if (tid == 0 && tile0 + kSpsTile < n) {  // next tile into the other buffer (its last readers passed the barrier below)
+      const uint32_t bytes = (uint32_t)tile_floats(tile0 + kSpsTile) * 4u;
+      mbar_arrive_expect_tx(bar0 + 8u * (buf ^ 1), bytes);
+      bulk_copy_g2s(smem_u32(X0 + (buf ^ 1) * kXstride), x + tile0 + kSpsTile, bytes, bar0 + 8u * (buf ^ 1));
+    }
+    mbar_wait(bar0 + 8u * buf, (phase >> buf) & 1u);
+    phase ^= 1u << buf;
+    sps_build_prefix_raw<acc_t, kPer>(X0 + buf * kXstride, min(span, n - tile0), span, P, s_warp_tot);
     // groups of four samples whose windows of every width lie inside the row take the vector path; the last
     // halo + 3 samples of the row are done one by one below
     const int nfast = min(kSpsTile, max(0, n - halo - 3 - tile0 + 1)) / 4;  // groups q < nfast: tile0 + 4q + 3 + halo <= n
@@ -444,7 +501,9 @@ __global__ void __launch_bounds__(kSpsThreads) dd_sps_fill_kernel(const SpsParam
 template <int K, bool WIDE>
 static cudaError_t launch_sps(const SpsParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
   // per launch: the attribute is per device and the call is cheap (no static flag: not device- or thread-safe)
-  cudaError_t e = cudaFuncSetAttribute(dd_sps_kernel<K, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(dd_sps_kernel<K, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(dd_sps_kernel<K, WIDE>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   if (e != cudaSuccess) return e;
   dd_sps_kernel<K, WIDE><<<grid, kSpsThreads, smem, stream>>>(sp);
   return cudaGetLastError();
@@ -483,8 +542,9 @@ bool sps_wide(const dd_plan_t* p, const dd::RangePlan& r, int nwidths) {
 
 size_t sps_smem(bool wide, int nwidths) {
   const size_t span = (size_t)dd::kSpsTile + ((size_t)1 << (nwidths - 1));
-  // V is padded to a whole number of samples per thread (the larger of the kernels' choices)
-  return dd::sps_v_offset(span, wide ? 8 : 4) + (size_t)dd::sps_per(nwidths <= 9 ? 9 : 12) * dd::kSpsThreads * 4;
+  // then two raw-sample buffers (search kernel) / one staging buffer (fill kernel), each padded to a whole number of
+  // samples per thread (the larger of the kernels' choices)
+  return dd::sps_v_offset(span, wide ? 8 : 4) + 2 * (size_t)dd::sps_per(nwidths <= 9 ? 9 : 12) * dd::kSpsThreads * 4;
 }
 
 }  // namespace
@@ -570,10 +630,10 @@ int dd_sps_candidates(const dd_plan_t* p, const float* plane_dev, int32_t nwidth
     const size_t smem = sps_smem(wide, nwidths);
     const dim3 grid((unsigned)r.ndm, (unsigned)p->nbeams);
     if (wide) {
-      e = cudaFuncSetAttribute(dd::dd_sps_fill_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+      e = cudaFuncSetAttribute(dd::dd_sps_fill_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);
       if (e == cudaSuccess) dd::dd_sps_fill_kernel<true><<<grid, dd::kSpsThreads, smem, stream>>>(sp);
     } else {
-      e = cudaFuncSetAttribute(dd::dd_sps_fill_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+      e = cudaFuncSetAttribute(dd::dd_sps_fill_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);
       if (e == cudaSuccess) dd::dd_sps_fill_kernel<false><<<grid, dd::kSpsThreads, smem, stream>>>(sp);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
