@@ -379,24 +379,85 @@ def run_ours(args, w):
         snr = torch.empty((rows, K), dtype=torch.float32, device=dev)
         tmx = torch.empty((rows, K), dtype=torch.int32, device=dev)
         cnt = torch.empty((rows, K), dtype=torch.int32, device=dev)
-        for _ in range(2):
-            plan.sps_execute(out, K, thr, snr, tmx, cnt, stream)
-        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        s0.record(stream)
-        for _ in range(3):
-            plan.sps_execute(out, K, thr, snr, tmx, cnt, stream)
-        s1.record(stream)
-        torch.cuda.synchronize()
-        sps_ms = s0.elapsed_time(s1) / 3
+        offs = torch.empty(rows * K + 1, dtype=torch.int64, device=dev)
+        cand = torch.empty((1 << 20, 4), dtype=torch.int32, device=dev)
+        stats = torch.zeros((rows, 2), dtype=torch.int64, device=dev)
+
+        def timed(fn, reps=5):
+            for _ in range(2):
+                fn()
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            s0.record(stream)
+            for _ in range(reps):
+                fn()
+            s1.record(stream)
+            torch.cuda.synchronize()
+            return s0.elapsed_time(s1) / reps
+
+        plan.set_profiling(0)
+        two_pass_ms = timed(lambda: plan.sps_execute(out, K, thr, snr, tmx, cnt, stream))
+        # row statistics from the dedispersion epilogue (dd_plan_set_row_stats): the search then reads the plane once
+        plan.set_row_stats(stats)
+        exec_stats_ms = timed(lambda: plan.execute(x, out, stream), reps=3)
+        sps_ms = timed(lambda: plan.sps_execute(out, K, thr, snr, tmx, cnt, stream))
+        cand_ms = timed(lambda: plan.sps_candidates(out, K, thr, cnt, offs, cand, cand.shape[0], stream))
+        plan.set_row_stats(None)
         plane_bytes = plan.out_elems() * 4
         hbm = float(peaks.get("hbm_gbs", 6650.0))
         sps = {"kernel": "dd_sps_kernel", "widths": K, "threshold": thr, "ms": sps_ms, "rows": rows,
+               "row_statistics": "from the dedispersion epilogue (dd_plan_set_row_stats): one pass over the plane",
+               "ms_two_pass_without_epilogue_statistics": two_pass_ms, "ms_dd_execute_with_statistics": exec_stats_ms,
+               "ms_candidate_list": cand_ms, "candidates_above_threshold": int(offs[-1].item()),
                "roofline": {"bound": "hbm", "achieved": plane_bytes / (sps_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
                             "frac": plane_bytes / (sps_ms * 1e-3) / 1e9 / hbm,
-                            "algorithmic_bytes": "the DM-time plane read once (4 B per DM-trial sample)"},
-               "candidates_above_threshold": int(cnt.sum().item())}
-        del snr, tmx, cnt
+                            "algorithmic_bytes": "the DM-time plane read once (4 B per DM-trial sample)"}}
+        del snr, tmx, cnt, offs, cand, stats
+
+    # NEXT-4: the pulsar-side chain on the rows of range 0 of the plane just written:
+    # downsample by 8 -> running-median de-reddening (window 129) -> re-sampling; HBM-bound steps except the median
+    post = None
+    if rank == 0 and world == 1 and not args.no_post:
+        try:
+            info = plan.range_info(0)
+            ndm, nout, pitch = info["ndm"], info["nout"], info["pitch"]
+            src = out[info["offset"]:]
+            F, Wn = 8, 129
+            nd = nout // F
+            hbm = float(peaks.get("hbm_gbs", 6650.0))
+            d = torch.empty((ndm, nd), dtype=torch.float32, device=dev)
+            rr = torch.empty((ndm, nd), dtype=torch.float32, device=dev)
+            rs = B.Resample(1.4, -2.0e-4, 0.0, w.tsamp_s * F, nd)
+            rsm = torch.empty((ndm, rs.out_len), dtype=torch.float32, device=dev)
+
+            def timed_post(fn, reps=5):
+                fn()
+                s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                s0.record(stream)
+                for _ in range(reps):
+                    fn()
+                s1.record(stream)
+                torch.cuda.synchronize()
+                return s0.elapsed_time(s1) / reps
+
+            t_ds = timed_post(lambda: B.post_downsample(src, ndm, pitch, nout, F, d, nd, stream))
+            t_md = timed_post(lambda: B.post_dered(d, ndm, nd, nd, Wn, None, rr, nd, stream))
+            t_rs = timed_post(lambda: rs.execute(rr, ndm, nd, rsm, rs.out_len, stream))
+
+            def line(ms, nbytes, bound):
+                return {"ms": ms, "bound": bound, "achieved_gb_s": nbytes / (ms * 1e-3) / 1e9,
+                        "frac_of_hbm_peak": nbytes / (ms * 1e-3) / 1e9 / hbm}
+
+            post = {"rows": ndm, "samples_per_row": nout, "downsample_factor": F, "median_window": Wn,
+                    "downsample": line(t_ds, ndm * (nout + nd) * 4, "hbm"),
+                    "running_median": dict(line(t_md, ndm * nd * 8, "alu (order statistics; HBM bytes shown for scale)"),
+                                           samples_per_s=ndm * nd / (t_md * 1e-3)),
+                    "resample": line(t_rs, ndm * (nd + rs.out_len) * 4, "hbm")}
+            rs.destroy()
+            del d, rr, rsm
+        except Exception as e:
+            post = {"skipped": repr(e)}
 
     # NEXT-3: the exact two-channel sub-band variant, an opt-in shortcut that performs about half the
     # adds of the brute-force count the roofline divides by -- reported beside the metric, never inside `value`
@@ -456,7 +517,7 @@ def run_ours(args, w):
                        "l2": "inputs larger than L2 (1.07 GB input, 4.0 GB packed copy, 3.8 GB output per step)",
                        "parallelism": "replicas: one beam per GPU, no collective"},
             "input_gb_per_s": world * w.nchans * w.nsamps * (w.in_bits // 8) / (ms_total / args.steps * 1e-3) / 1e9,
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps, "subband": subband, "other_configs": other,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps, "post": post, "subband": subband, "other_configs": other,
             "gpu_launches": plan.launches() * args.steps, "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
@@ -476,6 +537,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=0, help="end-to-end steps (0 = as many as --steps)")
     ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--no-subband", action="store_true")
+    ap.add_argument("--no-post", action="store_true")
     ap.add_argument("--variant", type=int, default=0, help="dd_plan_set_kernel variant of the timed plan (measurements)")
     ap.add_argument("--stub-body", action="store_true", help=argparse.SUPPRESS)  # tests: N-rank plumbing on CPU / gloo
     ap.add_argument("--no-e2e", action="store_true")

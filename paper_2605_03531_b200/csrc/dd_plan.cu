@@ -38,6 +38,7 @@ using dd::cuda_fail;
 
 // Dispersion constant of the north_star, s MHz^2 cm^3 / pc  (PAPER.md:258 prints 4.14881 ms GHz^2).
 constexpr double kDispersion = 4.148808e3;
+constexpr int kSmCount = 148;  // B200 (the library is built for sm_100a only); used by the tile cost model
 
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
@@ -164,6 +165,14 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
     cost *= (double)nblocks * D / (double)r.ndm;
     if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
     if (Cc < 16) cost *= 1.0 + 0.05 * (16 / Cc - 1);  // shorter stages synchronise more often
+    {
+      // wave quantisation: a grid that is not a multiple of the SM count leaves SMs idle in its last wave.  It only
+      // matters for short rows (the tail plans of dd_stream_push at 800-spectra blocks: a few dozen CTAs).
+      const int64_t H = round_up((r.nout + r.NL - 1) / r.NL, 16);
+      const int64_t nctas = (int64_t)nblocks * ((H + T - 1) / T) * p.nbeams;
+      const int64_t slots = (int64_t)kSmCount * (G * T == 256 ? 2 : 1);
+      cost *= (double)((nctas + slots - 1) / slots * slots) / (double)nctas;
+    }
     *stages_out = stages;
     *cost_out = cost;
     return true;

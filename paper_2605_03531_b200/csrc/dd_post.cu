@@ -68,95 +68,96 @@ __device__ __forceinline__ float key2f(uint32_t k) {
 __global__ void __launch_bounds__(kMedWarps * 32) dd_running_median_kernel(const float* __restrict__ in, long long in_pitch,
                                                                           long long n, int W, float* __restrict__ med,
                                                                           float* __restrict__ out, long long out_pitch) {
-  extern __shared__ uint32_t keys[];  // keys of samples [base, base + span)
+  extern __shared__ uint32_t keys[];  // keys of samples [base, base + span), then the medians of the tile's outputs
   const int h = (W - 1) / 2;
   const long long t0 = (long long)blockIdx.x * (kMedWarps * kMedSeg);
-  const long long t1 = min(n, t0 + (long long)kMedWarps * kMedSeg);
+  const int nt = (int)min((long long)kMedWarps * kMedSeg, n - t0);  // outputs of this tile
   const float* x = in + (long long)blockIdx.y * in_pitch;
-  auto wstart = [&](long long t) { return min(max(t - h, 0LL), n - W); };
-  const long long base = wstart(t0);
-  const int span = (int)(wstart(t1 - 1) + W - base);
+  // window start of output t (relative to the tile: t = t0 + r) is clamp(t - h, 0, n - W); everything below is in
+  // 32-bit offsets from `base`, the window start of the tile's first output
+  const long long base = min(max(t0 - h, 0LL), n - W);
+  const int smax = (int)(n - W - base);                 // largest window start, relative to base
+  const int off = (int)(t0 - h - base);                 // window start of output r before clamping = r + off
+  const int span = min(max(nt - 1 + off, 0), smax) + W;  // samples staged
+  uint32_t* meds = keys + (kMedWarps * kMedSeg + W);
   for (int i = threadIdx.x; i < span; i += blockDim.x) keys[i] = f2key(__ldg(x + base + i));
   __syncthreads();
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long ts = t0 + (long long)warp * kMedSeg;
-  const long long te = min(t1, ts + kMedSeg);
-  if (ts >= te) return;
-
-  // ---- first window of the segment: radix select of the element of rank h
-  long long s = wstart(ts);
-  const uint32_t* win = keys + (s - base);
-  uint32_t m = 0;
-  for (int b = 31; b >= 0; --b) {
-    const uint32_t trial = m | (1u << b);
-    int c = 0;
-    for (int i = lane; i < W; i += 32) c += win[i] < trial;
-    c = __reduce_add_sync(0xffffffffu, c);
-    if (c <= h) m = trial;  // at most h keys are below `trial`: the rank-h key is >= trial
-  }
-  int below = 0, equal = 0;
-  for (int i = lane; i < W; i += 32) {
-    const uint32_t k = win[i];
-    below += k < m;
-    equal += k == m;
-  }
-  below = __reduce_add_sync(0xffffffffu, below);
-  equal = __reduce_add_sync(0xffffffffu, equal);
-
-  float* orow = out ? out + (long long)blockIdx.y * out_pitch : nullptr;
-  float* mrow = med ? med + (long long)blockIdx.y * out_pitch : nullptr;
-  uint32_t my_m = 0;  // lane l keeps the median of output ts + 32*q + l until the warp stores 32 of them at once
-  for (long long t = ts; t < te; ++t) {
-    const long long sn = wstart(t);
-    if (sn != s) {  // the window moves by one sample: keys[s] leaves, keys[s + W] enters
-      const uint32_t ko = keys[s - base], ki = keys[s - base + W];
-      s = sn;
-      below += (int)(ki < m) - (int)(ko < m);
-      equal += (int)(ki == m) - (int)(ko == m);
-      win = keys + (s - base);
-      if (below > h) {  // exactly h+1 keys below m: the median is the largest of them
-        uint32_t best = 0;
-        int cnt = 0;
-        for (int i = lane; i < W; i += 32) {
-          const uint32_t k = win[i];
-          if (k < m) {
-            cnt = k > best ? 1 : cnt + (k == best);
-            best = max(best, k);
-          }
-        }
-        const uint32_t all = __reduce_max_sync(0xffffffffu, best);
-        cnt = __reduce_add_sync(0xffffffffu, (best == all && cnt > 0) ? cnt : 0);
-        m = all;
-        equal = cnt;
-        below -= cnt;
-      } else if (below + equal <= h) {  // exactly h keys at or below m: the median is the smallest key above m
-        uint32_t best = 0xffffffffu;
-        int cnt = 0;
-        for (int i = lane; i < W; i += 32) {
-          const uint32_t k = win[i];
-          if (k > m) {
-            cnt = k < best ? 1 : cnt + (k == best);
-            best = min(best, k);
-          }
-        }
-        const uint32_t all = __reduce_min_sync(0xffffffffu, best);
-        cnt = __reduce_add_sync(0xffffffffu, (best == all && cnt > 0) ? cnt : 0);
-        below += equal;
-        m = all;
-        equal = cnt;
-      }
+  const int rs = warp * kMedSeg, re = min(nt, rs + kMedSeg);  // this warp's outputs [rs, re) of the tile
+  if (rs < re) {
+    // ---- first window of the segment: radix select of the element of rank h
+    int s = min(max(rs + off, 0), smax);
+    const uint32_t* win = keys + s;
+    uint32_t m = 0;
+    for (int b = 31; b >= 0; --b) {
+      const uint32_t trial = m | (1u << b);
+      int c = 0;
+      for (int i = lane; i < W; i += 32) c += win[i] < trial;
+      c = __reduce_add_sync(0xffffffffu, c);
+      if (c <= h) m = trial;  // at most h keys are below `trial`: the rank-h key is >= trial
     }
-    const int slot = (int)((t - ts) & 31);
-    if (lane == slot) my_m = m;
-    if (slot == 31 || t == te - 1) {  // coalesced store of up to 32 outputs
-      const long long tt = t - slot + lane;
-      if (lane <= slot) {
-        const float mv = key2f(my_m);
-        if (mrow) mrow[tt] = mv;
-        if (orow) orow[tt] = __fsub_rn(key2f(keys[tt - base]), mv);
-      }
+    int below = 0, equal = 0;
+    for (int i = lane; i < W; i += 32) {
+      const uint32_t k = win[i];
+      below += k < m;
+      equal += k == m;
     }
+    below = __reduce_add_sync(0xffffffffu, below);
+    equal = __reduce_add_sync(0xffffffffu, equal);
+    if (lane == 0) meds[rs] = m;
+    for (int r = rs + 1; r < re; ++r) {
+      const int sn = min(max(r + off, 0), smax);
+      if (sn != s) {  // the window moves by one sample: keys[s] leaves, keys[s + W] enters
+        const uint32_t ko = keys[s], ki = keys[s + W];
+        s = sn;
+        below += (int)(ki < m) - (int)(ko < m);
+        equal += (int)(ki == m) - (int)(ko == m);
+        win = keys + s;
+        if (below > h) {  // exactly h+1 keys below m: the median is the largest of them
+          uint32_t best = 0;
+          int cnt = 0;
+          for (int i = lane; i < W; i += 32) {
+            const uint32_t k = win[i];
+            if (k < m) {
+              cnt = k > best ? 1 : cnt + (k == best);
+              best = max(best, k);
+            }
+          }
+          const uint32_t all = __reduce_max_sync(0xffffffffu, best);
+          cnt = __reduce_add_sync(0xffffffffu, (best == all && cnt > 0) ? cnt : 0);
+          m = all;
+          equal = cnt;
+          below -= cnt;
+        } else if (below + equal <= h) {  // exactly h keys at or below m: the median is the smallest key above m
+          uint32_t best = 0xffffffffu;
+          int cnt = 0;
+          for (int i = lane; i < W; i += 32) {
+            const uint32_t k = win[i];
+            if (k > m) {
+              cnt = k < best ? 1 : cnt + (k == best);
+              best = min(best, k);
+            }
+          }
+          const uint32_t all = __reduce_min_sync(0xffffffffu, best);
+          cnt = __reduce_add_sync(0xffffffffu, (best == all && cnt > 0) ? cnt : 0);
+          below += equal;
+          m = all;
+          equal = cnt;
+        }
+      }
+      if (lane == 0) meds[r] = m;
+    }
+  }
+  __syncthreads();
+  // coalesced stores of the tile: median and sample minus median (the sample of output r sits at keys[r + t0 - base])
+  float* orow = out ? out + (long long)blockIdx.y * out_pitch + t0 : nullptr;
+  float* mrow = med ? med + (long long)blockIdx.y * out_pitch + t0 : nullptr;
+  const int xoff = (int)(t0 - base);
+  for (int r = threadIdx.x; r < nt; r += blockDim.x) {
+    const float mv = key2f(meds[r]);
+    if (mrow) mrow[r] = mv;
+    if (orow) orow[r] = __fsub_rn(key2f(keys[r + xoff]), mv);
   }
 }
 
@@ -165,24 +166,30 @@ __global__ void __launch_bounds__(kMedWarps * 32) dd_running_median_kernel(const
 // recurrence of Eq 3.3; out[k] = fl32( sum_i x[i] * |[u_k, u_{k+1}) n [i, i+1)| ), accumulated left to right in
 // double with explicitly rounded operations (no FMA).  rev: the series is read backwards and written backwards.
 // ------------------------------------------------------------------------------------------------------------
+constexpr int kResampleRows = 4;  // rows per thread: the bin edges (doubles, shared by all rows) are loaded once for four rows
 __global__ void __launch_bounds__(256) dd_resample_kernel(const float* __restrict__ in, long long in_pitch, long long n,
-                                                          const double* __restrict__ u, long long M, int rev,
+                                                          const double* __restrict__ u, long long M, int rev, long long nrows,
                                                           float* __restrict__ out, long long out_pitch) {
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= M) return;
-  const float* x = in + (long long)blockIdx.y * in_pitch;
-  auto X = [&](long long i) { return (double)__ldg(x + (rev ? n - 1 - i : i)); };
   const double a = u[k], b = u[k + 1];
   const long long i0 = (long long)floor(a), i1 = (long long)floor(b);
-  double s;
-  if (i0 == i1) {
-    s = __dmul_rn(X(i0), __dsub_rn(b, a));
-  } else {
-    s = __dmul_rn(X(i0), __dsub_rn((double)(i0 + 1), a));
-    for (long long i = i0 + 1; i < i1; ++i) s = __dadd_rn(s, X(i));
-    if (i1 < n) s = __dadd_rn(s, __dmul_rn(X(i1), __dsub_rn(b, (double)i1)));
+  const double f0 = i0 == i1 ? __dsub_rn(b, a) : __dsub_rn((double)(i0 + 1), a);  // weight of the first input bin
+  const double f1 = __dsub_rn(b, (double)i1);                                       // weight of the last one (i1 > i0)
+  const long long r0 = (long long)blockIdx.y * kResampleRows;
+#pragma unroll
+  for (int q = 0; q < kResampleRows; ++q) {
+    const long long r = r0 + q;
+    if (r >= nrows) break;
+    const float* x = in + r * in_pitch;
+    auto X = [&](long long i) { return (double)__ldg(x + (rev ? n - 1 - i : i)); };
+    double s = __dmul_rn(X(i0), f0);
+    if (i0 != i1) {
+      for (long long i = i0 + 1; i < i1; ++i) s = __dadd_rn(s, X(i));
+      if (i1 < n) s = __dadd_rn(s, __dmul_rn(X(i1), f1));
+    }
+    out[r * out_pitch + (rev ? M - 1 - k : k)] = __double2float_rn(s);
   }
-  out[(long long)blockIdx.y * out_pitch + (rev ? M - 1 - k : k)] = __double2float_rn(s);
 }
 
 }  // namespace dd
@@ -273,7 +280,7 @@ int dd_post_dered(const float* in_dev, int64_t nrows, int64_t in_pitch, int64_t 
       window > DD_POST_MAX_WINDOW || in_pitch < n || out_pitch < n)
     return DD_ERR_INVALID;
   if (nrows == 0) return DD_OK;
-  const size_t smem = (size_t)(dd::kMedWarps * dd::kMedSeg + window) * sizeof(uint32_t);
+  const size_t smem = (size_t)(2 * dd::kMedWarps * dd::kMedSeg + window) * sizeof(uint32_t);
   cudaError_t e = cudaFuncSetAttribute(dd::dd_running_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   if (e != cudaSuccess) return dd::cuda_fail(e, "cudaFuncSetAttribute(dd_running_median_kernel)");
   for (int64_t r0 = 0; r0 < nrows; r0 += kMaxGridRows) {
@@ -342,10 +349,11 @@ int dd_resample_execute(const dd_resample_t* r, const float* in_dev, int64_t nro
   int rc = check_device(r->device);
   if (rc != DD_OK) return rc;
   if (nrows == 0 || r->M == 0) return DD_OK;
-  for (int64_t r0 = 0; r0 < nrows; r0 += kMaxGridRows) {
-    dim3 grid((unsigned)((r->M + 255) / 256), (unsigned)std::min<int64_t>(kMaxGridRows, nrows - r0));
+  for (int64_t r0 = 0; r0 < nrows; r0 += kMaxGridRows * dd::kResampleRows) {
+    const int64_t nr = std::min<int64_t>(kMaxGridRows * dd::kResampleRows, nrows - r0);
+    dim3 grid((unsigned)((r->M + 255) / 256), (unsigned)((nr + dd::kResampleRows - 1) / dd::kResampleRows));
     dd::dd_resample_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
-        in_dev + r0 * in_pitch, in_pitch, r->n, r->d_edges, r->M, r->reversed, out_dev + r0 * out_pitch, out_pitch);
+        in_dev + r0 * in_pitch, in_pitch, r->n, r->d_edges, r->M, r->reversed, nr, out_dev + r0 * out_pitch, out_pitch);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return dd::cuda_fail(e, "dd_resample_kernel launch");
   }

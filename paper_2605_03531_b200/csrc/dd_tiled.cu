@@ -413,7 +413,9 @@ struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upp
 // ------------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------------
-template <int NL, int MODE, int NT>
+// STATS: also accumulate sum x and sum x^2 of every row written (dd_plan_set_row_stats); a separate instantiation so
+// that the default kernel keeps its register allocation (measured: 0.4 % on config 3 with a run-time flag)
+template <int NL, int MODE, int NT, bool STATS = false>
 __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParams p) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int tid = threadIdx.x;
@@ -540,8 +542,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
 
   // ---------------- a4: DM-time writer, fp32 (I2F rounds to nearest even) -------------------------
   const long long i = tau * p.T + ti;
-  const bool active = i < p.H;  // (threads past the lane segment keep running: the row statistics reduce over whole warps)
-  if (!active && !p.stats) return;
+  const bool active = i < p.H;  // (with STATS threads past the lane segment keep running: the sums reduce over whole warps)
+  if (!active && !STATS) return;
   float* obase = p.out + (long long)beam * p.out_beam_stride;
 #pragma unroll
   for (int j = 0; j < RD; ++j) {
@@ -554,18 +556,20 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
 #pragma unroll
     for (int m = 0; m < NL; ++m) {
       const long long t = i + (long long)m * p.H;  // consecutive threads -> consecutive floats
-      if (active && t < p.nout) {
+      if ((!STATS || active) && t < p.nout) {
         // second byte plane of uint16 input: S = S_lo + 256*S_hi.  Both plane sums are < 2^24, hence exact
         // floats, and the fused multiply-add rounds the exact total once: fl32(S), as the definition asks.
         if (p.accum_scale != 0.0f)
           orow[t] = __fmaf_rn(__uint2float_rn(v[m]), p.accum_scale, orow[t]);
         else
           orow[t] = __uint2float_rn(v[m]);
-        s1 += v[m];
-        s2 += (unsigned long long)v[m] * v[m];
+        if constexpr (STATS) {
+          s1 += v[m];
+          s2 += (unsigned long long)v[m] * v[m];
+        }
       }
     }
-    if (p.stats) {  // sum x, sum x^2 of this row's piece: one pair of atomics per warp and trial (exact integers)
+    if constexpr (STATS) {  // sum x, sum x^2 of this row's piece: one pair of atomics per warp and trial (exact integers)
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
         s1 += __shfl_down_sync(0xffffffffu, s1, o);
@@ -585,12 +589,21 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
 // ------------------------------------------------------------------------------------------------
 template <int NL, int MODE, int NT>
 static cudaError_t launch_tiled_t(const TiledParams& tp, long long nctas, size_t smem, cudaStream_t stream) {
-  dd_tiled_kernel<NL, MODE, NT><<<(unsigned)nctas, NT, smem, stream>>>(tp);
+  if (tp.stats) {
+    if constexpr (NL != 16)  // (row statistics are offered for uint8 input only, whose byte-lane ranges have one plane)
+      dd_tiled_kernel<NL, MODE, NT, true><<<(unsigned)nctas, NT, smem, stream>>>(tp);
+    else
+      dd_tiled_kernel<16, MODE, NT, true><<<(unsigned)nctas, NT, smem, stream>>>(tp);
+  } else {
+    dd_tiled_kernel<NL, MODE, NT><<<(unsigned)nctas, NT, smem, stream>>>(tp);
+  }
   return cudaGetLastError();
 }
 
 template <int NL, int MODE, int NT>
 static cudaError_t set_smem_t() {
+  cudaError_t e = cudaFuncSetAttribute(dd_tiled_kernel<NL, MODE, NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(dd_tiled_kernel<NL, MODE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
