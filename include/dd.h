@@ -129,7 +129,9 @@ int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out);
  * shape.  tuning == NULL means automatic.  (The library reads no environment variables.)
  *   mode        -1 automatic; 0 / 1 / 2 force the table form of the tiled kernel (see dd_plan_tile_info); the delta
  *               form is refused (falls back to 0) for a range with a delay step above 1 between neighbouring trials
- *   byte_lanes  -1 or 1 automatic; 0: never use 8-bit lanes (undecimated coarse ranges then run on 16-/32-bit lanes)
+ *   byte_lanes  -1 automatic; 1: 8-bit lanes wherever they apply, uint16 input as two byte planes (automatic for uint8;
+ *               undecimated uint16 input automatically runs on uint16 lanes instead, table form 5); 0: never use 8-bit or
+ *               uint16 lanes (undecimated coarse ranges then run on 16-/32-bit lanes with the table forms 0 / 1)
  *   trial_groups, words_per_cta, chans_per_stage, stages
  *               all 0: automatic; else the CTA shape: trial_groups * words_per_cta in {256, 512} threads,
  *               words_per_cta a multiple of 32, chans_per_stage in {4, 8, .., 32}, 2 <= stages <= 8.  A shape that
@@ -210,10 +212,11 @@ int dd_plan_set_workspace(dd_plan_t* plan, void* dev, int64_t bytes);
 /* Choose the dedispersion kernel variant (DD_KERNEL_*).  All variants produce identical bits. */
 int dd_plan_set_kernel(dd_plan_t* plan, int32_t variant);
 /* Tile shape the tiled kernel uses for range r (any pointer may be NULL): trials per CTA, packed time
- * words per CTA, time lanes per packed word (8 = 16-bit lanes, 4 = 32-bit lanes), channels between
- * flushes of the packed accumulators, and the table mode: 0 = one shared-memory load per (channel, trial),
+ * words per CTA, time lanes per packed word (16 = 8-bit lanes, 8 = 16-bit lanes, 4 = 32-bit lanes), channels between
+ * flushes of the packed accumulators (0: never), and the table mode: 0 = one shared-memory load per (channel, trial),
  * 1 = load skipped when the delay equals the previous trial's, 2 = delta form (all delay steps inside a
- * group of 8 trials are 0 or 1; one changed bit per trial). */
+ * group of 8 trials are 0 or 1; one changed bit per trial), 5 = uint16 samples in the 16-bit lanes (undecimated
+ * uint16 input; 32-bit byte offsets, load skipped on equal offsets). */
 int dd_plan_tile_info(const dd_plan_t* plan, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta,
                       int32_t* lanes, int32_t* flush_chans, int32_t* mode);
 

@@ -40,7 +40,11 @@ __host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? 
 //                      interleaved: superword 2i + p) replace both channels: one load and one add per trial and PAIR.
 //                      Table per quad of pairs: one "changed" bit per trial step and pair as in kModeDelta, plus a byte
 //                      offset per trial and pair that selects the row (U_0 or U_1) and the delay.
-enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3, kModeDeltaPair = 4 };
+//   kModeWide          uint16 samples in the 16-bit lanes of NL = 8 (undecimated uint16 input on coarse DM grids): a lane has no
+//                      headroom, so a word w of two lanes is accumulated as E += w (mod 2^32) and O += w >> 16; lane sums are
+//                      E - (O << 16) and O.  Table: eight 32-bit byte offsets inside the stage (row included) per (channel,
+//                      trial group); the load is skipped when the offset equals the previous trial's.
+enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3, kModeDeltaPair = 4, kModeWide = 5 };
 __host__ __device__ constexpr bool is_delta(int mode) {
   return mode == kModeDelta || mode == kModeDeltaShare || mode == kModeDeltaPair;
 }
@@ -59,6 +63,7 @@ __host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 
 // included -- or one 16-byte entry per channel quad in delta mode.
 __host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int NL, int Cc, int G) {
   if (mode == 4) return (size_t)(Cc / 8) * (size_t)G * 80;  // kModeDeltaPair: 5 entries per quad of pairs (8 rows)
+  if (mode == 5) return (size_t)Cc * (size_t)G * 32;        // kModeWide: eight 32-bit byte offsets per (channel, trial group)
   return (size_t)(is_delta(mode) ? Cc / 4 : Cc) * (size_t)G * 16;
 }
 

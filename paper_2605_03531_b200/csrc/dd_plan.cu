@@ -138,7 +138,14 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
   // sample (the bound of the offsets-table modes), uint16 input as two byte planes.  dd_tuning_t::byte_lanes = 0
   // switches it off.
   const int flush16 = 65280 / 255;
-  if (r.decim == 1 && r.mode != dd::kModeDelta && (int64_t)p.nchans <= (int64_t)120 * flush16 && tune.byte_lanes != 0) {
+  if (p.in_bits == 16 && r.decim == 1 && r.mode != dd::kModeDelta && tune.byte_lanes < 0) {
+    // undecimated uint16 input on a coarse grid: the samples themselves in 16-bit lanes (kModeWide).  Shared memory
+    // delivers 2 bytes per add either way, but one pass with 1.5 ALU instructions per two adds replaces two byte-plane
+    // passes of the 8-bit-lane kernel.  dd_tuning_t::byte_lanes = 1 keeps the two byte planes, 0 the 32-bit lanes.
+    r.NL = 8;
+    r.flush = 0;
+    r.mode = dd::kModeWide;
+  } else if (r.decim == 1 && r.mode != dd::kModeDelta && (int64_t)p.nchans <= (int64_t)120 * flush16 && tune.byte_lanes != 0) {
     r.NL = 16;
     r.flush = flush16;
     r.mode = dd::kModeGeneral;
@@ -258,7 +265,7 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
   dmin.assign(nbc, 0);
   span.assign(nbc, 0);
   const bool delta = r.mode == dd::kModeDelta;
-  const size_t words_per_entry = 4;
+  const size_t words_per_entry = r.mode == dd::kModeWide ? 8 : 4;
   const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
   std::vector<uint32_t>& meta = r.h_meta;
   meta.assign(nentries * words_per_entry, 0);
@@ -285,7 +292,7 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
             }
         } else {
           uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * words_per_entry];
-          if (r.NL == 16) {  // byte offsets inside the stage, row of the channel included
+          if (r.NL == 16 || r.mode == dd::kModeWide) {  // byte offsets inside the stage, row of the channel included
             for (int j = 0; j < r.RD; ++j)
               e[j] = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg + j, c) - d0)) * 16u;
           } else {

@@ -75,6 +75,7 @@ struct TiledParams {
   int blk0, nblk;    // trial blocks of this launch: blk0 .. blk0 + nblk - 1
   int rowpitch;      // superwords per staged row = T + Smax
   int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
+  uint32_t one;       // 1: a multiplier ptxas cannot fold, keeps integer adds on the FMA-side pipe as IMAD (add_bytes)
   float accum_scale;  // 0: store; else out = value * accum_scale + out (high byte plane of uint16 input)
   unsigned long long* stats;  // nullptr, or [beam][trial of this range][2]: sum x and sum x^2 of the rows written (dd_plan_set_row_stats)
   long long stats_beam_stride;
@@ -267,27 +268,75 @@ __device__ __forceinline__ void stage_pairs(uint4 (&acc)[kRD], uint32_t sdata, u
   }
 }
 
+// uint16 lanes (kModeWide, NL = 8): a word w holds two uint16 samples with no headroom.  E += w (mod 2^32; one IADD3 for
+// two channels) and O += w >> 16 (one LEA.HI per channel) give the lane sums E - (O << 16) and O, exact while the channel
+// sum fits 32 bits (checked at plan creation).  Channels in pairs; per channel and trial group two table entries = eight
+// 32-bit byte offsets inside the stage (row included); a trial whose offset equals the previous trial's keeps the
+// registers (upper channels of a coarse grid still repeat delays).  Bound by shared memory: 2 bytes per add.
+__device__ __forceinline__ void add_wide(uint4& E, uint4& O, const uint4& a, const uint4& b) {
+  E.x = E.x + a.x + b.x, E.y = E.y + a.y + b.y, E.z = E.z + a.z + b.z, E.w = E.w + a.w + b.w;
+  O.x += a.x >> 16, O.y += a.y >> 16, O.z += a.z >> 16, O.w += a.w >> 16;
+  asm volatile("" : "+r"(O.x), "+r"(O.y), "+r"(O.z), "+r"(O.w));  // keeps each shift-add one LEA.HI
+  O.x += b.x >> 16, O.y += b.y >> 16, O.z += b.z >> 16, O.w += b.w >> 16;
+}
+__device__ __forceinline__ uint32_t word_of(const uint4& m, int j) { return j == 0 ? m.x : j == 1 ? m.y : j == 2 ? m.z : m.w; }
+
+__device__ __forceinline__ void stage_wide(uint4 (&E)[kRD], uint4 (&O)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
+                                           uint32_t meta_row) {
+#pragma unroll 1
+  for (int cc = 0; cc < Cc; cc += 2) {
+    uint4 ma[2], mb[2];
+    lds_sw(ma[0], smeta), lds_sw(ma[1], smeta + 16);
+    lds_sw(mb[0], smeta + meta_row), lds_sw(mb[1], smeta + meta_row + 16);
+    smeta += 2 * meta_row;
+    uint4 wa, wb;
+    uint32_t pa = ma[0].x, pb = mb[0].x;
+    lds_sw(wa, sdata + pa);
+    lds_sw(wb, sdata + pb);
+    add_wide(E[0], O[0], wa, wb);
+#pragma unroll
+    for (int j = 1; j < kRD; ++j) {
+      const uint32_t oa = word_of(ma[j >> 2], j & 3), ob = word_of(mb[j >> 2], j & 3);
+      lds_if_ne(wa, sdata + oa, oa, pa);
+      lds_if_ne(wb, sdata + ob, ob, pb);
+      pa = oa, pb = ob;
+      add_wide(E[j], O[j], wa, wb);
+    }
+  }
+}
+
 // 8-bit lanes (NL = 16): channels in pairs, one table entry (kRD16 32-bit byte offsets) per channel.
 // A loaded word w holds the bytes b0..b3 of four time lanes.  Two accumulators per word:
-//   e += w & 0x00ff00ff            two 16-bit lanes: A0 | A2 << 16 (sums of b0 and b2)   LOP3 + half an IADD3 per channel
-//   r += w >> 8                    = A1 + 2^8 A2 + 2^16 A3  (mod 2^32)                    one LEA.HI per channel
+//   e += w & 0x00ff00ff            two 16-bit lanes: A0 | A2 << 16 (sums of b0 and b2)   LOP3 (ALU pipe) + IMAD (FMA-side pipe)
+//   r += w >> 8                    = A1 + 2^8 A2 + 2^16 A3  (mod 2^32)                    one LEA.HI (ALU pipe)
 // A2 is known from e, so r - (A2 << 8) = A1 + 2^16 A3 separates exactly as long as every lane sum stays below
 // 2^16 (upper bytes moved out every 256 channels, as for the 16-bit lanes); wrap-around of r is harmless.
-// (Measured alternatives: the shift-add as IMAD.HI or IMAD.WIDE on the idle FMA pipe is slower -- ptxas adds
-// register moves or splits it into a multiply plus 64-bit adds.)
-__device__ __forceinline__ void add_bytes(uint4& e, uint4& r, const uint4& a, const uint4& b) {
-  e.x = e.x + (a.x & 0x00ff00ffu) + (b.x & 0x00ff00ffu);
-  e.y = e.y + (a.y & 0x00ff00ffu) + (b.y & 0x00ff00ffu);
-  e.z = e.z + (a.z & 0x00ff00ffu) + (b.z & 0x00ff00ffu);
-  e.w = e.w + (a.w & 0x00ff00ffu) + (b.w & 0x00ff00ffu);
-  r.x = r.x + (a.x >> 8) + (b.x >> 8);
-  r.y = r.y + (a.y >> 8) + (b.y >> 8);
-  r.z = r.z + (a.z >> 8) + (b.z >> 8);
-  r.w = r.w + (a.w >> 8) + (b.w >> 8);
+// The kernel is bound by the ALU pipe (LOP3, LEA.HI, IADD3 all issue there at 2 warp-instructions / clk / SM), so the
+// add of the masked word runs on the otherwise idle FMA-side pipe as an IMAD whose multiplier is a kernel parameter
+// holding 1 (ptxas folds a literal 1 back into an IADD3): 2 ALU + 1 FMA instruction per word instead of 2.5 ALU.
+// Measured (configs 2 / 5): 5.73 -> 5.08 ms / 336.7 -> 297.8 ms; with the two shift-adds forced to stay LEA.HI
+// (ptxas otherwise forms SHF + LEA.HI + IMAD.IADD, one more issue slot per pair of words) 4.90 / 286.6 ms.
+// (Measured alternatives: the shift-add as IMAD.HI or IMAD.WIDE is slower -- ptxas adds register moves or splits it
+// into a multiply plus 64-bit adds; lanes 1 and 3 of one word in four by IDP4A with one-hot selectors into plain
+// 32-bit sums, which takes two more instructions off the ALU pipe, is slower too: 5.03 / 294.0 ms.)
+__device__ __forceinline__ uint32_t mad1(uint32_t t, uint32_t one, uint32_t e) {
+  uint32_t d;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(t), "r"(one), "r"(e));
+  return d;
+}
+__device__ __forceinline__ void add_bytes(uint4& e, uint4& r, const uint4& a, const uint4& b, uint32_t one) {
+  e.x = mad1(b.x & 0x00ff00ffu, one, mad1(a.x & 0x00ff00ffu, one, e.x));
+  e.y = mad1(b.y & 0x00ff00ffu, one, mad1(a.y & 0x00ff00ffu, one, e.y));
+  e.z = mad1(b.z & 0x00ff00ffu, one, mad1(a.z & 0x00ff00ffu, one, e.z));
+  e.w = mad1(b.w & 0x00ff00ffu, one, mad1(a.w & 0x00ff00ffu, one, e.w));
+  // two dependent (x >> 8) + r steps, kept apart so that each stays one LEA.HI
+  r.x += a.x >> 8, r.y += a.y >> 8, r.z += a.z >> 8, r.w += a.w >> 8;
+  asm volatile("" : "+r"(r.x), "+r"(r.y), "+r"(r.z), "+r"(r.w));
+  r.x += b.x >> 8, r.y += b.y >> 8, r.z += b.z >> 8, r.w += b.w >> 8;
 }
 
 __device__ __forceinline__ void stage_bytes(uint4 (&e)[kRD16], uint4 (&r)[kRD16], uint32_t sdata, uint32_t smeta, int Cc,
-                                            uint32_t meta_row) {
+                                            uint32_t meta_row, uint32_t one) {
 #pragma unroll 1
   for (int cc = 0; cc < Cc; cc += 2) {
     uint4 ma, mb;  // byte offsets of the four trials inside the stage (row included): one add per address
@@ -295,10 +344,10 @@ __device__ __forceinline__ void stage_bytes(uint4 (&e)[kRD16], uint4 (&r)[kRD16]
     lds_sw(mb, smeta + meta_row);
     smeta += 2 * meta_row;
     uint4 xa, xb;
-    lds_sw(xa, sdata + ma.x), lds_sw(xb, sdata + mb.x), add_bytes(e[0], r[0], xa, xb);
-    lds_sw(xa, sdata + ma.y), lds_sw(xb, sdata + mb.y), add_bytes(e[1], r[1], xa, xb);
-    lds_sw(xa, sdata + ma.z), lds_sw(xb, sdata + mb.z), add_bytes(e[2], r[2], xa, xb);
-    lds_sw(xa, sdata + ma.w), lds_sw(xb, sdata + mb.w), add_bytes(e[3], r[3], xa, xb);
+    lds_sw(xa, sdata + ma.x), lds_sw(xb, sdata + mb.x), add_bytes(e[0], r[0], xa, xb, one);
+    lds_sw(xa, sdata + ma.y), lds_sw(xb, sdata + mb.y), add_bytes(e[1], r[1], xa, xb, one);
+    lds_sw(xa, sdata + ma.z), lds_sw(xb, sdata + mb.z), add_bytes(e[2], r[2], xa, xb, one);
+    lds_sw(xa, sdata + ma.w), lds_sw(xb, sdata + mb.w), add_bytes(e[3], r[3], xa, xb, one);
   }
 }
 
@@ -327,13 +376,14 @@ struct Lanes<4> {  // four 32-bit lanes: plain sums
     for (int j = 0; j < kRD; ++j) acc[j] = make_uint4(0, 0, 0, 0);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row, uint32_t one) {
     if constexpr (is_delta(MODE))
       stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
     else
       stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
   }
   __device__ __forceinline__ void flush() {}
+  template <int MODE>
   __device__ __forceinline__ void values(int j, uint32_t (&v)[4]) const {
     v[0] = acc[j].x, v[1] = acc[j].y, v[2] = acc[j].z, v[3] = acc[j].w;
   }
@@ -347,8 +397,10 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
     for (int j = 0; j < kRD; ++j) acc[j] = hi[j] = make_uint4(0, 0, 0, 0);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
-    if constexpr (MODE == kModeDeltaPair)
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row, uint32_t one) {
+    if constexpr (MODE == kModeWide)
+      stage_wide(acc, hi, sdata, smeta, Cc, meta_row);  // acc = E, hi = O
+    else if constexpr (MODE == kModeDeltaPair)
       stage_pairs(acc, sdata, smeta, Cc, meta_row);
     else if constexpr (is_delta(MODE))
       stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
@@ -359,8 +411,14 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
 #pragma unroll
     for (int j = 0; j < kRD; ++j) carry_save(acc[j], hi[j]);
   }
+  template <int MODE>
   __device__ __forceinline__ void values(int j, uint32_t (&v)[8]) const {
     const uint32_t lo[4] = {acc[j].x, acc[j].y, acc[j].z, acc[j].w}, up[4] = {hi[j].x, hi[j].y, hi[j].z, hi[j].w};
+    if constexpr (MODE == kModeWide) {  // acc = E = sum of the words, hi = O = sum of their upper halves
+#pragma unroll
+      for (int q = 0; q < 4; ++q) v[2 * q] = lo[q] - (up[q] << 16), v[2 * q + 1] = up[q];
+      return;
+    }
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       v[2 * q] = (lo[q] & 0xffffu) + ((up[q] & 0xffffu) << 8);
@@ -377,8 +435,8 @@ struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upp
     for (int j = 0; j < kRD16; ++j) e[j] = r[j] = he[j] = hq[j] = make_uint4(0, 0, 0, 0);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row) {
-    stage_bytes(e, r, sdata, smeta, Cc, meta_row);
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row, uint32_t one) {
+    stage_bytes(e, r, sdata, smeta, Cc, meta_row, one);
   }
   // invariant: e = A0 | A2 << 16,  r = A1 + 2^8 A2 + 2^16 A3 (mod 2^32),  lane sum = A + 256 * (he | hq lane)
   static __device__ __forceinline__ void flush_word(uint32_t& e, uint32_t& r, uint32_t& he, uint32_t& hq) {
@@ -396,6 +454,7 @@ struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upp
       flush_word(e[j].w, r[j].w, he[j].w, hq[j].w);
     }
   }
+  template <int MODE>
   __device__ __forceinline__ void values(int j, uint32_t (&v)[16]) const {
     const uint32_t ew[4] = {e[j].x, e[j].y, e[j].z, e[j].w}, rw[4] = {r[j].x, r[j].y, r[j].z, r[j].w};
     const uint32_t hew[4] = {he[j].x, he[j].y, he[j].z, he[j].w}, hqw[4] = {hq[j].x, hq[j].y, hq[j].z, hq[j].w};
@@ -512,7 +571,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   Lanes<NL> lanes;
   lanes.init();
   const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
-  const uint32_t entry_bytes = MODE == kModeDeltaPair ? 80u : 16u;  // table bytes per (channel | quad, trial group)
+  const uint32_t entry_bytes = MODE == kModeDeltaPair ? 80u : MODE == kModeWide ? 32u : 16u;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
   const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
@@ -527,14 +586,14 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     }
     mbar_wait(bar_base + 8u * s, ph);
     const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
-    lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row);
+    lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row, p.one);
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_base + 8u * (nstages + s));  // stage may be refilled
     if (++s == nstages) {
       s = 0;
       ph ^= 1u;
     }
-    if (NL != 4 && ++since_flush == p.flush_stages) {  // packed lanes could overflow next: move their upper bytes
+    if (NL != 4 && MODE != kModeWide && ++since_flush == p.flush_stages) {  // packed lanes could overflow next: move their upper bytes
       since_flush = 0;
       lanes.flush();
     }
@@ -551,7 +610,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     if (jj >= p.ndm) break;  // warp-uniform
     float* orow = obase + (long long)jj * p.pitch;
     uint32_t v[NL];
-    lanes.values(j, v);
+    lanes.template values<MODE>(j, v);
     unsigned long long s1 = 0, s2 = 0;
 #pragma unroll
     for (int m = 0; m < NL; ++m) {
@@ -611,7 +670,7 @@ static cudaError_t set_smem_t() {
   X(8, kModeGeneral, 256) X(8, kModeGeneralReuse, 256) X(8, kModeDelta, 256)                   \
   X(8, kModeGeneral, 512) X(8, kModeGeneralReuse, 512) X(8, kModeDelta, 512)                   \
   X(8, kModeDeltaShare, 256) X(8, kModeDeltaShare, 512) X(4, kModeDeltaShare, 256) X(4, kModeDeltaShare, 512) \
-  X(8, kModeDeltaPair, 256) X(8, kModeDeltaPair, 512)                                           \
+  X(8, kModeDeltaPair, 256) X(8, kModeDeltaPair, 512) X(8, kModeWide, 256) X(8, kModeWide, 512)  \
   X(4, kModeGeneral, 256) X(4, kModeGeneralReuse, 256) X(4, kModeDelta, 256)                   \
   X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)                   \
   X(16, kModeGeneral, 256) X(16, kModeGeneral, 512)
@@ -651,6 +710,7 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.rowpitch = pairs ? r.T + r.Smax2 : r.T + r.Smax;
   tp.stats = (p->row_stats && r.planes == 1) ? p->row_stats + 2 * r.row0 : nullptr;
   tp.stats_beam_stride = 2 * p->rows_per_beam;
+  tp.one = 1u;
   tp.flush_stages = r.flush > 0 ? r.flush / r.Cc : 0;  // pairs: a stage holds Cc/2 pair sums of twice the size: same interval
   const long long nctas = (long long)nblk * r.ntau * p->nbeams;
   if (nctas <= 0 || nctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;

@@ -64,8 +64,8 @@ def test_cfg4_shaped_uint16(variant):
     assert want[0][0].max() > 2 ** 24        # the inexact regime is exercised
     plan, flat = gpu_run(w, x, variant)
     check_full(w, x, plan, flat, want)
-    if variant == TILED:   # x1 range: two byte planes of 8-bit lanes; x8 range: 32-bit lanes
-        assert plan.tile_info(0)["lanes"] == 16 and plan.tile_info(1)["lanes"] == 4
+    if variant == TILED:   # x1 range: uint16 lanes (table form 5); x8 range: 32-bit lanes
+        assert plan.tile_info(0)["lanes"] == 8 and plan.tile_info(0)["mode"] == 5 and plan.tile_info(1)["lanes"] == 4
 
 
 def test_uint16_extreme_values_exact_rounding():
@@ -256,13 +256,19 @@ def test_byte_lanes_coarse_dm_grid(bits):
     x[0, 100:420, :] = 2 ** bits - 1
     x[1, ::3, 500:9000] = 2 ** bits - 1
     w = W.Workload("bytes", 750.0, -200.0 / nch, nch, 655.36e-6, ns, 2, bits, (W.DMRange(0.0, 3.0, 70, 1),), 1, 0, 0)
-    plan, flat = gpu_run(w, x, TILED)
+    plan, flat = gpu_run(w, x, TILED, tuning=dict(byte_lanes=1))
     assert plan.tile_info(0)["lanes"] == 16 and plan.tile_info(0)["mode"] == 0
     assert plan.launches() == 1 + bits // 8
     check_full(w, x, plan, flat)
     plan2, flat2 = gpu_run(w, x, TILED, tuning=dict(byte_lanes=0))
     assert plan2.tile_info(0)["lanes"] == (8 if bits == 8 else 4)
     assert np.array_equal(flat.view(np.uint32)[flat != -1.0], flat2.view(np.uint32)[flat2 != -1.0])
+    # automatic choice: byte lanes for uint8; uint16 samples in 16-bit lanes (E / O accumulators, table form 5)
+    plan3, flat3 = gpu_run(w, x, TILED)
+    info = plan3.tile_info(0)
+    assert (info["lanes"], info["mode"]) == ((16, 0) if bits == 8 else (8, 5))
+    assert plan3.launches() == 2
+    assert np.array_equal(flat.view(np.uint32)[flat != -1.0], flat3.view(np.uint32)[flat3 != -1.0])
 
 
 @pytest.mark.parametrize("bits", [8, 16])

@@ -55,8 +55,8 @@ def _decode(plan, r):
                 rel[:, :, j, q::4] = cur.transpose(0, 2, 1)
         assert np.array_equal(anyb, e[..., 3]), "any-changed bits are the OR of the quad's changed bits"
         assert (e[..., 0] & 0x80808080 == 0).all()                            # bit 7 of each byte is unused
-    elif info["lanes"] == 16:                                                 # 32-bit byte offsets, row included
-        e = meta.reshape(nb, cpad, g, 4).astype(np.int64)
+    elif info["lanes"] == 16 or info["mode"] == 5:                            # 32-bit byte offsets, row included
+        e = meta.reshape(nb, cpad, g, rd).astype(np.int64)
         assert (e % 16 == 0).all()
         rel = (e // 16 - rowoff[None, :, None, None]).transpose(0, 2, 3, 1)
     else:                                                                     # 16-bit superword offsets
@@ -80,8 +80,9 @@ def test_kernel_tables_reproduce_the_delay_table(cfg):
         got, rd, shape = _decode(plan, r)
         assert np.array_equal(got, _padded_delays(plan, r, shape, rd)), (cfg, r)
         # shared memory of the launch: ring + barriers + prefetch pad fits the 227 KB opt-in limit
-        meta_stage = (shape["chans_per_stage"] // 4 if plan.tile_info(r)["mode"] == 2 else shape["chans_per_stage"]) \
-            * shape["trial_groups"] * 16
+        mode = plan.tile_info(r)["mode"]
+        meta_stage = (shape["chans_per_stage"] // 4 if mode == 2 else shape["chans_per_stage"]) \
+            * shape["trial_groups"] * (32 if mode == 5 else 16)
         stage = -(-(shape["chans_per_stage"] * shape["row_superwords"] * 16 + meta_stage) // 128) * 128
         assert 128 + shape["stages"] * stage + 512 <= 227 * 1024 and shape["stages"] >= 2
     plan.destroy()
@@ -89,18 +90,21 @@ def test_kernel_tables_reproduce_the_delay_table(cfg):
 
 def test_lane_widths_and_modes_of_the_five_configs():
     """Which adder each range gets: delta-coded 16-bit lanes for the fine DM grids of
-    config 3, 8-bit lanes for undecimated coarse grids, 32-bit lanes for decimated uint16."""
-    want = {1: [(16, 0)], 2: [(16, 0)], 3: [(8, 2), (8, 2), (8, 2)], 4: [(16, 0), (4, None)], 5: [(16, 0)]}
+    config 3, 8-bit lanes for undecimated coarse grids of uint8 data, uint16 lanes for undecimated uint16 data, 32-bit
+    lanes for decimated uint16."""
+    want = {1: [(16, 0)], 2: [(16, 0)], 3: [(8, 2), (8, 2), (8, 2)], 4: [(8, 5), (4, None)], 5: [(16, 0)]}
     for cfg, exp in want.items():
         plan = _host_plan(W.CONFIGS[cfg])
         for r, (lanes, mode) in enumerate(exp):
             info = plan.tile_info(r)
             assert info["lanes"] == lanes and (mode is None or info["mode"] == mode), (cfg, r, info)
-            if lanes == 8:   # 255 + flush*maxval <= 65535, at most 256 flushes
+            if lanes == 8 and info["mode"] == 5:
+                assert info["flush_chans"] == 0   # E (mod 2^32) and O never overflow: no flush
+            elif lanes == 8:   # 255 + flush*maxval <= 65535, at most 256 flushes
                 maxval = 255 * plan.ranges[r][3]
                 assert 255 + info["flush_chans"] * maxval <= 65535
                 assert -(-plan.tile_shape(r)["cpad"] // info["flush_chans"]) <= 256
-        assert plan.launches() == sum(1 + (2 if (cfg == 4 and r == 0) else 1) for r in range(len(exp)))
+        assert plan.launches() == 2 * len(exp)   # one pack and one dedispersion launch per range
         plan.destroy()
 
 
@@ -124,7 +128,9 @@ def test_host_only_plans_cannot_execute_and_edge_shapes_build():
         info = p.tile_info(0)
         if info["mode"] == 2 or decim > 1:          # delta-coded or decimated: 16-bit lanes while they can hold the sums
             assert info["lanes"] == (8 if bits == 8 and nch <= 30720 else 4)
-        else:                                       # undecimated, coarse steps: byte lanes (uint16: two planes)
+        elif bits == 16:                            # undecimated uint16, coarse steps: the samples in 16-bit lanes
+            assert info["lanes"] == 8 and info["mode"] == 5
+        else:                                       # undecimated uint8, coarse steps: byte lanes
             assert info["lanes"] == (16 if nch <= 30720 else 4)
         p.destroy()
 
