@@ -172,6 +172,26 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
  */
 int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream);
 
+/*
+ * dd_execute_host_async / dd_host_wait: the same end-to-end path for a stream of beams or blocks, one call per step
+ * (a search node processes one beam after the other).  dd_execute_host_async enqueues what dd_execute_host
+ * does and returns without waiting; dd_host_wait blocks until every call made so far has finished (all results are in
+ * their out_host buffers, all in_host buffers have been read).  The plan owns two slots of staging buffers, used
+ * alternately, and a second copy stream for the uploads, so that with back-to-back calls the upload of step i+1 and the
+ * end of the download of step i run while the kernels of the steps in between compute: per step the time tends to
+ * max(kernels, upload, download) instead of their partial sum.  Rules: both host buffers page-locked (else the copies
+ * serialise); in_host must stay unchanged and out_host untouched until dd_host_wait returns; the out_host buffers of two
+ * consecutive calls must differ (their copies may overlap in time); the same cuda_stream for consecutive calls (a change
+ * of stream first waits for everything in flight).  dd_execute_host == dd_execute_host_async + dd_host_wait.  Errors as
+ * dd_execute_host; after an error everything in flight has been drained.
+ */
+int dd_execute_host_async(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream);
+int dd_host_wait(dd_plan_t* plan);
+/* Launches per range of the host path (1 .. 64, default 4): each finished piece of a range's rows is copied back while the
+ * next is computed.  More pieces shorten the copy left over after the last kernel of a synchronous call; fewer pieces
+ * cost fewer partial waves of CTAs, which is what matters when calls are queued back to back. */
+int dd_plan_set_host_pieces(dd_plan_t* plan, int32_t pieces);
+
 /* dd_plan_destroy: frees host and device memory of the plan.  NULL is a no-op returning DD_OK.  The
  * caller must make sure no execute of this plan is still running. */
 int dd_plan_destroy(dd_plan_t* plan);

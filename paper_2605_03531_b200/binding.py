@@ -19,7 +19,7 @@ DD_LAYOUT_CHANNEL_MAJOR, DD_LAYOUT_SPECTRUM_MAJOR = 0, 1
 
 # every symbol include/dd.h declares
 SYMBOLS = [
-    "dd_plan_create", "dd_execute", "dd_execute_host", "dd_plan_destroy", "dd_plan_out_elems",
+    "dd_plan_create", "dd_execute", "dd_execute_host", "dd_execute_host_async", "dd_host_wait", "dd_plan_set_host_pieces", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_executed_adds", "dd_plan_pair_info",
     "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
@@ -73,6 +73,9 @@ def _load():
         lib.dd_plan_create.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_execute.argtypes = [vp, vp, vp, vp]
         lib.dd_execute_host.argtypes = [vp, vp, vp, vp]
+        lib.dd_execute_host_async.argtypes = [vp, vp, vp, vp]
+        lib.dd_host_wait.argtypes = [vp]
+        lib.dd_plan_set_host_pieces.argtypes = [vp, i32]
         lib.dd_plan_destroy.argtypes = [vp]
         lib.dd_plan_out_elems.argtypes = [vp, P(i64)]
         lib.dd_plan_beam_stride.argtypes = [vp, P(i64)]
@@ -216,6 +219,23 @@ class Plan:
                 return a.data_ptr()
             return a.ctypes.data
         _chk(_load().dd_execute_host(self._h, addr(in_host), addr(out_host), _stream_ptr(stream)), "dd_execute_host")
+
+    def execute_host_async(self, in_host, out_host, stream=None) -> None:
+        """dd_execute_host without the final wait (page-locked buffers; consecutive calls need different out_host)."""
+        def addr(a):
+            if isinstance(a, int):
+                return a
+            if hasattr(a, "data_ptr"):
+                return a.data_ptr()
+            return a.ctypes.data
+        _chk(_load().dd_execute_host_async(self._h, addr(in_host), addr(out_host), _stream_ptr(stream)),
+             "dd_execute_host_async")
+
+    def host_wait(self) -> None:
+        _chk(_load().dd_host_wait(self._h), "dd_host_wait")
+
+    def set_host_pieces(self, pieces: int) -> None:
+        _chk(_load().dd_plan_set_host_pieces(self._h, pieces), "dd_plan_set_host_pieces")
 
     # -- queries
     def out_elems(self) -> int:

@@ -151,9 +151,18 @@ struct dd_plan {
   mutable std::vector<int> prof_kind, prof_range, prof_count;  // per slot*max_launches
   // host path: staging buffers, a copy stream and events so that the device-to-host copy of finished trial
   // blocks overlaps the dedispersion of the following ones
-  void* h_in_dev = nullptr;
-  float* h_out_dev = nullptr;
-  cudaStream_t copy_stream = nullptr;
+  // Two slots of staging buffers, so that back-to-back calls (dd_execute_host_async) overlap the upload of step i+1
+  // and the tail of the download of step i with the kernels in between.
+  void* h_in_dev[2] = {nullptr, nullptr};
+  float* h_out_dev[2] = {nullptr, nullptr};
+  cudaStream_t copy_stream = nullptr;  // device-to-host pieces
+  cudaStream_t h2d_stream = nullptr;   // host-to-device input
+  cudaStream_t host_stream = nullptr;  // the caller's stream of the last host call (dd_host_wait synchronises it)
+  cudaEvent_t ev_in_ready[2] = {nullptr, nullptr};  // input of the slot has arrived
+  cudaEvent_t ev_in_free[2] = {nullptr, nullptr};   // the kernels that read the slot's input are done
+  cudaEvent_t ev_out_free[2] = {nullptr, nullptr};  // the slot's output has been copied back
+  long long host_calls = 0;            // slot of a call = host_calls % 2
+  int host_pieces = 4;                 // launches per range of the host path (dd_plan_set_host_pieces)
   std::vector<cudaEvent_t> host_events;
 };
 

@@ -608,10 +608,16 @@ int dd_plan_destroy(dd_plan_t* p) {
   }
   for (cudaEvent_t e : p->prof_events) cudaEventDestroy(e);
   if (p->ws && p->ws_owned) cudaFree(p->ws);
-  if (p->h_in_dev) cudaFree(p->h_in_dev);
-  if (p->h_out_dev) cudaFree(p->h_out_dev);
+  for (int s = 0; s < 2; ++s) {
+    if (p->h_in_dev[s]) cudaFree(p->h_in_dev[s]);
+    if (p->h_out_dev[s]) cudaFree(p->h_out_dev[s]);
+    if (p->ev_in_ready[s]) cudaEventDestroy(p->ev_in_ready[s]);
+    if (p->ev_in_free[s]) cudaEventDestroy(p->ev_in_free[s]);
+    if (p->ev_out_free[s]) cudaEventDestroy(p->ev_out_free[s]);
+  }
   for (cudaEvent_t e : p->host_events) cudaEventDestroy(e);
   if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+  if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
   delete p;
   return DD_OK;
 }
@@ -673,15 +679,23 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
   return DD_OK;
 }
 
-// Everything dd_execute_host enqueues.  Any failure is returned to the caller below, which drains both streams
-// before handing the error on (the caller's buffers must not be touched by copies still in flight).
-static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out_host, cudaStream_t stream) {
+// Everything a host call enqueues, for staging slot `slot`.  Any failure is returned to the caller below, which drains
+// all streams before handing the error on (the caller's buffers must not be touched by copies still in flight).
+//   h2d_stream : in_host -> h_in_dev[slot], once the kernels of the call that used this slot before have read it
+//   stream     : pack kernels (wait for the upload), then the dedispersion kernels a few trial blocks at a time (the first
+//                waits until the slot's previous output has been copied back)
+//   copy_stream: each finished piece -> out_host while the next blocks are computed
+static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out_host, cudaStream_t stream, int slot) {
   const size_t in_bytes = (size_t)plan->nbeams * plan->nchans * plan->nsamps * (plan->in_bits / 8);
   const bool all_direct = plan->variant == DD_KERNEL_DIRECT;
+  void* const in_dev = plan->h_in_dev[slot];
+  float* const out_dev = plan->h_out_dev[slot];
   // The DM-time plane is 3.6x the input: its copy back is the larger half of the transfer time.  Every range is
   // dedispersed in a few launches of consecutive trial blocks; as soon as one is done (event), its rows -- one
   // contiguous piece per beam -- go back on the copy stream while the next blocks are computed.
-  constexpr int kPieces = 8;  // per range: pieces of >= 1 trial block, ~14 waves of CTAs each for config 3
+  // per range: pieces of >= 1 trial block.  Config 3, ms per step synchronous / queued back to back: 1 piece 152.5 / 116.0,
+  // 2: 140.4 / 116.4, 4: 137.4 / 117.4, 8: 138.8 / 120.0, 16: 143.0 / 124.2 (every launch ends in a partial wave)
+  const int kPieces = plan->host_pieces;
   size_t nev = 0;
   auto next_event = [&](cudaEvent_t* ev) -> cudaError_t {
     if (nev == plan->host_events.size()) {
@@ -701,40 +715,52 @@ static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out
     if ((rc = cudaStreamWaitEvent(plan->copy_stream, ev, 0)) != cudaSuccess) return rc;
     for (int b = 0; b < plan->nbeams; ++b) {
       const size_t off = (size_t)b * plan->beam_stride + r.offset + (size_t)j0 * r.pitch;
-      rc = cudaMemcpyAsync(out_host + off, plan->h_out_dev + off, (size_t)(j1 - j0) * r.pitch * sizeof(float),
+      rc = cudaMemcpyAsync(out_host + off, out_dev + off, (size_t)(j1 - j0) * r.pitch * sizeof(float),
                            cudaMemcpyDeviceToHost, plan->copy_stream);
       if (rc != cudaSuccess) return rc;
     }
     return cudaSuccess;
   };
-  DD_CUDA(cudaMemcpyAsync(plan->h_in_dev, in_host, in_bytes, cudaMemcpyHostToDevice, stream));
-  for (const auto& r : plan->ranges) {
-    if (all_direct || !r.tiled_ok) continue;
-    DD_CUDA(dd::launch_pack(plan, r, plan->h_in_dev, stream));
-    if (dd::use_pairs(plan, r)) DD_CUDA(dd::launch_pairs(plan, r, stream));
-  }
+  DD_CUDA(cudaStreamWaitEvent(plan->h2d_stream, plan->ev_in_free[slot], 0));  // (never recorded yet: no wait)
+  DD_CUDA(cudaMemcpyAsync(in_dev, in_host, in_bytes, cudaMemcpyHostToDevice, plan->h2d_stream));
+  DD_CUDA(cudaEventRecord(plan->ev_in_ready[slot], plan->h2d_stream));
+  DD_CUDA(cudaStreamWaitEvent(stream, plan->ev_in_ready[slot], 0));
+  bool reads_input_late = all_direct;  // the direct kernel reads the input itself
   for (const auto& r : plan->ranges) {
     if (all_direct || !r.tiled_ok) {
-      DD_CUDA(dd::launch_direct(plan, r, plan->h_in_dev, plan->h_out_dev, stream));
+      reads_input_late = true;
+      continue;
+    }
+    DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
+    if (dd::use_pairs(plan, r)) DD_CUDA(dd::launch_pairs(plan, r, stream));
+  }
+  if (!reads_input_late) DD_CUDA(cudaEventRecord(plan->ev_in_free[slot], stream));
+  DD_CUDA(cudaStreamWaitEvent(stream, plan->ev_out_free[slot], 0));
+  for (const auto& r : plan->ranges) {
+    if (all_direct || !r.tiled_ok) {
+      DD_CUDA(dd::launch_direct(plan, r, in_dev, out_dev, stream));
       DD_CUDA(copy_rows(r, 0, r.ndm));
       continue;
     }
     const int per = std::max(1, (r.nblocks + kPieces - 1) / kPieces);
     for (int b0 = 0; b0 < r.nblocks; b0 += per) {
       const int nb = std::min(per, r.nblocks - b0);
-      DD_CUDA(dd::launch_tiled(plan, r, plan->h_out_dev, stream, b0, nb));
+      DD_CUDA(dd::launch_tiled(plan, r, out_dev, stream, b0, nb));
       DD_CUDA(copy_rows(r, b0 * r.Dcta, std::min(r.ndm, (b0 + nb) * r.Dcta)));
     }
   }
-  // the caller's stream, which this call synchronises, waits for the last copy
-  cudaEvent_t done;
-  DD_CUDA(next_event(&done));
-  DD_CUDA(cudaEventRecord(done, plan->copy_stream));
-  DD_CUDA(cudaStreamWaitEvent(stream, done, 0));
+  if (reads_input_late) DD_CUDA(cudaEventRecord(plan->ev_in_free[slot], stream));
+  DD_CUDA(cudaEventRecord(plan->ev_out_free[slot], plan->copy_stream));
   return DD_OK;
 }
 
-int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
+static void host_drain(dd_plan_t* plan) {
+  if (plan->h2d_stream) cudaStreamSynchronize(plan->h2d_stream);
+  cudaStreamSynchronize(plan->host_stream);
+  if (plan->copy_stream) cudaStreamSynchronize(plan->copy_stream);
+}
+
+int dd_execute_host_async(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
   if (!plan || !in_host || !out_host || plan->device < 0) return DD_ERR_INVALID;
   {
     int cur = -1;
@@ -753,21 +779,54 @@ int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void*
       return DD_ERR_NOMEM;
     }
   }
-  if (!plan->h_in_dev) {
-    if (cudaMalloc(&plan->h_in_dev, in_bytes) != cudaSuccess) { plan->h_in_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
+  const int slot = (int)(plan->host_calls % 2);
+  if (!plan->h_in_dev[slot]) {
+    if (cudaMalloc(&plan->h_in_dev[slot], in_bytes) != cudaSuccess) { plan->h_in_dev[slot] = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
   }
-  if (!plan->h_out_dev) {
-    if (cudaMalloc(&plan->h_out_dev, out_bytes) != cudaSuccess) { plan->h_out_dev = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
+  if (!plan->h_out_dev[slot]) {
+    if (cudaMalloc(&plan->h_out_dev[slot], out_bytes) != cudaSuccess) { plan->h_out_dev[slot] = nullptr; cudaGetLastError(); return DD_ERR_NOMEM; }
   }
   if (!plan->copy_stream) DD_CUDA(cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
-  const int rc = execute_host_enqueue(plan, in_host, out_host, stream);
+  if (!plan->h2d_stream) DD_CUDA(cudaStreamCreateWithFlags(&plan->h2d_stream, cudaStreamNonBlocking));
+  for (int s = 0; s < 2; ++s) {
+    if (!plan->ev_in_ready[s]) DD_CUDA(cudaEventCreateWithFlags(&plan->ev_in_ready[s], cudaEventDisableTiming));
+    if (!plan->ev_in_free[s]) DD_CUDA(cudaEventCreateWithFlags(&plan->ev_in_free[s], cudaEventDisableTiming));
+    if (!plan->ev_out_free[s]) DD_CUDA(cudaEventCreateWithFlags(&plan->ev_out_free[s], cudaEventDisableTiming));
+  }
+  if (plan->host_calls > 0 && plan->host_stream != stream) host_drain(plan);  // a change of stream breaks the stream order the slots rely on
+  plan->host_stream = stream;
+  const int rc = execute_host_enqueue(plan, in_host, out_host, stream, slot);
+  ++plan->host_calls;
   if (rc != DD_OK) {  // drain what was enqueued: no copy may still read or write the caller's buffers after we return
-    cudaStreamSynchronize(stream);
-    cudaStreamSynchronize(plan->copy_stream);
+    host_drain(plan);
     return rc;
   }
-  DD_CUDA(cudaStreamSynchronize(stream));
   return DD_OK;
+}
+
+int dd_plan_set_host_pieces(dd_plan_t* plan, int32_t pieces) {
+  if (!plan || pieces < 1 || pieces > 64) return DD_ERR_INVALID;
+  plan->host_pieces = pieces;
+  return DD_OK;
+}
+
+int dd_host_wait(dd_plan_t* plan) {
+  if (!plan || plan->device < 0) return DD_ERR_INVALID;
+  if (plan->host_calls == 0) return DD_OK;
+  {
+    int cur = -1;
+    DD_CUDA(cudaGetDevice(&cur));
+    if (cur != plan->device) return DD_ERR_DEVICE;
+  }
+  DD_CUDA(cudaStreamSynchronize(plan->h2d_stream));
+  DD_CUDA(cudaStreamSynchronize(plan->host_stream));
+  DD_CUDA(cudaStreamSynchronize(plan->copy_stream));
+  return DD_OK;
+}
+
+int dd_execute_host(dd_plan_t* plan, const void* in_host, float* out_host, void* cuda_stream) {
+  const int rc = dd_execute_host_async(plan, in_host, out_host, cuda_stream);
+  return rc != DD_OK ? rc : dd_host_wait(plan);
 }
 
 int dd_plan_out_elems(const dd_plan_t* p, int64_t* total_floats) {

@@ -292,6 +292,37 @@ def test_host_path_pieces_and_beams(bits):
         check_full(w, x, plan, hout.numpy(), want, check_pad=False)
 
 
+@pytest.mark.parametrize("variant", [TILED, DIRECT])
+def test_host_path_async_back_to_back_steps(variant):
+    """dd_execute_host_async: five steps with different inputs queued back to back (two staging slots used
+    alternately, uploads on their own stream), one dd_host_wait, every step's plane equal to the oracle's; then the
+    synchronous call on the same plan, and a change of stream in between."""
+    import torch
+    from paper_2605_03531_b200 import binding as B
+    nch, ns, steps = 80, 2 ** 13 + 40, 5
+    w = W.Workload("hostasync", 750.0, -200.0 / nch, nch, 1.31072e-3, ns, 2, 8,
+                   (W.DMRange(0.0, 0.1, 300, 1), W.DMRange(30.0, 2.5, 100, 1), W.DMRange(280.0, 5.0, 33, 4)), 1, 0, 0)
+    rng = np.random.default_rng(4242)
+    xs = [rng.integers(0, 256, size=(2, nch, ns), dtype=np.uint8) for _ in range(steps)]
+    plan = B.Plan.from_workload(w)
+    plan.set_kernel(variant)
+    hins = [torch.from_numpy(x).pin_memory() for x in xs]
+    houts = [torch.full((plan.out_elems(),), -1.0, dtype=torch.float32).pin_memory() for _ in range(steps)]
+    side = torch.cuda.Stream()
+    for s in range(steps):
+        plan.execute_host_async(hins[s], houts[s], torch.cuda.current_stream())
+    plan.host_wait()
+    for s in range(steps):
+        check_full(w, xs[s], plan, houts[s].numpy(), check_pad=False)
+    # another stream (everything in flight is drained first), then the synchronous form
+    houts[0].fill_(-1.0), houts[1].fill_(-1.0)
+    plan.execute_host_async(hins[3], houts[0], side)
+    plan.execute_host(hins[1], houts[1], side)
+    check_full(w, xs[3], plan, houts[0].numpy(), check_pad=False)
+    check_full(w, xs[1], plan, houts[1].numpy(), check_pad=False)
+    plan.host_wait()   # nothing in flight: returns at once
+
+
 def test_shared_partial_sums_variant():
     """DD_KERNEL_SHARED: the sum of a channel quad is reused across neighbouring trials
     while none of its delays changes.  Fewer executed adds, identical bits (delta ranges; others unchanged)."""
