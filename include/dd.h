@@ -128,7 +128,9 @@ int dd_plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out);
  * choices of the plan builder overridden -- for tests and measurements; the results never change, only the kernel
  * shape.  tuning == NULL means automatic.  (The library reads no environment variables.)
  *   mode        -1 automatic; 0 / 1 / 2 force the table form of the tiled kernel (see dd_plan_tile_info); the delta
- *               form is refused (falls back to 0) for a range with a delay step above 1 between neighbouring trials
+ *               form is refused (falls back to 0) for a range with a delay step above 1 between neighbouring trials;
+ *               6 asks for the hybrid form wherever at least one leading channel chunk can be delta-coded (automatic:
+ *               only when that part is large enough to pay)
  *   byte_lanes  -1 automatic; 1: 8-bit lanes wherever they apply, uint16 input as two byte planes (automatic for uint8;
  *               undecimated uint16 input automatically runs on uint16 lanes instead, table form 5); 0: never use 8-bit or
  *               uint16 lanes (undecimated coarse ranges then run on 16-/32-bit lanes with the table forms 0 / 1)
@@ -236,9 +238,13 @@ int dd_plan_set_kernel(dd_plan_t* plan, int32_t variant);
  * flushes of the packed accumulators (0: never), and the table mode: 0 = one shared-memory load per (channel, trial),
  * 1 = load skipped when the delay equals the previous trial's, 2 = delta form (all delay steps inside a
  * group of 8 trials are 0 or 1; one changed bit per trial), 5 = uint16 samples in the 16-bit lanes (undecimated
- * uint16 input; 32-bit byte offsets, load skipped on equal offsets). */
+ * uint16 input; 32-bit byte offsets, load skipped on equal offsets), 6 = hybrid: the leading channel chunks (pipeline
+ * stages; the highest channels, whose delay steps never exceed 1) use form 2, the others form 1, 7 = the same on
+ * uint16 lanes (forms 2 / 5).  dd_plan_delta_chunks: how many leading chunks of chans_per_stage channels use form 2
+ * (all of them for mode 2, none for 0 / 1 / 5). */
 int dd_plan_tile_info(const dd_plan_t* plan, int32_t r, int32_t* dm_per_cta, int32_t* words_per_cta,
                       int32_t* lanes, int32_t* flush_chans, int32_t* mode);
+int dd_plan_delta_chunks(const dd_plan_t* plan, int32_t r, int32_t* chunks);
 
 /* More of the tile shape of range r (any pointer may be NULL): trial groups per CTA, channels per pipeline
  * stage, ring depth, superwords per staged channel row, channel rows incl. zero padding, trial blocks, and

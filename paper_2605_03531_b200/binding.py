@@ -22,7 +22,7 @@ SYMBOLS = [
     "dd_plan_create", "dd_execute", "dd_execute_host", "dd_execute_host_async", "dd_host_wait", "dd_plan_set_host_pieces", "dd_plan_destroy", "dd_plan_out_elems",
     "dd_plan_beam_stride", "dd_plan_range_info", "dd_plan_get_delays", "dd_plan_work", "dd_plan_launches",
     "dd_plan_executed_adds", "dd_plan_pair_info",
-    "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info",
+    "dd_plan_workspace_bytes", "dd_plan_set_workspace", "dd_plan_set_kernel", "dd_plan_tile_info", "dd_plan_delta_chunks",
     "dd_plan_create_host", "dd_plan_create_tail", "dd_plan_create_tuned", "dd_plan_tile_shape", "dd_plan_table",
     "dd_sps_rows", "dd_sps_execute", "dd_sps_candidates", "dd_plan_set_row_stats", "dd_stream_create", "dd_stream_push", "dd_stream_plan", "dd_stream_info", "dd_stream_destroy",
     "dd_plan_set_profiling", "dd_plan_kernel_times", "dd_strerror", "dd_last_cuda_error", "dd_version",
@@ -89,6 +89,7 @@ def _load():
         lib.dd_plan_set_workspace.argtypes = [vp, vp, i64]
         lib.dd_plan_set_kernel.argtypes = [vp, i32]
         lib.dd_plan_tile_info.argtypes = [vp, i32, P(i32), P(i32), P(i32), P(i32), P(i32)]
+        lib.dd_plan_delta_chunks.argtypes = [vp, i32, P(i32)]
         lib.dd_plan_create_host.argtypes = [P(dd_config_t), P(vp)]
         lib.dd_plan_create_tail.argtypes = [P(dd_config_t), ctypes.c_int64, P(vp)]
         lib.dd_plan_create_tuned.argtypes = [P(dd_config_t), P(dd_tuning_t), i32, P(vp)]
@@ -302,6 +303,11 @@ class Plan:
         vals = [ctypes.c_int32() for _ in range(5)]
         _chk(_load().dd_plan_tile_info(self._h, r, *[ctypes.byref(v) for v in vals]), "dd_plan_tile_info")
         return {k: v.value for k, v in zip(["dm_per_cta", "words_per_cta", "lanes", "flush_chans", "mode"], vals)}
+
+    def delta_chunks(self, r: int) -> int:
+        v = ctypes.c_int32()
+        _chk(_load().dd_plan_delta_chunks(self._h, r, ctypes.byref(v)), "dd_plan_delta_chunks")
+        return int(v.value)
 
     def tile_shape(self, r: int) -> dict:
         vals = [ctypes.c_int32() for _ in range(7)]

@@ -26,7 +26,8 @@ constexpr int kRD16 = 4;          // the same for NL = 16 (twice the accumulator
 __host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? kRD16 : kRD; }
 
 // How the tiled kernel finds the staged superword of (channel, trial):
-//   kModeGeneral       per channel and trial group: kRD 16-bit superword offsets, one shared-memory load per trial
+//   kModeGeneral       per channel and trial: a 32-bit byte offset inside the stage (row of the channel included), one
+//                      shared-memory load per trial
 //   kModeGeneralReuse  same table; the load is skipped when the offset equals the previous trial's
 //   kModeDelta         every delay step inside a trial group is 0 or 1 (fine DM grids): per channel the
 //                      offset of the group's first trial plus one "changed" bit per later trial; a changed
@@ -44,7 +45,17 @@ __host__ __device__ constexpr int trials_per_thread(int NL) { return NL == 16 ? 
 //                      headroom, so a word w of two lanes is accumulated as E += w (mod 2^32) and O += w >> 16; lane sums are
 //                      E - (O << 16) and O.  Table: eight 32-bit byte offsets inside the stage (row included) per (channel,
 //                      trial group); the load is skipped when the offset equals the previous trial's.
-enum TiledMode { kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3, kModeDeltaPair = 4, kModeWide = 5 };
+//   kModeHybrid        per channel CHUNK (pipeline stage): the leading chunks -- the highest channels, whose delay steps
+//                      never exceed 1 -- carry the delta table, the remaining ones the offsets table with reuse.  A range whose
+//                      lowest channels step by a little more than one sample per trial keeps the delta kernel for most
+//                      of its channels instead of losing it altogether.
+//   kModeWideHybrid    the same for uint16 lanes (kModeWide adder in both kinds of chunk)
+enum TiledMode {
+  kModeGeneral = 0, kModeGeneralReuse = 1, kModeDelta = 2, kModeDeltaShare = 3, kModeDeltaPair = 4, kModeWide = 5,
+  kModeHybrid = 6, kModeWideHybrid = 7
+};
+__host__ __device__ constexpr bool is_hybrid(int mode) { return mode == kModeHybrid || mode == kModeWideHybrid; }
+__host__ __device__ constexpr bool is_wide(int mode) { return mode == kModeWide || mode == kModeWideHybrid; }
 __host__ __device__ constexpr bool is_delta(int mode) {
   return mode == kModeDelta || mode == kModeDeltaShare || mode == kModeDeltaPair;
 }
@@ -58,13 +69,12 @@ __host__ __device__ constexpr int delta_bit(int j, int q) { return (((j - 1) * 4
 // for a block whose delays spread over `spread` superwords.
 __host__ __device__ constexpr int aligned_span(int spread) { return (spread + 7 + 7) / 8 * 8; }
 
-// Meta bytes per pipeline stage of Cc channels and G trial groups: one 16-byte entry per (channel, trial
-// group) -- eight 16-bit superword offsets, or (NL = 16) four 32-bit byte offsets inside the stage, row
-// included -- or one 16-byte entry per channel quad in delta mode.
+// Meta bytes per pipeline stage of Cc channels and G trial groups: one 32-bit byte offset inside the stage (row
+// included) per (channel, trial) -- or one 16-byte entry per channel quad and trial group in delta mode.
 __host__ __device__ constexpr size_t tiled_meta_bytes(int mode, int NL, int Cc, int G) {
   if (mode == 4) return (size_t)(Cc / 8) * (size_t)G * 80;  // kModeDeltaPair: 5 entries per quad of pairs (8 rows)
-  if (mode == 5) return (size_t)Cc * (size_t)G * 32;        // kModeWide: eight 32-bit byte offsets per (channel, trial group)
-  return (size_t)(is_delta(mode) ? Cc / 4 : Cc) * (size_t)G * 16;
+  if (is_delta(mode)) return (size_t)(Cc / 4) * (size_t)G * 16;
+  return (size_t)Cc * (size_t)G * (size_t)trials_per_thread(NL) * 4;  // one 32-bit byte offset per (channel, trial)
 }
 
 struct RangePlan {
@@ -82,6 +92,7 @@ struct RangePlan {
   int64_t plane_bytes = 0;  // bytes of one packed plane in the workspace
   int flush = 0;     // channels between flushes of the 16-bit lanes (0: never, 32-bit lanes)
   int mode = 0;      // TiledMode
+  int nd = 0;        // hybrid modes: leading channel chunks with the delta table (0 otherwise)
   int G = 0;         // trial groups per CTA (kRD trials each)
   int T = 0;         // superwords per CTA (multiple of 32)
   int Dcta = 0;      // trials per CTA = G*kRD
@@ -100,7 +111,7 @@ struct RangePlan {
   // tables of the tiled kernel: host copies (built by dd_plan.cu build_tables) and their device twins
   std::vector<uint32_t> h_meta;
   std::vector<int32_t> h_dmin, h_span;
-  uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] RD 16-bit offsets (delay - dmin, superwords);
+  uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] RD 32-bit byte offsets inside the stage;
                                 // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits}
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)

@@ -96,10 +96,12 @@ int max_block_span(const dd_plan& p, const dd::RangePlan& r, int Dcta) {
 }
 
 // Which table form the tiled kernel uses for this range (dd_internal.h TiledMode).  Trial groups are the
-// kRD-aligned runs of trials counted from the start of the range.
-int choose_mode(const dd_plan& p, const dd::RangePlan& r, const dd_tuning_t& tune) {
-  bool delta = true;
+// kRD-aligned runs of trials counted from the start of the range.  *delta_prefix = number of leading channels
+// (highest frequencies) none of whose delay steps inside a trial group exceeds 1: the whole range is delta-coded when
+// that is every channel, and a hybrid range delta-codes the channel chunks inside that prefix.
+int choose_mode(const dd_plan& p, const dd::RangePlan& r, const dd_tuning_t& tune, int* delta_prefix) {
   int64_t same = 0, total = 0;
+  int prefix = p.nchans;  // first channel with a step above 1 (delays grow with the channel index, so do their steps)
   for (int j = 0; j + 1 < r.ndm; ++j) {
     if ((j + 1) % dd::kRD == 0) continue;  // first trial of a group always loads
     const int32_t* d0 = &r.delays[(size_t)j * p.nchans];
@@ -107,14 +109,16 @@ int choose_mode(const dd_plan& p, const dd::RangePlan& r, const dd_tuning_t& tun
     for (int c = 0; c < p.nchans; ++c) {
       const int32_t inc = d1[c] - d0[c];
       same += inc == 0;
-      delta = delta && inc <= 1;
+      if (inc > 1 && c < prefix) prefix = c;
     }
     total += p.nchans;
   }
+  const bool delta = prefix == p.nchans;
+  *delta_prefix = prefix;
   int mode = delta ? dd::kModeDelta : (total > 0 && (double)same / (double)total >= 0.25) ? dd::kModeGeneralReuse
                                                                                          : dd::kModeGeneral;
-  if (tune.mode >= 0) mode = tune.mode;  // dd_plan_create_tuned; delta is refused when it does not apply
-  if (mode < 0 || mode > 2 || (mode == dd::kModeDelta && !delta)) mode = dd::kModeGeneral;
+  if (tune.mode >= 0 && tune.mode <= 2) mode = tune.mode;  // dd_plan_create_tuned; delta is refused when it does not apply
+  if (mode == dd::kModeDelta && !delta) mode = dd::kModeGeneral;
   return mode;
 }
 
@@ -133,18 +137,33 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
     r.NL = 4;
     r.flush = 0;
   }
-  r.mode = choose_mode(p, r, tune);
+  int delta_prefix = 0;
+  r.mode = choose_mode(p, r, tune, &delta_prefix);
+  r.nd = 0;
+  // Hybrid (dd_internal.h kModeHybrid): not delta-codable as a whole, but a leading part of the channels is.  Taken
+  // automatically for DECIMATED ranges when that part is at least a tenth of the channels: there the alternative is the
+  // offsets table alone (measured on config 3 with DM steps 0.22 / 0.45 / 0.9, lowest-channel delay steps of 1.06-1.09
+  // samples per trial, 96 % of the channels delta-coded: x2 21.1 -> 18.4 ms, x4 17.9 -> 15.7 ms; config 4's x8 range,
+  // 40 % delta-coded: 21.1 -> 19.6 ms).  Undecimated ranges keep the 8-bit-lane kernel (uint8; 35.6 ms against 36.6 ms
+  // hybrid in the same experiment: near the limit of the delta form half of all trial steps reload, and it is bound by
+  // shared memory like the offsets form) or the uint16-lane kernel (uint16; config 4 range 0: 236.3 against 236.1 ms).
+  // dd_tuning_t::mode = 6 asks for it wherever a chunk qualifies.
+  bool hybrid = false;
+  if (r.mode != dd::kModeDelta && (tune.mode < 0 || tune.mode == 6) && delta_prefix >= 4)
+    hybrid = tune.mode == 6 || (r.decim > 1 && (double)delta_prefix >= 0.10 * (double)p.nchans);
   // Undecimated ranges that cannot use the delta table run on 8-bit lanes: half the shared-memory traffic per
   // sample (the bound of the offsets-table modes), uint16 input as two byte planes.  dd_tuning_t::byte_lanes = 0
   // switches it off.
   const int flush16 = 65280 / 255;
-  if (p.in_bits == 16 && r.decim == 1 && r.mode != dd::kModeDelta && tune.byte_lanes < 0) {
+  if (hybrid && !(p.in_bits == 16 && r.decim == 1 && tune.byte_lanes < 0)) {
+    r.mode = dd::kModeHybrid;  // lanes as chosen above (16-bit with headroom, or 32-bit)
+  } else if (p.in_bits == 16 && r.decim == 1 && r.mode != dd::kModeDelta && tune.byte_lanes < 0) {
     // undecimated uint16 input on a coarse grid: the samples themselves in 16-bit lanes (kModeWide).  Shared memory
     // delivers 2 bytes per add either way, but one pass with 1.5 ALU instructions per two adds replaces two byte-plane
     // passes of the 8-bit-lane kernel.  dd_tuning_t::byte_lanes = 1 keeps the two byte planes, 0 the 32-bit lanes.
     r.NL = 8;
     r.flush = 0;
-    r.mode = dd::kModeWide;
+    r.mode = hybrid ? dd::kModeWideHybrid : dd::kModeWide;
   } else if (r.decim == 1 && r.mode != dd::kModeDelta && (int64_t)p.nchans <= (int64_t)120 * flush16 && tune.byte_lanes != 0) {
     r.NL = 16;
     r.flush = flush16;
@@ -162,7 +181,8 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
     const int D = G * r.RD;
     if (T + smax > 65535) return false;  // 16-bit offsets
     if (r.flush > 0 && Cc > r.flush) return false;
-    if (r.mode == dd::kModeDelta && (size_t)Cc * (size_t)(T + smax) * 16 > 65536) return false;  // 16-bit byte offsets
+    if ((r.mode == dd::kModeDelta || dd::is_hybrid(r.mode)) && (size_t)Cc * (size_t)(T + smax) * 16 > 65536)
+      return false;  // 16-bit byte offsets of the delta table
     const size_t stage = (size_t)Cc * (size_t)(T + smax) * 16 + dd::tiled_meta_bytes(r.mode, r.NL, Cc, G);
     const int stages = (int)std::min<size_t>(6, budget / stage);
     if (stages < min_stages) return false;
@@ -239,6 +259,10 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
   r.Dcta = r.G * r.RD;
   r.nblocks = (r.ndm + r.Dcta - 1) / r.Dcta;
   r.Cpad = (int)round_up(p.nchans, r.Cc);
+  if (dd::is_hybrid(r.mode)) {
+    r.nd = found ? delta_prefix / r.Cc : 0;  // whole chunks inside the delta-codable prefix
+    if (r.nd == 0) r.mode = r.mode == dd::kModeWideHybrid ? dd::kModeWide : dd::kModeGeneralReuse;
+  }
   if (r.flush > 0) r.flush = r.flush / r.Cc * r.Cc;
   r.Smax = max_block_span(p, r, r.Dcta);  // the true maximum over every (trial block, channel)
   if (r.T + r.Smax > 65535) r.tiled_ok = 0;
@@ -265,10 +289,15 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
   dmin.assign(nbc, 0);
   span.assign(nbc, 0);
   const bool delta = r.mode == dd::kModeDelta;
-  const size_t words_per_entry = r.mode == dd::kModeWide ? 8 : 4;
-  const size_t nentries = delta ? nbc / 4 * r.G : nbc * r.G;
+  // words of one chunk's table slice in the delta form (one 4-word entry per quad and trial group) and in the general
+  // forms (one 32-bit byte offset per channel and trial); a trial block holds its chunks' slices one after the other,
+  // a hybrid range its nd delta slices first
+  const size_t nchunks = (size_t)r.Cpad / r.Cc;
+  const size_t wd = (size_t)(r.Cc / 4) * r.G * 4, wg = (size_t)r.Cc * r.G * r.RD;
+  const size_t nd = delta ? nchunks : (size_t)r.nd;
+  const size_t words_per_block = nd * wd + (nchunks - nd) * wg;
   std::vector<uint32_t>& meta = r.h_meta;
-  meta.assign(nentries * words_per_entry, 0);
+  meta.assign((size_t)r.nblocks * words_per_block, 0);
   // rows past nchans are the zero rows of the packed input: delay 0 for every trial
   auto delay = [&](int j, int c) { return c < p.nchans ? r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c] : 0; };
   for (int b = 0; b < r.nblocks; ++b) {
@@ -280,8 +309,9 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
       if (span[(size_t)b * r.Cpad + c] > r.Smax) r.tiled_ok = 0;  // cannot happen (Smax is this maximum); never overrun a row
       for (int g = 0; g < r.G; ++g) {
         const int jg = j0 + g * r.RD;
-        if (delta) {
-          uint32_t* e = &meta[(((size_t)b * (r.Cpad / 4) + c / 4) * r.G + g) * 4];
+        const size_t k = (size_t)c / r.Cc, ci = (size_t)c % r.Cc;
+        if (k < nd) {
+          uint32_t* e = &meta[(size_t)b * words_per_block + k * wd + ((ci / 4) * r.G + g) * 4];
           const int q = c % 4;
           const uint32_t off = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg, c) - d0)) * 16u;
           e[1 + q / 2] |= off << (16 * (q % 2));  // byte offset inside the stage, < 64 KB (choose_tile)
@@ -291,13 +321,9 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
               e[3] |= 1u << j;  // some channel of the quad changes at this trial step
             }
         } else {
-          uint32_t* e = &meta[(((size_t)b * r.Cpad + c) * r.G + g) * words_per_entry];
-          if (r.NL == 16 || r.mode == dd::kModeWide) {  // byte offsets inside the stage, row of the channel included
-            for (int j = 0; j < r.RD; ++j)
-              e[j] = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg + j, c) - d0)) * 16u;
-          } else {
-            for (int j = 0; j < r.RD; ++j) e[j / 2] |= (uint32_t)(delay(jg + j, c) - d0) << (16 * (j % 2));
-          }
+          uint32_t* e = &meta[(size_t)b * words_per_block + nd * wd + (k - nd) * wg + (ci * r.G + g) * r.RD];
+          for (int j = 0; j < r.RD; ++j)  // byte offsets inside the stage, row of the channel included
+            e[j] = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg + j, c) - d0)) * 16u;
         }
       }
     }
@@ -550,7 +576,7 @@ static int plan_create_device(const dd_config_t* cfg, dd_plan_t** plan_out, int6
 int dd_plan_create(const dd_config_t* cfg, dd_plan_t** plan_out) { return plan_create_device(cfg, plan_out, 0); }
 
 int dd_plan_create_tuned(const dd_config_t* cfg, const dd_tuning_t* tuning, int32_t host_only, dd_plan_t** plan_out) {
-  if (tuning && (tuning->mode < -1 || tuning->mode > 2 || tuning->byte_lanes < -1 || tuning->byte_lanes > 1))
+  if (tuning && (tuning->mode < -1 || (tuning->mode > 2 && tuning->mode != 6) || tuning->byte_lanes < -1 || tuning->byte_lanes > 1))
     return DD_ERR_INVALID;
   return host_only ? plan_create_host(cfg, plan_out, 0, tuning) : plan_create_device(cfg, plan_out, 0, tuning);
 }
@@ -1050,6 +1076,13 @@ int dd_plan_tile_shape(const dd_plan_t* p, int32_t r, int32_t* trial_groups, int
   if (cpad) *cpad = q.Cpad;
   if (nblocks) *nblocks = q.nblocks;
   if (tiled) *tiled = q.tiled_ok;
+  return DD_OK;
+}
+
+int dd_plan_delta_chunks(const dd_plan_t* p, int32_t r, int32_t* chunks) {
+  if (!p || !chunks || r < 0 || r >= (int)p->ranges.size()) return DD_ERR_INVALID;
+  const auto& q = p->ranges[r];
+  *chunks = !q.tiled_ok ? 0 : q.mode == dd::kModeDelta ? q.Cpad / q.Cc : q.nd;
   return DD_OK;
 }
 

@@ -72,6 +72,7 @@ struct TiledParams {
   float* out;           // beam 0, this range
   long long out_beam_stride, pitch, Wp, H, nout, ntau;
   int ndm, Cpad, G, T, Cc, nstages;
+  int nd;            // hybrid modes: leading channel chunks that carry the delta table
   int blk0, nblk;    // trial blocks of this launch: blk0 .. blk0 + nblk - 1
   int rowpitch;      // superwords per staged row = T + Smax
   int flush_stages;  // move the upper bytes of the packed lanes away every this many stages (NL == 8, 16)
@@ -99,36 +100,48 @@ __device__ __forceinline__ uint32_t off16(const uint4& m, int j) {  // j-th 16-b
   return (j & 1) ? (w >> 16) : (w & 0xffffu);
 }
 
-// general modes: channels in pairs, one table entry (kRD 16-bit superword offsets) per channel
-template <bool REUSE>
-__device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
-                                              uint32_t row_bytes, uint32_t meta_row) {
+// general modes (kModeGeneral, kModeGeneralReuse, kModeWide): channels in pairs; per channel and trial group the table
+// holds kRD 32-bit byte offsets inside the stage, row of the channel included (two 16-byte entries), so an address is one
+// add.  REUSE: a trial whose offset equals the previous trial's keeps the registers (one compare, the load predicated
+// off).  WIDE: uint16 samples in the 16-bit lanes (add_wide), else packed lanes with headroom (add_pair).
+__device__ __forceinline__ uint32_t word_of(const uint4& m, int j) { return j == 0 ? m.x : j == 1 ? m.y : j == 2 ? m.z : m.w; }
+
+// uint16 lanes (kModeWide, NL = 8): a word w holds two uint16 samples with no headroom.  E += w (mod 2^32; one IADD3 for
+// two channels) and O += w >> 16 (one LEA.HI per channel) give the lane sums E - (O << 16) and O, exact while the channel
+// sum fits 32 bits (checked at plan creation).  Bound by shared memory: 2 bytes per add.
+__device__ __forceinline__ void add_wide(uint4& E, uint4& O, const uint4& a, const uint4& b) {
+  E.x = E.x + a.x + b.x, E.y = E.y + a.y + b.y, E.z = E.z + a.z + b.z, E.w = E.w + a.w + b.w;
+  O.x += a.x >> 16, O.y += a.y >> 16, O.z += a.z >> 16, O.w += a.w >> 16;
+  asm volatile("" : "+r"(O.x), "+r"(O.y), "+r"(O.z), "+r"(O.w));  // keeps each shift-add one LEA.HI
+  O.x += b.x >> 16, O.y += b.y >> 16, O.z += b.z >> 16, O.w += b.w >> 16;
+}
+
+template <bool REUSE, bool WIDE>
+__device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
+                                              uint32_t meta_row) {
 #pragma unroll 1
   for (int cc = 0; cc < Cc; cc += 2) {
-    uint4 ma, mb;
-    lds_sw(ma, smeta);
-    lds_sw(mb, smeta + meta_row);
+    uint4 ma[2], mb[2];
+    lds_sw(ma[0], smeta), lds_sw(ma[1], smeta + 16);
+    lds_sw(mb[0], smeta + meta_row), lds_sw(mb[1], smeta + meta_row + 16);
     smeta += 2 * meta_row;
-    const uint32_t ra = sdata, rb = sdata + row_bytes;
-    sdata += 2 * row_bytes;
     uint4 wa, wb;
-    uint32_t pa = off16(ma, 0), pb = off16(mb, 0);
-    lds_sw(wa, ra + pa * kSuperwordBytes);
-    lds_sw(wb, rb + pb * kSuperwordBytes);
-    add_pair(acc[0], wa, wb);
+    uint32_t pa = ma[0].x, pb = mb[0].x;
+    lds_sw(wa, sdata + pa);
+    lds_sw(wb, sdata + pb);
+    if constexpr (WIDE) add_wide(acc[0], hi[0], wa, wb); else add_pair(acc[0], wa, wb);
 #pragma unroll
     for (int j = 1; j < kRD; ++j) {
-      const uint32_t oa = off16(ma, j), ob = off16(mb, j);
+      const uint32_t oa = word_of(ma[j >> 2], j & 3), ob = word_of(mb[j >> 2], j & 3);
       if constexpr (REUSE) {
-        lds_if_ne(wa, ra + oa * kSuperwordBytes, oa, pa);
-        lds_if_ne(wb, rb + ob * kSuperwordBytes, ob, pb);
-        pa = oa;
-        pb = ob;
+        lds_if_ne(wa, sdata + oa, oa, pa);
+        lds_if_ne(wb, sdata + ob, ob, pb);
+        pa = oa, pb = ob;
       } else {
-        lds_sw(wa, ra + oa * kSuperwordBytes);
-        lds_sw(wb, rb + ob * kSuperwordBytes);
+        lds_sw(wa, sdata + oa);
+        lds_sw(wb, sdata + ob);
       }
-      add_pair(acc[j], wa, wb);
+      if constexpr (WIDE) add_wide(acc[j], hi[j], wa, wb); else add_pair(acc[j], wa, wb);
     }
   }
 }
@@ -149,8 +162,8 @@ __device__ __forceinline__ void add1(uint4& acc, const uint4& t) {
   acc.w += t.w;
 }
 
-template <int J, bool SHARE>
-__device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint4& t4,
+template <int J, bool SHARE, bool WIDE>
+__device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint4& t4,
                                             uint32_t& aa, uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits,
                                             uint32_t any) {
   if constexpr (J < kRD) {
@@ -179,16 +192,19 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4& wa, uint4&
     }
     if constexpr (SHARE) {
       add1(acc[J], t4);  // the quad's sum is unchanged since the last taken step: one term per word
+    } else if constexpr (WIDE) {
+      add_wide(acc[J], hi[J], wa, wb);
+      add_wide(acc[J], hi[J], wc, wd);
     } else {
       add_pair(acc[J], wa, wb);
       add_pair(acc[J], wc, wd);
     }
-    delta_steps<J + 1, SHARE>(acc, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
+    delta_steps<J + 1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
   }
 }
 
-template <bool SHARE>
-__device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes,
+template <bool SHARE, bool WIDE = false>
+__device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
                                             uint32_t meta_row) {
   uint4 m;
   lds_sw(m, smeta);
@@ -215,11 +231,14 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint32_t sdata, u
     if constexpr (SHARE) {
       sum4(t4, wa, wb, wc, wd);
       add1(acc[0], t4);
+    } else if constexpr (WIDE) {
+      add_wide(acc[0], hi[0], wa, wb);
+      add_wide(acc[0], hi[0], wc, wd);
     } else {
       add_pair(acc[0], wa, wb);
       add_pair(acc[0], wc, wd);
     }
-    delta_steps<1, SHARE>(acc, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
+    delta_steps<1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
   }
 }
 
@@ -265,43 +284,6 @@ __device__ __forceinline__ void stage_pairs(uint4 (&acc)[kRD], uint32_t sdata, u
     add_pair(acc[0], wa, wb);
     add_pair(acc[0], wc, wd);
     pair_steps<1>(acc, wa, wb, wc, wd, sdata, oa, ob, oc, od, m.x, any);
-  }
-}
-
-// uint16 lanes (kModeWide, NL = 8): a word w holds two uint16 samples with no headroom.  E += w (mod 2^32; one IADD3 for
-// two channels) and O += w >> 16 (one LEA.HI per channel) give the lane sums E - (O << 16) and O, exact while the channel
-// sum fits 32 bits (checked at plan creation).  Channels in pairs; per channel and trial group two table entries = eight
-// 32-bit byte offsets inside the stage (row included); a trial whose offset equals the previous trial's keeps the
-// registers (upper channels of a coarse grid still repeat delays).  Bound by shared memory: 2 bytes per add.
-__device__ __forceinline__ void add_wide(uint4& E, uint4& O, const uint4& a, const uint4& b) {
-  E.x = E.x + a.x + b.x, E.y = E.y + a.y + b.y, E.z = E.z + a.z + b.z, E.w = E.w + a.w + b.w;
-  O.x += a.x >> 16, O.y += a.y >> 16, O.z += a.z >> 16, O.w += a.w >> 16;
-  asm volatile("" : "+r"(O.x), "+r"(O.y), "+r"(O.z), "+r"(O.w));  // keeps each shift-add one LEA.HI
-  O.x += b.x >> 16, O.y += b.y >> 16, O.z += b.z >> 16, O.w += b.w >> 16;
-}
-__device__ __forceinline__ uint32_t word_of(const uint4& m, int j) { return j == 0 ? m.x : j == 1 ? m.y : j == 2 ? m.z : m.w; }
-
-__device__ __forceinline__ void stage_wide(uint4 (&E)[kRD], uint4 (&O)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
-                                           uint32_t meta_row) {
-#pragma unroll 1
-  for (int cc = 0; cc < Cc; cc += 2) {
-    uint4 ma[2], mb[2];
-    lds_sw(ma[0], smeta), lds_sw(ma[1], smeta + 16);
-    lds_sw(mb[0], smeta + meta_row), lds_sw(mb[1], smeta + meta_row + 16);
-    smeta += 2 * meta_row;
-    uint4 wa, wb;
-    uint32_t pa = ma[0].x, pb = mb[0].x;
-    lds_sw(wa, sdata + pa);
-    lds_sw(wb, sdata + pb);
-    add_wide(E[0], O[0], wa, wb);
-#pragma unroll
-    for (int j = 1; j < kRD; ++j) {
-      const uint32_t oa = word_of(ma[j >> 2], j & 3), ob = word_of(mb[j >> 2], j & 3);
-      lds_if_ne(wa, sdata + oa, oa, pa);
-      lds_if_ne(wb, sdata + ob, ob, pb);
-      pa = oa, pb = ob;
-      add_wide(E[j], O[j], wa, wb);
-    }
   }
 }
 
@@ -355,7 +337,7 @@ __device__ __forceinline__ void stage_bytes(uint4 (&e)[kRD16], uint4 (&r)[kRD16]
 // per-thread accumulators of the three lane widths
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void carry_save(uint32_t& lo, uint32_t& hi) {  // 16-bit lanes: hi += lo >> 8, lo &= 0xff
-  hi += (lo >> 8) & 0x00ff00ffu;
+  hi += __byte_perm(lo, 0u, 0x4341u);  // bytes 1 and 3 moved down in one PRMT (a shift and a mask are two ALU instructions)
   lo &= 0x00ff00ffu;
 }
 __device__ __forceinline__ void carry_save(uint4& lo, uint4& hi) {
@@ -376,11 +358,15 @@ struct Lanes<4> {  // four 32-bit lanes: plain sums
     for (int j = 0; j < kRD; ++j) acc[j] = make_uint4(0, 0, 0, 0);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row, uint32_t one) {
-    if constexpr (is_delta(MODE))
-      stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {
+    if constexpr (is_delta(MODE) || MODE == kModeHybrid)  // (a hybrid range: this call is one of its delta-coded chunks)
+      stage_delta<MODE == kModeDeltaShare>(acc, acc, sdata, smeta, Cc, meta_row);
     else
-      stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
+      stage_general<MODE == kModeGeneralReuse, false>(acc, acc, sdata, smeta, Cc, meta_row);
+  }
+  template <int MODE>
+  __device__ __forceinline__ void stage_rest(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {  // hybrid: the other chunks
+    stage_general<true, false>(acc, acc, sdata, smeta, Cc, meta_row);
   }
   __device__ __forceinline__ void flush() {}
   template <int MODE>
@@ -397,15 +383,19 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
     for (int j = 0; j < kRD; ++j) acc[j] = hi[j] = make_uint4(0, 0, 0, 0);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row, uint32_t one) {
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {
     if constexpr (MODE == kModeWide)
-      stage_wide(acc, hi, sdata, smeta, Cc, meta_row);  // acc = E, hi = O
+      stage_general<true, true>(acc, hi, sdata, smeta, Cc, meta_row);  // acc = E, hi = O
     else if constexpr (MODE == kModeDeltaPair)
       stage_pairs(acc, sdata, smeta, Cc, meta_row);
-    else if constexpr (is_delta(MODE))
-      stage_delta<MODE == kModeDeltaShare>(acc, sdata, smeta, Cc, row_bytes, meta_row);
+    else if constexpr (is_delta(MODE) || is_hybrid(MODE))  // (a hybrid range: this call is one of its delta-coded chunks)
+      stage_delta<MODE == kModeDeltaShare, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row);
     else
-      stage_general<MODE == kModeGeneralReuse>(acc, sdata, smeta, Cc, row_bytes, meta_row);
+      stage_general<MODE == kModeGeneralReuse, false>(acc, hi, sdata, smeta, Cc, meta_row);
+  }
+  template <int MODE>
+  __device__ __forceinline__ void stage_rest(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {  // hybrid: the other chunks
+    stage_general<true, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row);
   }
   __device__ __forceinline__ void flush() {
 #pragma unroll
@@ -414,7 +404,7 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
   template <int MODE>
   __device__ __forceinline__ void values(int j, uint32_t (&v)[8]) const {
     const uint32_t lo[4] = {acc[j].x, acc[j].y, acc[j].z, acc[j].w}, up[4] = {hi[j].x, hi[j].y, hi[j].z, hi[j].w};
-    if constexpr (MODE == kModeWide) {  // acc = E = sum of the words, hi = O = sum of their upper halves
+    if constexpr (is_wide(MODE)) {  // acc = E = sum of the words, hi = O = sum of their upper halves
 #pragma unroll
       for (int q = 0; q < 4; ++q) v[2 * q] = lo[q] - (up[q] << 16), v[2 * q + 1] = up[q];
       return;
@@ -435,9 +425,11 @@ struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upp
     for (int j = 0; j < kRD16; ++j) e[j] = r[j] = he[j] = hq[j] = make_uint4(0, 0, 0, 0);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t row_bytes, uint32_t meta_row, uint32_t one) {
+  __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {
     stage_bytes(e, r, sdata, smeta, Cc, meta_row, one);
   }
+  template <int MODE>
+  __device__ __forceinline__ void stage_rest(uint32_t, uint32_t, int, uint32_t) {}  // (no hybrid form on 8-bit lanes)
   // invariant: e = A0 | A2 << 16,  r = A1 + 2^8 A2 + 2^16 A3 (mod 2^32),  lane sum = A + 256 * (he | hq lane)
   static __device__ __forceinline__ void flush_word(uint32_t& e, uint32_t& r, uint32_t& he, uint32_t& hq) {
     uint32_t q = r - ((e >> 16) << 8);  // A1 | A3 << 16
@@ -490,6 +482,10 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const uint32_t row_bytes = (uint32_t)p.rowpitch * kSuperwordBytes;
   const uint32_t data_bytes = (uint32_t)p.Cc * row_bytes;
   const uint32_t meta_bytes = (uint32_t)tiled_meta_bytes(MODE, NL, p.Cc, p.G);
+  // hybrid ranges: chunks 0 .. nd-1 (the highest channels, whose delay steps never exceed 1) carry the delta table, the
+  // others the offsets table; a trial block's slices lie in that order
+  const uint32_t meta_bytes_d = (uint32_t)tiled_meta_bytes(kModeDelta, NL, p.Cc, p.G);
+  const int nd = is_hybrid(MODE) ? p.nd : 0;
   const uint32_t stage_bytes = (uint32_t)tiled_stage_bytes(MODE, NL, p.Cc, p.rowpitch, p.G);
   const uint32_t stage0 = bar_base + kBarRegion;
   const int nchunks = p.Cpad / p.Cc;
@@ -511,7 +507,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   // already satisfied.  Row start and length of the warp's NEXT chunk are fetched one turn early.
   const uint4* Pbeam = p.P + (long long)beam * p.Cpad * p.Wp + tau * p.T;
   const long long tab = (long long)blk * p.Cpad;
-  const char* meta_blk = reinterpret_cast<const char*>(p.meta) + (size_t)blk * (size_t)nchunks * meta_bytes;
+  const char* meta_blk = reinterpret_cast<const char*>(p.meta) +
+                         (size_t)blk * ((size_t)nd * meta_bytes_d + (size_t)(nchunks - nd) * meta_bytes);
   const int lane = tid & 31;
   const int warp = tid >> 5;
   constexpr int kWarps = NT / 32;
@@ -535,8 +532,10 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
     if (lane == 0) {
-      mbar_arrive_expect_tx(full, total + meta_bytes);
-      bulk_copy_g2s(sbase + data_bytes, meta_blk + (size_t)k * meta_bytes, meta_bytes, full);
+      const uint32_t mb = k < nd ? meta_bytes_d : meta_bytes;
+      const size_t moff = k < nd ? (size_t)k * meta_bytes_d : (size_t)nd * meta_bytes_d + (size_t)(k - nd) * meta_bytes;
+      mbar_arrive_expect_tx(full, total + mb);
+      bulk_copy_g2s(sbase + data_bytes, meta_blk + moff, mb, full);
     }
     __syncwarp();
     if (lane < p.Cc)
@@ -571,9 +570,10 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   Lanes<NL> lanes;
   lanes.init();
   const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
-  const uint32_t entry_bytes = MODE == kModeDeltaPair ? 80u : MODE == kModeWide ? 32u : 16u;  // table bytes per (channel | quad, trial group)
+  const uint32_t entry_bytes = MODE == kModeDeltaPair ? 80u : (!is_delta(MODE) && NL != 16) ? 32u : 16u;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
   const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
+  const uint32_t meta_row_d = (uint32_t)p.G * 16u, meta_off_d = data_bytes + (uint32_t)g * 16u;  // delta chunks of a hybrid range
   int since_flush = 0;
 
   int s = 0;        // stage of the chunk being consumed
@@ -586,14 +586,21 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     }
     mbar_wait(bar_base + 8u * s, ph);
     const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
-    lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, row_bytes, meta_row, p.one);
+    if constexpr (is_hybrid(MODE)) {
+      if (it < nd)
+        lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off_d, p.Cc, meta_row_d, p.one);
+      else
+        lanes.template stage_rest<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row);
+    } else {
+      lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
+    }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_base + 8u * (nstages + s));  // stage may be refilled
     if (++s == nstages) {
       s = 0;
       ph ^= 1u;
     }
-    if (NL != 4 && MODE != kModeWide && ++since_flush == p.flush_stages) {  // packed lanes could overflow next: move their upper bytes
+    if (NL != 4 && !is_wide(MODE) && ++since_flush == p.flush_stages) {  // packed lanes could overflow next: move their upper bytes
       since_flush = 0;
       lanes.flush();
     }
@@ -671,6 +678,8 @@ static cudaError_t set_smem_t() {
   X(8, kModeGeneral, 512) X(8, kModeGeneralReuse, 512) X(8, kModeDelta, 512)                   \
   X(8, kModeDeltaShare, 256) X(8, kModeDeltaShare, 512) X(4, kModeDeltaShare, 256) X(4, kModeDeltaShare, 512) \
   X(8, kModeDeltaPair, 256) X(8, kModeDeltaPair, 512) X(8, kModeWide, 256) X(8, kModeWide, 512)  \
+  X(8, kModeHybrid, 256) X(8, kModeHybrid, 512) X(4, kModeHybrid, 256) X(4, kModeHybrid, 512)   \
+  X(8, kModeWideHybrid, 256) X(8, kModeWideHybrid, 512)                                        \
   X(4, kModeGeneral, 256) X(4, kModeGeneralReuse, 256) X(4, kModeDelta, 256)                   \
   X(4, kModeGeneral, 512) X(4, kModeGeneralReuse, 512) X(4, kModeDelta, 512)                   \
   X(16, kModeGeneral, 256) X(16, kModeGeneral, 512)
@@ -705,6 +714,7 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.T = r.T;
   tp.Cc = r.Cc;
   tp.nstages = pairs ? r.stages2 : r.stages;
+  tp.nd = r.nd;
   tp.blk0 = blk0;
   tp.nblk = nblk;
   tp.rowpitch = pairs ? r.T + r.Smax2 : r.T + r.Smax;

@@ -193,6 +193,42 @@ def test_table_modes_agree_on_fine_dm_grid(mode):
     check_full(w, x, plan, flat)
 
 
+@pytest.mark.parametrize("bits,decim,step,tuning,mode,lanes", [
+    (8, 4, 0.9, None, 6, 8),              # x4 uint8: the lowest channels step by 1.09 samples per trial -> delta chunks + offsets chunks
+    (8, 1, 0.23, dict(mode=6), 6, 8),     # x1 uint8, 1.11 at the bottom (automatic: 8-bit lanes): hybrid on request
+    (16, 1, 0.23, dict(mode=6), 7, 8),    # x1 uint16 (automatic: uint16 lanes, offsets table): hybrid on the same lanes
+    (16, 4, 0.9, None, 6, 4),             # x4 uint16: 32-bit lanes
+])
+def test_hybrid_table_modes(bits, decim, step, tuning, mode, lanes):
+    """Ranges that are delta-codable except for their lowest channels (dd_internal.h kModeHybrid / kModeWideHybrid):
+    every output element against the oracle, with saturated rows on both sides of the chunk boundary; then the same
+    plan with the offsets table forced (mode 1), identical bits."""
+    nch, ns = 300, 2 ** 15 + 37
+    rng = np.random.default_rng(31 * bits + decim)
+    x = rng.integers(0, 2 ** bits, size=(2, nch, ns), dtype=np.uint8 if bits == 8 else np.uint16)
+    x[0, 40:60, :] = 2 ** bits - 1
+    x[1, 250:, 1000:20000] = 2 ** bits - 1
+    w = W.Workload("hybrid", 750.0, -200.0 / nch, nch, 1.31072e-3, ns, 2, bits, (W.DMRange(100.0, step, 150, decim),), 1, 0, 0)
+    plan, flat = gpu_run(w, x, TILED, tuning=tuning)
+    info = plan.tile_info(0)
+    assert (info["mode"], info["lanes"]) == (mode, lanes), info
+    nd, shape = plan.delta_chunks(0), plan.tile_shape(0)
+    assert 0 < nd < shape["cpad"] // shape["chans_per_stage"]
+    check_full(w, x, plan, flat)
+    plan2, flat2 = gpu_run(w, x, TILED, tuning=dict(mode=1, byte_lanes=0))
+    assert plan2.tile_info(0)["mode"] == 1
+    assert np.array_equal(flat.view(np.uint32)[flat != -1.0], flat2.view(np.uint32)[flat2 != -1.0])
+
+
+def test_hybrid_forced_on_a_coarse_grid_with_few_delta_chunks():
+    """dd_tuning_t::mode = 6 on a config-2-shaped range: only the first chunks qualify; several trial blocks and tiles."""
+    w = W.scaled(W.CONFIGS[2], nchans=200, nsamps=2 ** 15, ranges=[W.DMRange(0.0, 0.5, 301, 1)])
+    x = W.generate(w)
+    plan, flat = gpu_run(w, x, TILED, tuning=dict(mode=6, byte_lanes=0))
+    assert plan.tile_info(0)["mode"] == 6 and plan.delta_chunks(0) >= 1
+    check_full(w, x, plan, flat)
+
+
 def test_delta_mode_is_refused_for_coarse_dm_grid():
     """Delay steps above 1 cannot be delta coded: the plan falls back to the offsets table."""
     w = W.scaled(W.CONFIGS[2], nchans=64, nsamps=2 ** 14, ranges=[W.DMRange(0.0, 2.0, 40, 1)])
@@ -331,7 +367,7 @@ def test_shared_partial_sums_variant():
                  ranges=[W.DMRange(0.0, 0.1, 203, 1), W.DMRange(200.0, 0.2, 150, 2), W.DMRange(600.0, 3.0, 41, 4)])
     x = W.generate(w)
     plan, flat = gpu_run(w, x, SHARED)
-    assert [plan.tile_info(r)["mode"] for r in range(3)] == [2, 2, 0]
+    assert [plan.tile_info(r)["mode"] for r in range(3)] == [2, 2, 6]   # (the coarse x4 range: hybrid, not shared)
     check_full(w, x, plan, flat)
     # saturated input: the quad sum 4*1020 still fits its 16-bit lane
     xs = np.full_like(x, 255)

@@ -29,39 +29,45 @@ def _padded_delays(plan, r, shape, rd):
 
 
 def _decode(plan, r):
-    """Delays implied by the kernel tables: [nblocks][Dcta][Cpad] (absolute, superwords)."""
+    """Delays implied by the kernel tables: [nblocks][Dcta][Cpad] (absolute, superwords).  A trial block holds the
+    table slices of its channel chunks one after the other: the first `delta_chunks` in the delta form (one 4-word
+    entry per channel quad and trial group), the others as one 32-bit byte offset per (channel, trial)."""
     info, shape = plan.tile_info(r), plan.tile_shape(r)
     rd = 4 if info["lanes"] == 16 else 8
     g, cc, cpad, rowp, nb = (shape[k] for k in ("trial_groups", "chans_per_stage", "cpad", "row_superwords", "nblocks"))
-    meta = plan.table(r, 0)
+    nchunks, nd = cpad // cc, plan.delta_chunks(r)
+    assert nd == (nchunks if info["mode"] == 2 else nd) and (nd == 0 or info["mode"] in (2, 6, 7))
+    assert 0 < nd < nchunks if info["mode"] in (6, 7) else True
+    meta = plan.table(r, 0).astype(np.int64)
     dmin = plan.table(r, 1).astype(np.int64).reshape(nb, cpad)
     span = plan.table(r, 2).astype(np.int64).reshape(nb, cpad)
+    wd, wg = cc // 4 * g * 4, cc * g * rd
+    assert meta.size == nb * (nd * wd + (nchunks - nd) * wg)
+    meta = meta.reshape(nb, nd * wd + (nchunks - nd) * wg)
     rowoff = (np.arange(cpad) % cc) * rowp                                    # superwords, row of the channel in its stage
-    if info["mode"] == 2:                                                     # delta table, one entry per channel quad
-        e = meta.reshape(nb, cpad // 4, g, 4).astype(np.int64)
-        rel = np.zeros((nb, g, rd, cpad), dtype=np.int64)
-        anyb = np.zeros((nb, cpad // 4, g), dtype=np.int64)
+    rel = np.zeros((nb, g, rd, cpad), dtype=np.int64)
+    cd = nd * cc                                                              # channels under the delta form
+    if nd:
+        e = meta[:, :nd * wd].reshape(nb, cd // 4, g, 4)
+        anyb = np.zeros((nb, cd // 4, g), dtype=np.int64)
         for q in range(4):
             field = (e[..., 1 + q // 2] >> (16 * (q % 2))) & 0xFFFF           # [nb][quad][g] byte offset in the stage
             assert (field % 16 == 0).all()
-            first = field // 16 - rowoff[q::4][None, :, None]
+            first = field // 16 - rowoff[q:cd:4][None, :, None]
             cur = first.copy()
-            rel[:, :, 0, q::4] = first.transpose(0, 2, 1)
+            rel[:, :, 0, q:cd:4] = first.transpose(0, 2, 1)
             for j in range(1, rd):
                 n = (j - 1) * 4 + q
                 bit = (e[..., 0] >> ((n // 7) * 8 + n % 7)) & 1
                 anyb |= bit << j
                 cur = cur + bit
-                rel[:, :, j, q::4] = cur.transpose(0, 2, 1)
+                rel[:, :, j, q:cd:4] = cur.transpose(0, 2, 1)
         assert np.array_equal(anyb, e[..., 3]), "any-changed bits are the OR of the quad's changed bits"
         assert (e[..., 0] & 0x80808080 == 0).all()                            # bit 7 of each byte is unused
-    elif info["lanes"] == 16 or info["mode"] == 5:                            # 32-bit byte offsets, row included
-        e = meta.reshape(nb, cpad, g, rd).astype(np.int64)
+    if nd < nchunks:                                                          # 32-bit byte offsets, row included
+        e = meta[:, nd * wd:].reshape(nb, cpad - cd, g, rd)
         assert (e % 16 == 0).all()
-        rel = (e // 16 - rowoff[None, :, None, None]).transpose(0, 2, 3, 1)
-    else:                                                                     # 16-bit superword offsets
-        e = meta.view(np.uint16).reshape(nb, cpad, g, 8).astype(np.int64)
-        rel = e.transpose(0, 2, 3, 1)
+        rel[:, :, :, cd:] = (e // 16 - rowoff[None, cd:, None, None]).transpose(0, 2, 3, 1)
     assert (rel >= 0).all() and (rel <= span[:, None, None, :]).all(), "every load stays inside the staged row"
     assert (dmin % 8 == 0).all() and (span % 8 == 0).all(), "staged rows start and end on 128-byte lines"
     assert (span + info["words_per_cta"] <= rowp).all()
@@ -81,8 +87,9 @@ def test_kernel_tables_reproduce_the_delay_table(cfg):
         assert np.array_equal(got, _padded_delays(plan, r, shape, rd)), (cfg, r)
         # shared memory of the launch: ring + barriers + prefetch pad fits the 227 KB opt-in limit
         mode = plan.tile_info(r)["mode"]
-        meta_stage = (shape["chans_per_stage"] // 4 if mode == 2 else shape["chans_per_stage"]) \
-            * shape["trial_groups"] * (32 if mode == 5 else 16)
+        rd = 4 if plan.tile_info(r)["lanes"] == 16 else 8
+        meta_stage = shape["chans_per_stage"] // 4 * shape["trial_groups"] * 16 if mode == 2 else \
+            shape["chans_per_stage"] * shape["trial_groups"] * rd * 4
         stage = -(-(shape["chans_per_stage"] * shape["row_superwords"] * 16 + meta_stage) // 128) * 128
         assert 128 + shape["stages"] * stage + 512 <= 227 * 1024 and shape["stages"] >= 2
     plan.destroy()
@@ -92,13 +99,13 @@ def test_lane_widths_and_modes_of_the_five_configs():
     """Which adder each range gets: delta-coded 16-bit lanes for the fine DM grids of
     config 3, 8-bit lanes for undecimated coarse grids of uint8 data, uint16 lanes for undecimated uint16 data, 32-bit
     lanes for decimated uint16."""
-    want = {1: [(16, 0)], 2: [(16, 0)], 3: [(8, 2), (8, 2), (8, 2)], 4: [(8, 5), (4, None)], 5: [(16, 0)]}
+    want = {1: [(16, 0)], 2: [(16, 0)], 3: [(8, 2), (8, 2), (8, 2)], 4: [(8, 5), (4, 6)], 5: [(16, 0)]}
     for cfg, exp in want.items():
         plan = _host_plan(W.CONFIGS[cfg])
         for r, (lanes, mode) in enumerate(exp):
             info = plan.tile_info(r)
             assert info["lanes"] == lanes and (mode is None or info["mode"] == mode), (cfg, r, info)
-            if lanes == 8 and info["mode"] == 5:
+            if lanes == 8 and info["mode"] in (5, 7):
                 assert info["flush_chans"] == 0   # E (mod 2^32) and O never overflow: no flush
             elif lanes == 8:   # 255 + flush*maxval <= 65535, at most 256 flushes
                 maxval = 255 * plan.ranges[r][3]
@@ -106,6 +113,41 @@ def test_lane_widths_and_modes_of_the_five_configs():
                 assert -(-plan.tile_shape(r)["cpad"] // info["flush_chans"]) <= 256
         assert plan.launches() == 2 * len(exp)   # one pack and one dedispersion launch per range
         plan.destroy()
+
+
+def test_hybrid_tables_where_only_the_lowest_channels_step_by_more_than_one():
+    """The mode cliff: a DM step a little too coarse for the lowest channels.  A decimated range keeps the
+    delta table for the chunks of channels above them (kModeHybrid) instead of dropping to the offsets table
+    altogether; undecimated data stays on 8-bit (uint8) or uint16 lanes unless the hybrid form is asked for
+    (dd_tuning_t::mode = 6: packed 16-bit lanes for uint8, uint16 lanes for uint16); a forced table form switches it off."""
+    w3 = W.CONFIGS[3]
+    cases = [  # (bits, (dm_lo, step, ndm, decim), tuning, expected mode, lanes)
+        (8, (600.0, 0.9, 600, 4), None, 6, 8),              # x4: lowest-channel step 1.09 samples per trial
+        (8, (0.0, 0.23, 600, 1), None, 0, 16),              # x1 uint8, step 1.11 at the bottom: byte lanes
+        (8, (0.0, 0.23, 600, 1), dict(mode=6), 6, 8),       # ... hybrid on request
+        (16, (0.0, 0.23, 600, 1), None, 5, 8),              # x1 uint16: uint16 lanes
+        (16, (0.0, 0.23, 600, 1), dict(mode=6), 7, 8),      # ... hybrid on request, same lanes
+        (16, (600.0, 0.9, 600, 4), None, 6, 4),             # x4 uint16: 32-bit lanes, hybrid
+    ]
+    for bits, rg, tuning, mode, lanes in cases:
+        p = B.Plan(w3.f_top_mhz, -200.0 / 1032, 1024 + 8, w3.tsamp_s, 2 ** 16, [rg], in_bits=bits, host_only=True,
+                   tuning=tuning)
+        info = p.tile_info(0)
+        assert (info["mode"], info["lanes"]) == (mode, lanes), (bits, rg, info)
+        got, rd, shape = _decode(p, 0)
+        assert np.array_equal(got, _padded_delays(p, 0, shape, rd))
+        if mode in (6, 7):
+            nd, cc = p.delta_chunks(0), shape["chans_per_stage"]
+            d = p.get_delays(0).astype(np.int64)
+            steps = np.diff(d, axis=0)
+            steps[7::8] = 0                                  # the first trial of a group always loads
+            first_bad = int(np.argmax(steps.max(axis=0) > 1))
+            assert nd == first_bad // cc and 0 < nd < shape["cpad"] // cc
+            forced = B.Plan(w3.f_top_mhz, -200.0 / 1032, 1024 + 8, w3.tsamp_s, 2 ** 16, [rg], in_bits=bits,
+                            host_only=True, tuning=dict(mode=1, byte_lanes=0))
+            assert forced.tile_info(0)["mode"] == 1 and forced.delta_chunks(0) == 0
+            forced.destroy()
+        p.destroy()
 
 
 def test_ascending_band_has_the_descending_delay_table():
