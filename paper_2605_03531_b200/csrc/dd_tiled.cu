@@ -64,6 +64,25 @@ __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4
   acc.z = acc.z + a.z + b.z;
   acc.w = acc.w + a.w + b.w;
 }
+// The delta kernel is bound by the ALU pipe (IADD3, LOP3, R2P, the predicated address steps: 79 % busy) while the
+// FMA-side pipe idles, so part of the adds of every trial step go there as IMADs (two per IADD3 they replace: more issue
+// slots, fewer ALU slots).  Words of the quad's second channel pair moved, config 3: 0: 111.8 ms, 1: 110.8, 2: 109.2,
+// 3: 109.1, 4: 112.6 (issue slots and shared memory take over).
+constexpr int kDeltaFmaWords = 2;
+// acc += t on the FMA-side pipe: IMAD with a multiplier of one that ptxas cannot fold (a kernel parameter)
+__device__ __forceinline__ uint32_t mad1(uint32_t t, uint32_t one, uint32_t e) {
+  uint32_t d;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(t), "r"(one), "r"(e));
+  return d;
+}
+// add_pair with the first NW words of the superword added by two IMADs each instead of one IADD3
+template <int NW>
+__device__ __forceinline__ void add_pair_mix(uint4& acc, const uint4& a, const uint4& b, uint32_t one) {
+  acc.x = NW > 0 ? mad1(b.x, one, mad1(a.x, one, acc.x)) : acc.x + a.x + b.x;
+  acc.y = NW > 1 ? mad1(b.y, one, mad1(a.y, one, acc.y)) : acc.y + a.y + b.y;
+  acc.z = NW > 2 ? mad1(b.z, one, mad1(a.z, one, acc.z)) : acc.z + a.z + b.z;
+  acc.w = NW > 3 ? mad1(b.w, one, mad1(a.w, one, acc.w)) : acc.w + a.w + b.w;
+}
 struct TiledParams {
   const uint4* P;       // packed input of this range [nbeams][Cpad][Wp]
   const uint4* meta;    // per trial block: offsets / changed bits (dd_internal.h RangePlan::d_meta)
@@ -165,7 +184,7 @@ __device__ __forceinline__ void add1(uint4& acc, const uint4& t) {
 template <int J, bool SHARE, bool WIDE>
 __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint4& wa, uint4& wb, uint4& wc, uint4& wd, uint4& t4,
                                             uint32_t& aa, uint32_t& ab, uint32_t& ac, uint32_t& ad, uint32_t bits,
-                                            uint32_t any) {
+                                            uint32_t any, uint32_t one) {
   if constexpr (J < kRD) {
     // A predicated-off LDS still occupies a slot of the shared-memory data pipe (ncu: one wavefront per
     // skipped load, 36 % of the pipe in the first version), so the whole trial step of the quad is skipped
@@ -197,15 +216,15 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
       add_wide(acc[J], hi[J], wc, wd);
     } else {
       add_pair(acc[J], wa, wb);
-      add_pair(acc[J], wc, wd);
+      add_pair_mix<kDeltaFmaWords>(acc[J], wc, wd, one);
     }
-    delta_steps<J + 1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
+    delta_steps<J + 1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any, one);
   }
 }
 
 template <bool SHARE, bool WIDE = false>
 __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
-                                            uint32_t meta_row) {
+                                            uint32_t meta_row, uint32_t one) {
   uint4 m;
   lds_sw(m, smeta);
 #pragma unroll 1
@@ -236,9 +255,9 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
       add_wide(acc[0], hi[0], wc, wd);
     } else {
       add_pair(acc[0], wa, wb);
-      add_pair(acc[0], wc, wd);
+      add_pair_mix<kDeltaFmaWords>(acc[0], wc, wd, one);
     }
-    delta_steps<1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any);
+    delta_steps<1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any, one);
   }
 }
 
@@ -301,11 +320,6 @@ __device__ __forceinline__ void stage_pairs(uint4 (&acc)[kRD], uint32_t sdata, u
 // (Measured alternatives: the shift-add as IMAD.HI or IMAD.WIDE is slower -- ptxas adds register moves or splits it
 // into a multiply plus 64-bit adds; lanes 1 and 3 of one word in four by IDP4A with one-hot selectors into plain
 // 32-bit sums, which takes two more instructions off the ALU pipe, is slower too: 5.03 / 294.0 ms.)
-__device__ __forceinline__ uint32_t mad1(uint32_t t, uint32_t one, uint32_t e) {
-  uint32_t d;
-  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(t), "r"(one), "r"(e));
-  return d;
-}
 __device__ __forceinline__ void add_bytes(uint4& e, uint4& r, const uint4& a, const uint4& b, uint32_t one) {
   e.x = mad1(b.x & 0x00ff00ffu, one, mad1(a.x & 0x00ff00ffu, one, e.x));
   e.y = mad1(b.y & 0x00ff00ffu, one, mad1(a.y & 0x00ff00ffu, one, e.y));
@@ -360,7 +374,7 @@ struct Lanes<4> {  // four 32-bit lanes: plain sums
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {
     if constexpr (is_delta(MODE) || MODE == kModeHybrid)  // (a hybrid range: this call is one of its delta-coded chunks)
-      stage_delta<MODE == kModeDeltaShare>(acc, acc, sdata, smeta, Cc, meta_row);
+      stage_delta<MODE == kModeDeltaShare>(acc, acc, sdata, smeta, Cc, meta_row, one);
     else
       stage_general<MODE == kModeGeneralReuse, false>(acc, acc, sdata, smeta, Cc, meta_row);
   }
@@ -389,7 +403,7 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
     else if constexpr (MODE == kModeDeltaPair)
       stage_pairs(acc, sdata, smeta, Cc, meta_row);
     else if constexpr (is_delta(MODE) || is_hybrid(MODE))  // (a hybrid range: this call is one of its delta-coded chunks)
-      stage_delta<MODE == kModeDeltaShare, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row);
+      stage_delta<MODE == kModeDeltaShare, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row, one);
     else
       stage_general<MODE == kModeGeneralReuse, false>(acc, hi, sdata, smeta, Cc, meta_row);
   }
