@@ -256,7 +256,10 @@ int dd_plan_tile_shape(const dd_plan_t* plan, int32_t r, int32_t* trial_groups, 
  * channel) (int32 superwords, multiple of 8), 2: its length beyond the time tile (int32).  After
  * dd_plan_set_kernel(DD_KERNEL_SUBBAND): 3 = the pair-mode table (per trial block, quad of pairs and trial group 20
  * words: changed bits, any bits, 0, 0, then eight 16-bit byte offsets per pair), 4, 5 = start / span per staged row
- * (rows 2v, 2v+1 = the two pre-summed rows of pair v), 6 = delta_v per pair (int32).  *bytes = size; the table is copied when host_buf != NULL
+ * (rows 2v, 2v+1 = the two pre-summed rows of pair v), 6 = delta_v per pair (int32).  7 = the channel whose packed row is
+ * staged in each row of a trial block's chunk sequence (int32 [trial blocks][channel rows]; a permutation inside every
+ * delta-coded chunk, chosen so that channels whose delays change at the same trials share a quad; tables 0 - 2 are
+ * indexed by that row).  *bytes = size; the table is copied when host_buf != NULL
  * (DD_ERR_NOMEM if cap_bytes is too small). */
 int dd_plan_table(const dd_plan_t* plan, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes);
 

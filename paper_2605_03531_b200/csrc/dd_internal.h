@@ -111,10 +111,12 @@ struct RangePlan {
   // tables of the tiled kernel: host copies (built by dd_plan.cu build_tables) and their device twins
   std::vector<uint32_t> h_meta;
   std::vector<int32_t> h_dmin, h_span;
+  std::vector<int32_t> h_chan;  // [nblocks][Cpad] channel whose packed row is staged in row s of the block's chunk sequence
   uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] RD 32-bit byte offsets inside the stage;
                                 // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits}
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
+  int32_t* d_chan = nullptr;    // [nblocks][Cpad] h_chan
   int32_t* d_delays = nullptr;  // [ndm][nchans], only for the direct kernel (lazy)
   // two-channel sub-bands (kModeDeltaPair), built by dd_plan_set_kernel(DD_KERNEL_SUBBAND): rows are pairs
   int pair_ok = 0;        // 1: this range runs in pair mode under DD_KERNEL_SUBBAND

@@ -300,20 +300,56 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
   meta.assign((size_t)r.nblocks * words_per_block, 0);
   // rows past nchans are the zero rows of the packed input: delay 0 for every trial
   auto delay = [&](int j, int c) { return c < p.nchans ? r.delays[(size_t)std::min(r.ndm - 1, j) * p.nchans + c] : 0; };
+  // Which channel sits in which row of a stage.  The sum runs over all channels, so their order is free, per trial
+  // block.  In the delta form a trial step of a channel QUAD costs shared-memory slots and issue slots as soon as one
+  // of its four channels changes its delay, so the channels of a chunk are dealt to quads by the fractional part of
+  // their (unrounded) delay at the middle trial of the block: channels that cross a rounding boundary at the same
+  // trials share a quad.  Config 3: quad steps with a change 42 / 54 / 57 % -> 27 / 28 / 33 % (ranges 0 / 1 / 2).
+  std::vector<int32_t>& chan = r.h_chan;
+  chan.resize(nbc);
+  for (int b = 0; b < r.nblocks; ++b)
+    for (int c = 0; c < r.Cpad; ++c) chan[(size_t)b * r.Cpad + c] = c;
+  if (nd > 0) {
+    const double ts = p.tsamp * (double)r.decim, inv_top = 1.0 / (p.f_top * p.f_top);
+    std::vector<double> phase(r.Cc);
+    std::vector<int32_t> order(r.Cc);
+    for (int b = 0; b < r.nblocks; ++b) {
+      const int jm = std::min(r.ndm - 1, b * r.Dcta + r.Dcta / 2);
+      const double dm = r.dm_lo + (double)jm * r.dm_step;
+      for (size_t k = 0; k < nd; ++k) {
+        for (int i = 0; i < r.Cc; ++i) {
+          const int c = (int)k * r.Cc + i;
+          order[i] = c;
+          if (c < p.nchans) {
+            const double f = p.f_top + (double)c * p.cw;
+            const double x = kDispersion * dm * (1.0 / (f * f) - inv_top) / ts + 0.5;
+            phase[i] = x - floor(x);
+          } else {
+            phase[i] = -1.0;  // zero rows never change: last
+          }
+        }
+        std::stable_sort(order.begin(), order.end(), [&](int32_t u, int32_t v) {
+          return phase[u - (int)k * r.Cc] > phase[v - (int)k * r.Cc];
+        });
+        for (int i = 0; i < r.Cc; ++i) chan[(size_t)b * r.Cpad + k * r.Cc + i] = order[i];
+      }
+    }
+  }
   for (int b = 0; b < r.nblocks; ++b) {
     const int j0 = b * r.Dcta;
-    for (int c = 0; c < r.Cpad; ++c) {
+    for (int s = 0; s < r.Cpad; ++s) {  // s = row of the staged chunk sequence, c = the channel that sits there
+      const int c = chan[(size_t)b * r.Cpad + s];
       const int32_t d0 = delay(j0, c) & ~7;  // delays are non-decreasing in j
-      dmin[(size_t)b * r.Cpad + c] = d0;
-      span[(size_t)b * r.Cpad + c] = (int32_t)round_up(delay(j0 + r.Dcta - 1, c) - d0, 8);
-      if (span[(size_t)b * r.Cpad + c] > r.Smax) r.tiled_ok = 0;  // cannot happen (Smax is this maximum); never overrun a row
+      dmin[(size_t)b * r.Cpad + s] = d0;
+      span[(size_t)b * r.Cpad + s] = (int32_t)round_up(delay(j0 + r.Dcta - 1, c) - d0, 8);
+      if (span[(size_t)b * r.Cpad + s] > r.Smax) r.tiled_ok = 0;  // cannot happen (Smax is this maximum); never overrun a row
       for (int g = 0; g < r.G; ++g) {
         const int jg = j0 + g * r.RD;
-        const size_t k = (size_t)c / r.Cc, ci = (size_t)c % r.Cc;
+        const size_t k = (size_t)s / r.Cc, si = (size_t)s % r.Cc;
         if (k < nd) {
-          uint32_t* e = &meta[(size_t)b * words_per_block + k * wd + ((ci / 4) * r.G + g) * 4];
-          const int q = c % 4;
-          const uint32_t off = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg, c) - d0)) * 16u;
+          uint32_t* e = &meta[(size_t)b * words_per_block + k * wd + ((si / 4) * r.G + g) * 4];
+          const int q = s % 4;
+          const uint32_t off = ((uint32_t)si * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg, c) - d0)) * 16u;
           e[1 + q / 2] |= off << (16 * (q % 2));  // byte offset inside the stage, < 64 KB (choose_tile)
           for (int j = 1; j < r.RD; ++j)
             if (delay(jg + j, c) != delay(jg + j - 1, c)) {
@@ -321,9 +357,9 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
               e[3] |= 1u << j;  // some channel of the quad changes at this trial step
             }
         } else {
-          uint32_t* e = &meta[(size_t)b * words_per_block + nd * wd + (k - nd) * wg + (ci * r.G + g) * r.RD];
+          uint32_t* e = &meta[(size_t)b * words_per_block + nd * wd + (k - nd) * wg + (si * r.G + g) * r.RD];
           for (int j = 0; j < r.RD; ++j)  // byte offsets inside the stage, row of the channel included
-            e[j] = ((uint32_t)(c % r.Cc) * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg + j, c) - d0)) * 16u;
+            e[j] = ((uint32_t)si * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg + j, c) - d0)) * 16u;
         }
       }
     }
@@ -337,6 +373,8 @@ int upload_tables(dd::RangePlan& r) {
   DD_CUDA(cudaMemcpy(r.d_meta, r.h_meta.data(), r.h_meta.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
   DD_CUDA(cudaMemcpy(r.d_dmin, r.h_dmin.data(), r.h_dmin.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   DD_CUDA(cudaMemcpy(r.d_span, r.h_span.data(), r.h_span.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMalloc(&r.d_chan, r.h_chan.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMemcpy(r.d_chan, r.h_chan.data(), r.h_chan.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   return DD_OK;
 }
 
@@ -626,6 +664,7 @@ int dd_plan_destroy(dd_plan_t* p) {
     if (r.d_meta) cudaFree(r.d_meta);
     if (r.d_dmin) cudaFree(r.d_dmin);
     if (r.d_span) cudaFree(r.d_span);
+    if (r.d_chan) cudaFree(r.d_chan);
     if (r.d_delays) cudaFree(r.d_delays);
     if (r.d_meta2) cudaFree(r.d_meta2);
     if (r.d_dmin2) cudaFree(r.d_dmin2);
@@ -1048,13 +1087,13 @@ int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* m
 }
 
 int dd_plan_table(const dd_plan_t* p, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes) {
-  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 6) return DD_ERR_INVALID;
+  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 7) return DD_ERR_INVALID;
   const auto& q = p->ranges[r];
-  const void* srcs[7] = {q.h_meta.data(), q.h_dmin.data(), q.h_span.data(), q.h_meta2.data(), q.h_dmin2.data(),
-                         q.h_span2.data(), q.h_delta.data()};
-  const size_t sizes[7] = {q.h_meta.size(), q.h_dmin.size(), q.h_span.size(), q.h_meta2.size(), q.h_dmin2.size(),
-                           q.h_span2.size(), q.h_delta.size()};
-  if (which >= 3 && !q.pair_ok) return DD_ERR_INVALID;
+  const void* srcs[8] = {q.h_meta.data(), q.h_dmin.data(), q.h_span.data(), q.h_meta2.data(), q.h_dmin2.data(),
+                         q.h_span2.data(), q.h_delta.data(), q.h_chan.data()};
+  const size_t sizes[8] = {q.h_meta.size(), q.h_dmin.size(), q.h_span.size(), q.h_meta2.size(), q.h_dmin2.size(),
+                           q.h_span2.size(), q.h_delta.size(), q.h_chan.size()};
+  if (which >= 3 && which <= 6 && !q.pair_ok) return DD_ERR_INVALID;
   const void* src = srcs[which];
   const size_t n = sizes[which] * 4;
   *bytes = (int64_t)n;

@@ -88,6 +88,7 @@ struct TiledParams {
   const uint4* meta;    // per trial block: offsets / changed bits (dd_internal.h RangePlan::d_meta)
   const int32_t* dmin;  // [nblocks][Cpad] first delay of the block = start of the staged row
   const int32_t* span;  // [nblocks][Cpad] delay spread of the block = staged row length beyond T
+  const int32_t* chan;  // [nblocks][Cpad] channel (row of P) staged in that row, or nullptr: the row index itself
   float* out;           // beam 0, this range
   long long out_beam_stride, pitch, Wp, H, nout, ntau;
   int ndm, Cpad, G, T, Cc, nstages;
@@ -527,7 +528,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const int warp = tid >> 5;
   constexpr int kWarps = NT / 32;
   const int ahead = nstages - 2;
-  int pf_d0 = 0;
+  int pf_d0 = 0, pf_row = 0;
   uint32_t pf_bytes = 0;
   auto prefetch = [&](int k) {
     pf_bytes = 0;
@@ -535,6 +536,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
       const int c = k * p.Cc + lane;
       pf_d0 = __ldg(p.dmin + tab + c);
       pf_bytes = (uint32_t)(p.T + __ldg(p.span + tab + c)) * kSuperwordBytes;
+      pf_row = p.chan ? __ldg(p.chan + tab + c) : c;
     }
   };
   // stage and wrap count of a chunk index are tracked incrementally (no divisions in the main loop)
@@ -553,7 +555,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     }
     __syncwarp();
     if (lane < p.Cc)
-      bulk_copy_g2s(sbase + lane * row_bytes, Pbeam + (long long)(k * p.Cc + lane) * p.Wp + pf_d0, pf_bytes, full);
+      bulk_copy_g2s(sbase + lane * row_bytes, Pbeam + (long long)pf_row * p.Wp + pf_d0, pf_bytes, full);
   };
   // this warp's chunks are warp, warp + kWarps, ...; (my_k, my_s, my_w) is the next one it has to issue
   int my_k = warp, my_s = warp % nstages;
@@ -715,6 +717,7 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.meta = pairs ? r.d_meta2 : r.d_meta;
   tp.dmin = pairs ? r.d_dmin2 : r.d_dmin;
   tp.span = pairs ? r.d_span2 : r.d_span;
+  tp.chan = pairs ? nullptr : r.d_chan;
   tp.out = out_dev + r.offset;
   tp.out_beam_stride = p->beam_stride;
   tp.pitch = r.pitch;

@@ -71,8 +71,15 @@ def _decode(plan, r):
     assert (rel >= 0).all() and (rel <= span[:, None, None, :]).all(), "every load stays inside the staged row"
     assert (dmin % 8 == 0).all() and (span % 8 == 0).all(), "staged rows start and end on 128-byte lines"
     assert (span + info["words_per_cta"] <= rowp).all()
-    absd = rel + dmin[:, None, None, :]
-    return absd.reshape(nb * g * rd, cpad), rd, shape
+    absd = rel + dmin[:, None, None, :]                                      # [nb][g][rd][row of the chunk sequence]
+    # which channel each row holds (dd_plan_table 7): a permutation inside every chunk, the identity outside the delta form
+    chan = plan.table(r, 7).astype(np.int64).reshape(nb, cpad)
+    assert np.array_equal(np.sort(chan.reshape(nb, nchunks, cc), axis=2),
+                          np.broadcast_to(np.arange(cpad).reshape(nchunks, cc), (nb, nchunks, cc)))
+    assert np.array_equal(chan[:, cd:], np.broadcast_to(np.arange(cd, cpad), (nb, cpad - cd)))
+    bych = np.empty_like(absd)
+    np.put_along_axis(bych, np.broadcast_to(chan[:, None, None, :], absd.shape), absd, axis=3)
+    return bych.reshape(nb * g * rd, cpad), rd, shape
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
