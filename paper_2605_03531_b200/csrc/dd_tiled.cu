@@ -66,9 +66,10 @@ __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4
 }
 // The delta kernel is bound by the ALU pipe (IADD3, LOP3, R2P, the predicated address steps: 79 % busy) while the
 // FMA-side pipe idles, so part of the adds of every trial step go there as IMADs (two per IADD3 they replace: more issue
-// slots, fewer ALU slots).  Words of the quad's second channel pair moved, config 3: 0: 111.8 ms, 1: 110.8, 2: 109.2,
-// 3: 109.1, 4: 112.6 (issue slots and shared memory take over).
-constexpr int kDeltaFmaWords = 2;
+// slots, fewer ALU slots).  Words per quad and trial step (of 8) moved, config 3: 0: 111.8 ms, 1: 110.8, 2: 109.2,
+// 3: 109.1, 4: 112.6 (issue slots and shared memory take over); with the channels dealt to quads by phase (dd_plan.cu
+// build_tables) 1: 103.5, 2: 102.1, 3: 100.7, 4: 104.1, 5: 109.2.
+constexpr int kDeltaFmaWords = 3;
 // acc += t on the FMA-side pipe: IMAD with a multiplier of one that ptxas cannot fold (a kernel parameter)
 __device__ __forceinline__ uint32_t mad1(uint32_t t, uint32_t one, uint32_t e) {
   uint32_t d;
@@ -216,7 +217,7 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
       add_wide(acc[J], hi[J], wa, wb);
       add_wide(acc[J], hi[J], wc, wd);
     } else {
-      add_pair(acc[J], wa, wb);
+      add_pair_mix<kDeltaFmaWords - 4>(acc[J], wa, wb, one);
       add_pair_mix<kDeltaFmaWords>(acc[J], wc, wd, one);
     }
     delta_steps<J + 1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any, one);
@@ -255,7 +256,7 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
       add_wide(acc[0], hi[0], wa, wb);
       add_wide(acc[0], hi[0], wc, wd);
     } else {
-      add_pair(acc[0], wa, wb);
+      add_pair_mix<kDeltaFmaWords - 4>(acc[0], wa, wb, one);
       add_pair_mix<kDeltaFmaWords>(acc[0], wc, wd, one);
     }
     delta_steps<1, SHARE, WIDE>(acc, hi, wa, wb, wc, wd, t4, aa, ab, ac, ad, bits, any, one);
