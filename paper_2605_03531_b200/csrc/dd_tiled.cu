@@ -130,8 +130,12 @@ __device__ __forceinline__ uint32_t word_of(const uint4& m, int j) { return j ==
 // uint16 lanes (kModeWide, NL = 8): a word w holds two uint16 samples with no headroom.  E += w (mod 2^32; one IADD3 for
 // two channels) and O += w >> 16 (one LEA.HI per channel) give the lane sums E - (O << 16) and O, exact while the channel
 // sum fits 32 bits (checked at plan creation).  Bound by shared memory: 2 bytes per add.
-__device__ __forceinline__ void add_wide(uint4& E, uint4& O, const uint4& a, const uint4& b) {
-  E.x = E.x + a.x + b.x, E.y = E.y + a.y + b.y, E.z = E.z + a.z + b.z, E.w = E.w + a.w + b.w;
+// words of E added by IMADs on the FMA-side pipe (the ALU pipe also carries the shift-adds and the offset compares; the
+// kernel is bound by shared memory, 92 % of the wavefront peak): config 4, 0: 256.5 ms, 2: 251.8, 4: 250.7
+constexpr int kWideFmaWords = 4;
+// (the packed adder of the offsets forms gains nothing from it: reuse form on a coarsened config 3, 84.5 -> 85.4 ms)
+__device__ __forceinline__ void add_wide(uint4& E, uint4& O, const uint4& a, const uint4& b, uint32_t one) {
+  add_pair_mix<kWideFmaWords>(E, a, b, one);
   O.x += a.x >> 16, O.y += a.y >> 16, O.z += a.z >> 16, O.w += a.w >> 16;
   asm volatile("" : "+r"(O.x), "+r"(O.y), "+r"(O.z), "+r"(O.w));  // keeps each shift-add one LEA.HI
   O.x += b.x >> 16, O.y += b.y >> 16, O.z += b.z >> 16, O.w += b.w >> 16;
@@ -139,7 +143,7 @@ __device__ __forceinline__ void add_wide(uint4& E, uint4& O, const uint4& a, con
 
 template <bool REUSE, bool WIDE>
 __device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
-                                              uint32_t meta_row) {
+                                              uint32_t meta_row, uint32_t one) {
 #pragma unroll 1
   for (int cc = 0; cc < Cc; cc += 2) {
     uint4 ma[2], mb[2];
@@ -150,7 +154,7 @@ __device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint4 (&hi)[kRD
     uint32_t pa = ma[0].x, pb = mb[0].x;
     lds_sw(wa, sdata + pa);
     lds_sw(wb, sdata + pb);
-    if constexpr (WIDE) add_wide(acc[0], hi[0], wa, wb); else add_pair(acc[0], wa, wb);
+    if constexpr (WIDE) add_wide(acc[0], hi[0], wa, wb, one); else add_pair(acc[0], wa, wb);
 #pragma unroll
     for (int j = 1; j < kRD; ++j) {
       const uint32_t oa = word_of(ma[j >> 2], j & 3), ob = word_of(mb[j >> 2], j & 3);
@@ -162,7 +166,7 @@ __device__ __forceinline__ void stage_general(uint4 (&acc)[kRD], uint4 (&hi)[kRD
         lds_sw(wa, sdata + oa);
         lds_sw(wb, sdata + ob);
       }
-      if constexpr (WIDE) add_wide(acc[j], hi[j], wa, wb); else add_pair(acc[j], wa, wb);
+      if constexpr (WIDE) add_wide(acc[j], hi[j], wa, wb, one); else add_pair(acc[j], wa, wb);
     }
   }
 }
@@ -214,8 +218,8 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
     if constexpr (SHARE) {
       add1(acc[J], t4);  // the quad's sum is unchanged since the last taken step: one term per word
     } else if constexpr (WIDE) {
-      add_wide(acc[J], hi[J], wa, wb);
-      add_wide(acc[J], hi[J], wc, wd);
+      add_wide(acc[J], hi[J], wa, wb, one);
+      add_wide(acc[J], hi[J], wc, wd, one);
     } else {
       add_pair_mix<kDeltaFmaWords - 4>(acc[J], wa, wb, one);
       add_pair_mix<kDeltaFmaWords>(acc[J], wc, wd, one);
@@ -253,8 +257,8 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
       sum4(t4, wa, wb, wc, wd);
       add1(acc[0], t4);
     } else if constexpr (WIDE) {
-      add_wide(acc[0], hi[0], wa, wb);
-      add_wide(acc[0], hi[0], wc, wd);
+      add_wide(acc[0], hi[0], wa, wb, one);
+      add_wide(acc[0], hi[0], wc, wd, one);
     } else {
       add_pair_mix<kDeltaFmaWords - 4>(acc[0], wa, wb, one);
       add_pair_mix<kDeltaFmaWords>(acc[0], wc, wd, one);
@@ -378,11 +382,11 @@ struct Lanes<4> {  // four 32-bit lanes: plain sums
     if constexpr (is_delta(MODE) || MODE == kModeHybrid)  // (a hybrid range: this call is one of its delta-coded chunks)
       stage_delta<MODE == kModeDeltaShare>(acc, acc, sdata, smeta, Cc, meta_row, one);
     else
-      stage_general<MODE == kModeGeneralReuse, false>(acc, acc, sdata, smeta, Cc, meta_row);
+      stage_general<MODE == kModeGeneralReuse, false>(acc, acc, sdata, smeta, Cc, meta_row, one);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage_rest(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {  // hybrid: the other chunks
-    stage_general<true, false>(acc, acc, sdata, smeta, Cc, meta_row);
+  __device__ __forceinline__ void stage_rest(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {  // hybrid: the other chunks
+    stage_general<true, false>(acc, acc, sdata, smeta, Cc, meta_row, one);
   }
   __device__ __forceinline__ void flush() {}
   template <int MODE>
@@ -401,17 +405,17 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {
     if constexpr (MODE == kModeWide)
-      stage_general<true, true>(acc, hi, sdata, smeta, Cc, meta_row);  // acc = E, hi = O
+      stage_general<true, true>(acc, hi, sdata, smeta, Cc, meta_row, one);  // acc = E, hi = O
     else if constexpr (MODE == kModeDeltaPair)
       stage_pairs(acc, sdata, smeta, Cc, meta_row);
     else if constexpr (is_delta(MODE) || is_hybrid(MODE))  // (a hybrid range: this call is one of its delta-coded chunks)
       stage_delta<MODE == kModeDeltaShare, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row, one);
     else
-      stage_general<MODE == kModeGeneralReuse, false>(acc, hi, sdata, smeta, Cc, meta_row);
+      stage_general<MODE == kModeGeneralReuse, false>(acc, hi, sdata, smeta, Cc, meta_row, one);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage_rest(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {  // hybrid: the other chunks
-    stage_general<true, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row);
+  __device__ __forceinline__ void stage_rest(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {  // hybrid: the other chunks
+    stage_general<true, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row, one);
   }
   __device__ __forceinline__ void flush() {
 #pragma unroll
@@ -445,7 +449,7 @@ struct Lanes<16> {  // sixteen 8-bit lanes: e, r as in add_bytes; he, hq the upp
     stage_bytes(e, r, sdata, smeta, Cc, meta_row, one);
   }
   template <int MODE>
-  __device__ __forceinline__ void stage_rest(uint32_t, uint32_t, int, uint32_t) {}  // (no hybrid form on 8-bit lanes)
+  __device__ __forceinline__ void stage_rest(uint32_t, uint32_t, int, uint32_t, uint32_t) {}  // (no hybrid form on 8-bit lanes)
   // invariant: e = A0 | A2 << 16,  r = A1 + 2^8 A2 + 2^16 A3 (mod 2^32),  lane sum = A + 256 * (he | hq lane)
   static __device__ __forceinline__ void flush_word(uint32_t& e, uint32_t& r, uint32_t& he, uint32_t& hq) {
     uint32_t q = r - ((e >> 16) << 8);  // A1 | A3 << 16
@@ -607,7 +611,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
       if (it < nd)
         lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off_d, p.Cc, meta_row_d, p.one);
       else
-        lanes.template stage_rest<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row);
+        lanes.template stage_rest<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
     } else {
       lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
     }
