@@ -347,7 +347,7 @@ void build_tables(const dd_plan& p, dd::RangePlan& r) {
         const int jg = j0 + g * r.RD;
         const size_t k = (size_t)s / r.Cc, si = (size_t)s % r.Cc;
         if (k < nd) {
-          uint32_t* e = &meta[(size_t)b * words_per_block + k * wd + ((si / 4) * r.G + g) * 4];
+          uint32_t* e = &meta[(size_t)b * words_per_block + k * wd + ((size_t)g * (r.Cc / 4) + si / 4) * 4];  // [group][quad]
           const int q = s % 4;
           const uint32_t off = ((uint32_t)si * (uint32_t)(r.T + r.Smax) + (uint32_t)(delay(jg, c) - d0)) * 16u;
           e[1 + q / 2] |= off << (16 * (q % 2));  // byte offset inside the stage, < 64 KB (choose_tile)

@@ -207,7 +207,9 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
       }
     } else {
       // (measured: one uniform branch per channel PAIR instead of per quad skips more predicated-off loads but
-      // costs more than it saves: 116.2 vs 111.7 ms on config 3; 109.7 vs 107.0 ms in the SHARE variant)
+      // costs more than it saves: 116.2 vs 111.7 ms on config 3; 109.7 vs 107.0 ms in the SHARE variant.  Staggering
+      // the two pairs of the quad by half a trial step, so that a reload is followed by the other pair's adds before
+      // its words are needed, doubles the branches and R2Ps: 108.4 vs 100.7 ms.)
       if (any & (1u << J)) {
         lds_if_bit<delta_bit(J, 0)>(wa, aa, bits);
         lds_if_bit<delta_bit(J, 1)>(wb, ab, bits);
@@ -228,9 +230,10 @@ __device__ __forceinline__ void delta_steps(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
   }
 }
 
+// (the entries of a trial group's quads follow each other: the table pointer advances by a constant)
 template <bool SHARE, bool WIDE = false>
 __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD], uint32_t sdata, uint32_t smeta, int Cc,
-                                            uint32_t meta_row, uint32_t one) {
+                                            uint32_t one) {
   uint4 m;
   lds_sw(m, smeta);
 #pragma unroll 1
@@ -251,7 +254,7 @@ __device__ __forceinline__ void stage_delta(uint4 (&acc)[kRD], uint4 (&hi)[kRD],
     lds_sw(wd, ad);
     // next quad's entry (the last one reads the first entry of the following stage slot or the pad: unused),
     // fetched now so that its latency hides behind this quad's adds
-    smeta += meta_row;
+    smeta += 16;
     lds_sw(m, smeta);
     if constexpr (SHARE) {
       sum4(t4, wa, wb, wc, wd);
@@ -380,7 +383,7 @@ struct Lanes<4> {  // four 32-bit lanes: plain sums
   template <int MODE>
   __device__ __forceinline__ void stage(uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row, uint32_t one) {
     if constexpr (is_delta(MODE) || MODE == kModeHybrid)  // (a hybrid range: this call is one of its delta-coded chunks)
-      stage_delta<MODE == kModeDeltaShare>(acc, acc, sdata, smeta, Cc, meta_row, one);
+      stage_delta<MODE == kModeDeltaShare>(acc, acc, sdata, smeta, Cc, one);
     else
       stage_general<MODE == kModeGeneralReuse, false>(acc, acc, sdata, smeta, Cc, meta_row, one);
   }
@@ -409,7 +412,7 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
     else if constexpr (MODE == kModeDeltaPair)
       stage_pairs(acc, sdata, smeta, Cc, meta_row);
     else if constexpr (is_delta(MODE) || is_hybrid(MODE))  // (a hybrid range: this call is one of its delta-coded chunks)
-      stage_delta<MODE == kModeDeltaShare, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, meta_row, one);
+      stage_delta<MODE == kModeDeltaShare, MODE == kModeWideHybrid>(acc, hi, sdata, smeta, Cc, one);
     else
       stage_general<MODE == kModeGeneralReuse, false>(acc, hi, sdata, smeta, Cc, meta_row, one);
   }
@@ -427,12 +430,12 @@ struct Lanes<8> {  // eight 16-bit lanes, value = lo + 256*hi
     if constexpr (is_wide(MODE)) {  // acc = E = sum of the words, hi = O = sum of their upper halves
 #pragma unroll
       for (int q = 0; q < 4; ++q) v[2 * q] = lo[q] - (up[q] << 16), v[2 * q + 1] = up[q];
-      return;
-    }
+    } else {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      v[2 * q] = (lo[q] & 0xffffu) + ((up[q] & 0xffffu) << 8);
-      v[2 * q + 1] = (lo[q] >> 16) + ((up[q] >> 16) << 8);
+      for (int q = 0; q < 4; ++q) {
+        v[2 * q] = (lo[q] & 0xffffu) + ((up[q] & 0xffffu) << 8);
+        v[2 * q + 1] = (lo[q] >> 16) + ((up[q] >> 16) << 8);
+      }
     }
   }
 };
@@ -593,8 +596,9 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const uint32_t thread_off = (uint32_t)ti * kSuperwordBytes;
   const uint32_t entry_bytes = MODE == kModeDeltaPair ? 80u : (!is_delta(MODE) && NL != 16) ? 32u : 16u;  // table bytes per (channel | quad, trial group)
   const uint32_t meta_row = (uint32_t)p.G * entry_bytes;             // bytes between consecutive channels (quads)
-  const uint32_t meta_off = data_bytes + (uint32_t)g * entry_bytes;
-  const uint32_t meta_row_d = (uint32_t)p.G * 16u, meta_off_d = data_bytes + (uint32_t)g * 16u;  // delta chunks of a hybrid range
+  // delta form: [trial group][quad] entries of 16 bytes; the other forms: [channel | quad of pairs][trial group]
+  const uint32_t meta_off_d = data_bytes + (uint32_t)g * (uint32_t)(p.Cc / 4) * 16u;
+  const uint32_t meta_off = (is_delta(MODE) && MODE != kModeDeltaPair) ? meta_off_d : data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
 
   int s = 0;        // stage of the chunk being consumed
@@ -609,7 +613,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
     const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
     if constexpr (is_hybrid(MODE)) {
       if (it < nd)
-        lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off_d, p.Cc, meta_row_d, p.one);
+        lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off_d, p.Cc, meta_row, p.one);
       else
         lanes.template stage_rest<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
     } else {

@@ -31,7 +31,7 @@ def _padded_delays(plan, r, shape, rd):
 def _decode(plan, r):
     """Delays implied by the kernel tables: [nblocks][Dcta][Cpad] (absolute, superwords).  A trial block holds the
     table slices of its channel chunks one after the other: the first `delta_chunks` in the delta form (one 4-word
-    entry per channel quad and trial group), the others as one 32-bit byte offset per (channel, trial)."""
+    entry per trial group and channel quad), the others as one 32-bit byte offset per (channel, trial)."""
     info, shape = plan.tile_info(r), plan.tile_shape(r)
     rd = 4 if info["lanes"] == 16 else 8
     g, cc, cpad, rowp, nb = (shape[k] for k in ("trial_groups", "chans_per_stage", "cpad", "row_superwords", "nblocks"))
@@ -48,7 +48,7 @@ def _decode(plan, r):
     rel = np.zeros((nb, g, rd, cpad), dtype=np.int64)
     cd = nd * cc                                                              # channels under the delta form
     if nd:
-        e = meta[:, :nd * wd].reshape(nb, cd // 4, g, 4)
+        e = meta[:, :nd * wd].reshape(nb, nd, g, cc // 4, 4).transpose(0, 1, 3, 2, 4).reshape(nb, cd // 4, g, 4)  # [chunk][group][quad]
         anyb = np.zeros((nb, cd // 4, g), dtype=np.int64)
         for q in range(4):
             field = (e[..., 1 + q // 2] >> (16 * (q % 2))) & 0xFFFF           # [nb][quad][g] byte offset in the stage
