@@ -259,7 +259,8 @@ int dd_plan_tile_shape(const dd_plan_t* plan, int32_t r, int32_t* trial_groups, 
  * (rows 2v, 2v+1 = the two pre-summed rows of pair v), 6 = delta_v per pair (int32).  7 = the channel whose packed row is
  * staged in each row of a trial block's chunk sequence (int32 [trial blocks][channel rows]; a permutation inside every
  * delta-coded chunk, chosen so that channels whose delays change at the same trials share a quad; tables 0 - 2 are
- * indexed by that row).  *bytes = size; the table is copied when host_buf != NULL
+ * indexed by that row); 8 = the same for the pair mode (row of the pair array staged in each row; tables 3 - 5 are indexed
+ * by the staged row, table 6 by the pair).  *bytes = size; the table is copied when host_buf != NULL
  * (DD_ERR_NOMEM if cap_bytes is too small). */
 int dd_plan_table(const dd_plan_t* plan, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes);
 

@@ -127,8 +127,9 @@ struct RangePlan {
   std::vector<uint32_t> h_meta2;          // [nblocks][Cpad/8][G][5 entries of 4 words]: {changed bits, any bits, 0, 0}, then 8 16-bit offsets per pair
   std::vector<int32_t> h_dmin2, h_span2;  // [nblocks][Cpad]: start / span of the staged row (both rows of a pair: those of channel 2v)
   std::vector<int32_t> h_delta;           // [Cpad/2] delta_v
+  std::vector<int32_t> h_chan2;           // [nblocks][Cpad] row of the pair array staged in each row of the block's chunk sequence
   uint4* d_meta2 = nullptr;
-  int32_t *d_dmin2 = nullptr, *d_span2 = nullptr, *d_delta = nullptr;
+  int32_t *d_dmin2 = nullptr, *d_span2 = nullptr, *d_delta = nullptr, *d_chan2 = nullptr;
   int64_t adds_pair = 0;  // adds executed per beam in pair mode (pre-sums included)
 };
 

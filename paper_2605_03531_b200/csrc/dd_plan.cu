@@ -408,17 +408,52 @@ void build_pair_tables(const dd_plan& p, dd::RangePlan& r) {
     r.h_delta[v] = lo;
   }
   const size_t nbc = (size_t)r.nblocks * r.Cpad;
+  // Which pair sits in which double row of a stage: as for the delta table (build_tables), the pairs of a chunk are
+  // dealt to quads by the delay phase of their first channel at the block's middle trial, per trial block.  h_chan2
+  // holds the source ROW (2v + p) of every staged row.
+  std::vector<int32_t> pairsrc(nbc / 2);  // [block][slot pair] -> pair
+  r.h_chan2.assign(nbc, 0);
+  {
+    const double ts = p.tsamp * (double)r.decim, inv_top = 1.0 / (p.f_top * p.f_top);
+    std::vector<double> phase(r.Cc2);
+    std::vector<int32_t> order(r.Cc2);
+    for (int b = 0; b < r.nblocks; ++b) {
+      const int jm = std::min(r.ndm - 1, b * r.Dcta + r.Dcta / 2);
+      const double dm = r.dm_lo + (double)jm * r.dm_step;
+      for (int k = 0; k < nvc / r.Cc2; ++k) {
+        for (int i = 0; i < r.Cc2; ++i) {
+          const int v = k * r.Cc2 + i, c = 2 * v;
+          order[i] = v;
+          if (c < p.nchans) {
+            const double f = p.f_top + (double)c * p.cw;
+            const double x = kDispersion * dm * (1.0 / (f * f) - inv_top) / ts + 0.5;
+            phase[i] = x - floor(x);
+          } else {
+            phase[i] = -1.0;
+          }
+        }
+        std::stable_sort(order.begin(), order.end(), [&](int32_t u, int32_t v) { return phase[u - k * r.Cc2] > phase[v - k * r.Cc2]; });
+        for (int i = 0; i < r.Cc2; ++i) {
+          const size_t u = (size_t)k * r.Cc2 + i;
+          pairsrc[(size_t)b * nvc + u] = order[i];
+          r.h_chan2[(size_t)b * r.Cpad + 2 * u] = 2 * order[i];
+          r.h_chan2[(size_t)b * r.Cpad + 2 * u + 1] = 2 * order[i] + 1;
+        }
+      }
+    }
+  }
   r.h_dmin2.assign(nbc, 0);
   r.h_span2.assign(nbc, 0);
   r.Smax2 = 0;
   for (int b = 0; b < r.nblocks; ++b)
-    for (int v = 0; v < nvc; ++v) {
+    for (int u = 0; u < nvc; ++u) {  // u = slot pair, v = the pair staged there
+      const int v = pairsrc[(size_t)b * nvc + u];
       const int j0 = b * r.Dcta;
       const int32_t d0 = pair_delay(p, r, j0, 2 * v) & ~7;
       const int32_t sp = (int32_t)round_up(pair_delay(p, r, j0 + r.Dcta - 1, 2 * v) - d0, 8);
       for (int q = 0; q < 2; ++q) {  // both pre-summed rows of the pair are staged over the span of channel 2v
-        r.h_dmin2[(size_t)b * r.Cpad + 2 * v + q] = d0;
-        r.h_span2[(size_t)b * r.Cpad + 2 * v + q] = sp;
+        r.h_dmin2[(size_t)b * r.Cpad + 2 * u + q] = d0;
+        r.h_span2[(size_t)b * r.Cpad + 2 * u + q] = sp;
       }
       r.Smax2 = std::max(r.Smax2, (int)sp);
     }
@@ -430,16 +465,17 @@ void build_pair_tables(const dd_plan& p, dd::RangePlan& r) {
   // table: five 16-byte entries per quad of pairs and trial group (dd_tiled.cu stage_pairs)
   r.h_meta2.assign((size_t)r.nblocks * (nvc / 4) * r.G * 20, 0);
   for (int b = 0; b < r.nblocks; ++b)
-    for (int v = 0; v < nvc; ++v) {
-      const int32_t d0 = r.h_dmin2[(size_t)b * r.Cpad + 2 * v];
-      const int q = v % 4;
+    for (int u = 0; u < nvc; ++u) {
+      const int v = pairsrc[(size_t)b * nvc + u];
+      const int32_t d0 = r.h_dmin2[(size_t)b * r.Cpad + 2 * u];
+      const int q = u % 4;
       for (int g = 0; g < r.G; ++g) {
         const int jg = b * r.Dcta + g * r.RD;
-        uint32_t* e = &r.h_meta2[(((size_t)b * (nvc / 4) + v / 4) * r.G + g) * 20];
+        uint32_t* e = &r.h_meta2[(((size_t)b * (nvc / 4) + u / 4) * r.G + g) * 20];
         auto D = [&](int j) { return pair_delay(p, r, j, 2 * v); };
         auto P = [&](int j) { return pair_delay(p, r, j, 2 * v + 1) - D(j) - r.h_delta[v]; };
         for (int j = 0; j < r.RD; ++j) {
-          const uint32_t off = ((uint32_t)((2 * v + P(jg + j)) % r.Cc) * (uint32_t)(r.T + r.Smax2) + (uint32_t)(D(jg + j) - d0)) * 16u;
+          const uint32_t off = ((uint32_t)((2 * u + P(jg + j)) % r.Cc) * (uint32_t)(r.T + r.Smax2) + (uint32_t)(D(jg + j) - d0)) * 16u;
           e[4 + 4 * q + j / 2] |= off << (16 * (j % 2));
           if (j > 0 && (D(jg + j) != D(jg + j - 1) || P(jg + j) != P(jg + j - 1))) {
             e[0] |= 1u << dd::delta_bit(j, q);
@@ -464,6 +500,8 @@ int upload_pair_tables(dd::RangePlan& r) {
   DD_CUDA(cudaMemcpy(r.d_dmin2, r.h_dmin2.data(), r.h_dmin2.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   DD_CUDA(cudaMemcpy(r.d_span2, r.h_span2.data(), r.h_span2.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   DD_CUDA(cudaMemcpy(r.d_delta, r.h_delta.data(), r.h_delta.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  DD_CUDA(cudaMalloc(&r.d_chan2, r.h_chan2.size() * sizeof(int32_t)));
+  DD_CUDA(cudaMemcpy(r.d_chan2, r.h_chan2.data(), r.h_chan2.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   return DD_OK;
 }
 
@@ -670,6 +708,7 @@ int dd_plan_destroy(dd_plan_t* p) {
     if (r.d_dmin2) cudaFree(r.d_dmin2);
     if (r.d_span2) cudaFree(r.d_span2);
     if (r.d_delta) cudaFree(r.d_delta);
+    if (r.d_chan2) cudaFree(r.d_chan2);
   }
   for (cudaEvent_t e : p->prof_events) cudaEventDestroy(e);
   if (p->ws && p->ws_owned) cudaFree(p->ws);
@@ -1087,13 +1126,13 @@ int dd_plan_kernel_times(const dd_plan_t* p, int32_t slot, int32_t cap, float* m
 }
 
 int dd_plan_table(const dd_plan_t* p, int32_t r, int32_t which, void* host_buf, int64_t cap_bytes, int64_t* bytes) {
-  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 7) return DD_ERR_INVALID;
+  if (!p || r < 0 || r >= (int)p->ranges.size() || !bytes || which < 0 || which > 8) return DD_ERR_INVALID;
   const auto& q = p->ranges[r];
-  const void* srcs[8] = {q.h_meta.data(), q.h_dmin.data(), q.h_span.data(), q.h_meta2.data(), q.h_dmin2.data(),
-                         q.h_span2.data(), q.h_delta.data(), q.h_chan.data()};
-  const size_t sizes[8] = {q.h_meta.size(), q.h_dmin.size(), q.h_span.size(), q.h_meta2.size(), q.h_dmin2.size(),
-                           q.h_span2.size(), q.h_delta.size(), q.h_chan.size()};
-  if (which >= 3 && which <= 6 && !q.pair_ok) return DD_ERR_INVALID;
+  const void* srcs[9] = {q.h_meta.data(), q.h_dmin.data(), q.h_span.data(), q.h_meta2.data(), q.h_dmin2.data(),
+                         q.h_span2.data(), q.h_delta.data(), q.h_chan.data(), q.h_chan2.data()};
+  const size_t sizes[9] = {q.h_meta.size(), q.h_dmin.size(), q.h_span.size(), q.h_meta2.size(), q.h_dmin2.size(),
+                           q.h_span2.size(), q.h_delta.size(), q.h_chan.size(), q.h_chan2.size()};
+  if (which >= 3 && which != 7 && !q.pair_ok) return DD_ERR_INVALID;
   const void* src = srcs[which];
   const size_t n = sizes[which] * 4;
   *bytes = (int64_t)n;

@@ -726,7 +726,7 @@ cudaError_t launch_tiled(const dd_plan* p, const RangePlan& r, float* out_dev, c
   tp.meta = pairs ? r.d_meta2 : r.d_meta;
   tp.dmin = pairs ? r.d_dmin2 : r.d_dmin;
   tp.span = pairs ? r.d_span2 : r.d_span;
-  tp.chan = pairs ? nullptr : r.d_chan;
+  tp.chan = pairs ? r.d_chan2 : r.d_chan;
   tp.out = out_dev + r.offset;
   tp.out_beam_stride = p->beam_stride;
   tp.pitch = r.pitch;

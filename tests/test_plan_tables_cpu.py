@@ -272,11 +272,18 @@ def _decode_pairs(plan, r):
     delta = plan.table(r, 6).astype(np.int64)
     assert (dmin % 8 == 0).all() and (span % 8 == 0).all() and (span + info["words_per_cta"] <= rowsw).all()
     assert np.array_equal(dmin[:, 0::2], dmin[:, 1::2]) and np.array_equal(span[:, 0::2], span[:, 1::2])
+    # which pair sits in which double row (dd_plan_table 8): a permutation of the pairs inside every chunk
+    chan2 = plan.table(r, 8).astype(np.int64).reshape(nb, cpad)
+    assert np.array_equal(chan2[:, 1::2], chan2[:, 0::2] + 1) and (chan2[:, 0::2] % 2 == 0).all()
+    src = chan2[:, 0::2] // 2                                                        # [nb][slot pair] -> pair
+    assert np.array_equal(np.sort(src.reshape(nb, nvc // (cc // 2), cc // 2), axis=2),
+                          np.broadcast_to(np.arange(nvc).reshape(nvc // (cc // 2), cc // 2), (nb, nvc // (cc // 2), cc // 2)))
     out = np.zeros((nb, g, 8, cpad), dtype=np.int64)
     anyb = np.zeros((nb, nvc // 4, g), dtype=np.int64)
     assert (e[..., 2:4] == 0).all()
     for q in range(4):
-        v = np.arange(q, nvc, 4)                                                    # the pairs in position q of their quad
+        v = np.arange(q, nvc, 4)                                                    # the slot pairs in position q of their quad
+        sv = src[:, v]                                                               # [nb][quad]: the pairs staged there
         prev = None
         for j in range(8):
             off = (e[..., 4 + 4 * q + j // 2] >> (16 * (j % 2))) & 0xFFFF             # [nb][quad][g] byte offset in the stage
@@ -293,8 +300,9 @@ def _decode_pairs(plan, r):
                 assert np.array_equal(chg, (off != prev).astype(np.int64)), "changed bit <=> the offset differs from the previous trial's"
                 anyb |= chg << j
             prev = off
-            out[:, :, j, 2 * q::8] = D.transpose(0, 2, 1)
-            out[:, :, j, 2 * q + 1::8] = (D + delta[None, v, None] + pbit).transpose(0, 2, 1)
+            idx = np.broadcast_to(sv[:, None, :], (nb, g, v.size))
+            np.put_along_axis(out[:, :, j, :], 2 * idx, D.transpose(0, 2, 1), axis=2)
+            np.put_along_axis(out[:, :, j, :], 2 * idx + 1, (D + delta[sv][:, :, None] + pbit).transpose(0, 2, 1), axis=2)
     assert np.array_equal(anyb, e[..., 1]), "any bits are the OR of the quad's changed bits"
     return out.reshape(nb * g * 8, cpad)
 
