@@ -292,6 +292,7 @@ __device__ __forceinline__ void pair_steps(uint4 (&acc)[kRD], uint4& wa, uint4& 
   }
 }
 
+// (Adds on the FMA-side pipe as in the delta form do not pay here: the pair mode is bound by shared memory, 72.2 -> 80.8 ms.)
 __device__ __forceinline__ void stage_pairs(uint4 (&acc)[kRD], uint32_t sdata, uint32_t smeta, int Cc, uint32_t meta_row) {
   // Cc = rows of the stage = 2 per pair; a quad of pairs = 8 rows
 #pragma unroll 1
