@@ -506,3 +506,37 @@ def test_subband_host_path_and_two_beams():
     plan, flat = gpu_run(w, x, SUBBAND, host_path=True)
     assert plan.pair_info(0)["enabled"] == 1 and plan.pair_info(1)["enabled"] == 1
     check_full(w, x, plan, flat, check_pad=False)
+
+
+def test_random_plans_every_element():
+    """Seeded random small plans -- fine, borderline (hybrid) and coarse DM grids, all decimations, both input widths,
+    one or two beams, two ranges each -- through the automatic kernel choice, every output element against the oracle.
+    Covers the table forms and lane widths in combinations no hand-written case names."""
+    rng = np.random.default_rng(20261105)
+    seen = set()
+    for i in range(28):
+        nch = int(rng.integers(20, 180))
+        f_top = float(rng.uniform(400.0, 1500.0))
+        cw = -float(rng.uniform(0.2, 0.5)) * f_top / nch
+        tsamp = float(rng.choice([327.68e-6, 655.36e-6, 1.31072e-3]))
+        bits = 16 if i % 3 == 2 else 8
+        nbeams = 1 + (i % 2)
+        f_lo = f_top + (nch - 1) * cw
+        ranges, maxd_in = [], 0
+        for k in range(2):
+            decim = int(rng.choice([1, 2, 4, 8]))
+            sweep_per_dm = 4.148808e3 * (f_lo ** -2 - f_top ** -2) / (tsamp * decim)
+            kind = (i + k) % 3
+            step = float((rng.uniform(0.2, 0.95), rng.uniform(0.95, 1.5), rng.uniform(1.5, 5.0))[kind]) / sweep_per_dm
+            ndm = int(rng.integers(40, 260)) if kind < 2 else int(rng.integers(10, 90))
+            lo = float(rng.uniform(0.0, 30.0)) * step
+            ranges.append(W.DMRange(lo, step, ndm, decim))
+            maxd_in = max(maxd_in, (int(sweep_per_dm * (lo + ndm * step)) + 2) * decim)
+        ns = maxd_in + int(rng.integers(700, 5000))
+        w = W.Workload("rand%d" % i, f_top, cw, nch, tsamp, ns, nbeams, bits, tuple(ranges), 1, 0, 0)
+        x = rng.integers(0, 2 ** bits, size=(nbeams, nch, ns), dtype=np.uint8 if bits == 8 else np.uint16)
+        x[0, nch // 3, : ns // 2] = 2 ** bits - 1
+        plan, flat = gpu_run(w, x, TILED)
+        check_full(w, x, plan, flat)
+        seen |= {(plan.tile_info(r)["lanes"], plan.tile_info(r)["mode"]) for r in range(2)}
+    assert {(8, 2), (16, 0), (8, 5), (8, 6)} <= seen, seen   # delta, 8-bit lanes, uint16 lanes and hybrid all occurred

@@ -206,32 +206,41 @@ def test_row_pitch_covers_every_channels_span_regression():
 
 
 def test_row_pitch_property_random_plans():
-    """Host-only property test over random small plans and multi-block fine-grid (delta) plans."""
+    """Host-only property test over random small plans: multi-block fine grids (delta form), grids whose lowest channels
+    step by a little more than one sample (hybrid forms) and coarse grids (offsets forms, 8-bit and uint16 lanes), both
+    input widths.  Every staged row fits its pitch, and the kernel tables, decoded independently of the kernel, give back
+    the plan's delay table for every (trial block, row, trial) -- channel dealing included."""
     rng = np.random.default_rng(20261104)
-    checked = delta_plans = 0
+    checked = 0
+    modes = {}
     for i in range(400):
         nch = int(rng.integers(4, 200))
         f_top = float(rng.uniform(300.0, 1500.0))
         cw = -float(rng.uniform(0.2, 0.6)) * f_top / nch
         tsamp = float(rng.choice([81.92e-6, 327.68e-6, 655.36e-6, 1.31072e-3]))
         decim = int(rng.choice([1, 2, 4, 8]))
-        fine = i % 2 == 0
-        ndm = int(rng.integers(200, 1000)) if fine else int(rng.integers(1, 80))
-        # fine: steps of at most ~1 sample at the lowest channel (delta mode); coarse: a few samples per trial
+        bits = 16 if i % 5 == 4 else 8
+        kind = i % 4            # 0, 2: fine; 1: coarse; 3: borderline
+        ndm = int(rng.integers(1, 80)) if kind == 1 else int(rng.integers(200, 1000))
+        # fine: steps of at most ~1 sample at the lowest channel (delta form); coarse: a few samples per trial
         f_lo = f_top + (nch - 1) * cw
         sweep_per_dm = 4.148808e3 * (f_lo ** -2 - f_top ** -2) / (tsamp * decim)
-        step = float(rng.uniform(0.2, 0.999) if fine else rng.uniform(1.0, 6.0)) / sweep_per_dm
+        step = float(rng.uniform(1.0, 6.0) if kind == 1 else rng.uniform(0.9, 1.6) if kind == 3 else rng.uniform(0.2, 0.999)) / sweep_per_dm
         lo = float(rng.uniform(0.0, 50.0)) * step
         maxd = int(sweep_per_dm * (lo + ndm * step)) + 2
         try:
-            p = B.Plan(f_top, cw, nch, tsamp, (maxd + 600) * decim, [(lo, step, ndm, decim)], host_only=True)
+            p = B.Plan(f_top, cw, nch, tsamp, (maxd + 600) * decim, [(lo, step, ndm, decim)], in_bits=bits, host_only=True)
         except B.DDError:
             continue
         assert _row_invariant(p, 0), (i, f_top, cw, nch, tsamp, decim, lo, step, ndm)
-        delta_plans += p.tile_info(0)["mode"] == 2
+        if p.tile_shape(0)["tiled"]:
+            got, rd, shape = _decode(p, 0)
+            assert np.array_equal(got, _padded_delays(p, 0, shape, rd)), (i, f_top, cw, nch, tsamp, decim, lo, step, ndm, bits)
+        m = p.tile_info(0)["mode"]
+        modes[m] = modes.get(m, 0) + 1
         checked += 1
         p.destroy()
-    assert checked > 300 and delta_plans > 100
+    assert checked > 300 and modes.get(2, 0) > 100 and modes.get(6, 0) > 10 and modes.get(0, 0) > 10 and modes.get(5, 0) > 3, modes
 
 
 def test_tuned_plan_goes_through_the_same_checks():
