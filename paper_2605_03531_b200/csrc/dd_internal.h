@@ -13,10 +13,11 @@ namespace dd {
 
 // Packed time word ("superword"): 16 bytes holding NL time lanes of one channel.
 //   lane m of superword i is the decimated sample y[i + m*H]   (H = lane segment length)
-//   NL = 16: sixteen 8-bit lanes (byte k of word q holds lane 4q+k); undecimated ranges whose delay steps
-//            are too coarse for the delta table.  uint16 input is split into two such byte planes (low and
-//            high byte) that are dedispersed one after the other: S = S_lo + 256*S_hi.
-//   NL = 8: eight 16-bit lanes (word q holds lanes 2q (low half) and 2q+1 (high half))
+//   NL = 16: sixteen 8-bit lanes (byte k of word q holds lane 4q+k); undecimated uint8 ranges whose delay steps
+//            are too coarse for the delta table.  (On request, dd_tuning_t::byte_lanes = 1, uint16 input is split into
+//            two such byte planes that are dedispersed one after the other: S = S_lo + 256*S_hi.)
+//   NL = 8: eight 16-bit lanes (word q holds lanes 2q (low half) and 2q+1 (high half)): samples with headroom for
+//           packed sums (uint8, decimated or delta-coded), or the uint16 samples themselves (kModeWide)
 //   NL = 4: four 32-bit lanes
 // A delay of d samples is a shift of d superwords for every lane at once, so any delay is a
 // 16-byte aligned access.

@@ -9,8 +9,10 @@
 // into two 16-bit time lanes (NL == 8), i.e. four algorithmic adds per instruction.  Packed lanes are kept
 // exact by a two-level carry-save scheme: every `flush` channels the upper bytes of the 16-bit lanes are
 // moved into a second packed accumulator (sum = lo + 256*hi), so the accumulators of a trial are 8
-// registers and never overflow.  Neighbouring trials that share a delay reuse the superword held in
-// registers (kModeDelta / kModeGeneralReuse).  The DM-time writer converts once (I2F.RN) and stores fp32.
+// registers and never overflow.  Part of the adds are issued as IMADs on the FMA-side pipe, which the ALU-pipe
+// instructions of the adder would otherwise leave idle.  Neighbouring trials that share a delay reuse the superword
+// held in registers (delta, reuse and hybrid table forms, dd_internal.h).  The DM-time writer converts once (I2F.RN)
+// and stores fp32.
 //
 // Integer sums are exact, so the result has the same bits as the definition whatever the order.
 #include <cuda_runtime.h>
