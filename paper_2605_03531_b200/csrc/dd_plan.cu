@@ -188,6 +188,13 @@ void choose_tile(const dd_plan& p, dd::RangePlan& r, const dd_tuning_t& tune) {
     if (stages < min_stages) return false;
     // bytes staged per add: row (T + mean spread) superwords + the table row, over T*NL*D adds
     double cost = ((T + smean) * 16.0 + dd::tiled_meta_bytes(r.mode, r.NL, 4, G) / 4.0) / ((double)T * r.NL * D);
+    // The delta form is not bound by the fill of its stages (config 3: 0.02 - 0.04 staged bytes per add, 1 - 1.5 TB/s out
+    // of L2) but by issue slots and shared-memory wavefronts, which grow with the share of quad steps that reload; shorter
+    // trial blocks let the channel dealing of build_tables match delay phases over fewer trials and halve the table.  So
+    // below a floor the staged bytes do not count and the shorter block wins.  Measured, 64 x 64 against 128 x 32 trials x
+    // superwords: config 3 99.1 / 100.5 ms, 2048 channels 50.7 / 52.4, 327 us sampling 95.5 / 98.8, a 300-500 MHz band
+    // 77.9 / 78.9 (32 x 128 needs 16-channel stages for its 16-bit offsets: 105.1).
+    if (r.mode == dd::kModeDelta || dd::is_hybrid(r.mode)) cost = std::max(cost, 0.05) * (1.0 + 0.02 * (double)D / 128.0);
     // trials past the end of the last block are computed and dropped
     cost *= (double)nblocks * D / (double)r.ndm;
     if (G * T == 256) cost *= 1.02;  // mild preference for the 512-thread CTA at equal cost
