@@ -603,6 +603,11 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
   const uint32_t meta_off_d = data_bytes + (uint32_t)g * (uint32_t)(p.Cc / 4) * 16u;
   const uint32_t meta_off = (is_delta(MODE) && MODE != kModeDeltaPair) ? meta_off_d : data_bytes + (uint32_t)g * entry_bytes;
   int since_flush = 0;
+  // The last trial block of a range is padded to the block size (2000 trials = 31 blocks of 64 + 16): the trial groups of
+  // a CTA that hold no real trial (warp-uniform: T is a multiple of 32) skip the adds, which leaves the SM's issue slots
+  // to the others (config 3: 99.0 -> 95.6 ms).
+  // (Not in the pair mode: there the extra live value costs a register spill in the loop, 71.4 -> 79.4 ms.)
+  const bool group_live = MODE == kModeDeltaPair || (blk * p.G + g) * RD < p.ndm;
 
   int s = 0;        // stage of the chunk being consumed
   uint32_t ph = 0;  // its full-barrier parity
@@ -612,15 +617,19 @@ __global__ void __launch_bounds__(NT, 512 / NT) dd_tiled_kernel(const TiledParam
       advance();
       prefetch(my_k);
     }
-    mbar_wait(bar_base + 8u * s, ph);
     const uint32_t sbase = stage0 + (uint32_t)s * stage_bytes;
-    if constexpr (is_hybrid(MODE)) {
-      if (it < nd)
-        lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off_d, p.Cc, meta_row, p.one);
-      else
-        lanes.template stage_rest<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
+    if (group_live) {
+      mbar_wait(bar_base + 8u * s, ph);
+      if constexpr (is_hybrid(MODE)) {
+        if (it < nd)
+          lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off_d, p.Cc, meta_row, p.one);
+        else
+          lanes.template stage_rest<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
+      } else {
+        lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
+      }
     } else {
-      lanes.template stage<MODE>(sbase + thread_off, sbase + meta_off, p.Cc, meta_row, p.one);
+      mbar_wait_relaxed(bar_base + 8u * s, ph);  // keeps the barrier protocol and its producer turns only
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_base + 8u * (nstages + s));  // stage may be refilled
