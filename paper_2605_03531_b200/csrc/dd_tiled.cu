@@ -66,12 +66,13 @@ __device__ __forceinline__ void add_pair(uint4& acc, const uint4& a, const uint4
   acc.z = acc.z + a.z + b.z;
   acc.w = acc.w + a.w + b.w;
 }
-// The delta kernel is bound by the ALU pipe (IADD3, LOP3, R2P, the predicated address steps: 79 % busy) while the
-// FMA-side pipe idles, so part of the adds of every trial step go there as IMADs (two per IADD3 they replace: more issue
+// The delta kernel was bound by the ALU pipe (IADD3, LOP3, R2P, the predicated address steps: 79 % busy) while the
+// FMA-side pipe idled, so part of the adds of every trial step go there as IMADs (two per IADD3 they replace: more issue
 // slots, fewer ALU slots).  Words per quad and trial step (of 8) moved, config 3: 0: 111.8 ms, 1: 110.8, 2: 109.2,
 // 3: 109.1, 4: 112.6 (issue slots and shared memory take over); with the channels dealt to quads by phase (dd_plan.cu
-// build_tables) 1: 103.5, 2: 102.1, 3: 100.7, 4: 104.1, 5: 109.2.
-constexpr int kDeltaFmaWords = 3;
+// build_tables) 1: 103.5, 2: 102.1, 3: 100.7, 4: 104.1, 5: 109.2; with the final tile and the padded trial groups
+// skipped 0: 97.8, 1: 95.1, 2: 95.1, 3: 95.5, 4: 99.8.
+constexpr int kDeltaFmaWords = 2;
 // acc += t on the FMA-side pipe: IMAD with a multiplier of one that ptxas cannot fold (a kernel parameter)
 __device__ __forceinline__ uint32_t mad1(uint32_t t, uint32_t one, uint32_t e) {
   uint32_t d;
