@@ -114,7 +114,8 @@ struct RangePlan {
   std::vector<int32_t> h_dmin, h_span;
   std::vector<int32_t> h_chan;  // [nblocks][Cpad] channel whose packed row is staged in row s of the block's chunk sequence
   uint4* d_meta = nullptr;      // general: [nblocks][Cpad][G] RD 32-bit byte offsets inside the stage;
-                                // delta: [nblocks][Cpad/4][G] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits}
+                                // delta: [nblocks][chunk][G][Cc/4] {changed bits, offA|offB<<16, offC|offD<<16, any-changed bits};
+                                // hybrid: a block's delta chunks first, then its offsets chunks (dd_plan.cu build_tables)
   int32_t* d_dmin = nullptr;    // [nblocks][Cpad] first delay of the block (superwords)
   int32_t* d_span = nullptr;    // [nblocks][Cpad] delay spread of the block (superwords)
   int32_t* d_chan = nullptr;    // [nblocks][Cpad] h_chan
