@@ -530,7 +530,7 @@ def run_ours(args, w):
             "dtype": "u%d" % w.in_bits, "data": "synthetic",
             "config": {"workload": w.name, "nchans": w.nchans, "nsamps": w.nsamps, "beams_per_gpu": 1,
                        "dm_trials": w.total_trials, "ranges": [[r.dm_lo, r.dm_step, r.ndm, r.decim] for r in w.ranges],
-                       "l2": "inputs larger than L2 (1.07 GB input, 4.0 GB packed copy, 3.8 GB output per step)",
+                       "l2": "inputs larger than L2 (1.07 GB input, 3.8 GB of packed copies written and read through a 2.2 GB scratch, 3.8 GB output per step)",
                        "parallelism": "replicas: one beam per GPU, no collective"},
             "input_gb_per_s": world * w.nchans * w.nsamps * (w.in_bits // 8) / (ms_total / args.steps * 1e-3) / 1e9,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "sps": sps, "post": post, "subband": subband, "other_configs": other,

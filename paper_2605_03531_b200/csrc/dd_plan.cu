@@ -624,8 +624,10 @@ static int plan_create_host(const dd_config_t* cfg, dd_plan_t** plan_out, int64_
       offset += (int64_t)r.ndm * r.pitch;
       p->dm_samples += (int64_t)p->nbeams * r.ndm * r.nout;
       choose_tile(*p, r, tune ? *tune : kAutoTuning);
-      r.ws_offset = p->ws_bytes;
-      p->ws_bytes += round_up(r.ws_bytes, 256);
+      // every range packs into the same scratch: a range is packed right before its dedispersion kernel (dd_execute), so
+      // the workspace is the largest packed copy, not their sum (config 3: 2.2 GB instead of 4.0 GB)
+      r.ws_offset = 0;
+      p->ws_bytes = std::max<int64_t>(p->ws_bytes, round_up(r.ws_bytes, 256));
     }
     if (rc == DD_OK) {
       p->beam_stride = offset;
@@ -761,31 +763,29 @@ int dd_execute(const dd_plan_t* plan, const void* in_dev, float* out_dev, void* 
   };
   if (plan->row_stats)  // row statistics for the single-pulse search: the kernels' epilogues add into zeroed sums
     DD_CUDA(cudaMemsetAsync(plan->row_stats, 0, (size_t)plan->nbeams * plan->rows_per_beam * 2 * sizeof(unsigned long long), stream));
-  // a2 for every range first, then a3+a4: the dedispersion kernels of consecutive ranges follow each
-  // other on the stream without a pack kernel draining the machine in between.
+  // Range by range: a2 (pack), then a3+a4.  The packed copies of all ranges share one scratch; the pack kernel of the
+  // next range (0.4 - 1 ms) starts in the tail of the dedispersion kernel before it, where SMs idle anyway.
   for (const auto& r : plan->ranges) {
-    if (all_direct || !r.tiled_ok) continue;
+    const int ri = (int)(&r - plan->ranges.data());
+    if (all_direct || !r.tiled_ok) {
+      if (!r.d_delays) return DD_ERR_INVALID;  // uploaded by dd_plan_create / dd_plan_set_kernel
+      DD_CUDA(ev_before(2, ri));
+      DD_CUDA(dd::launch_direct(plan, r, in_dev, out_dev, stream));
+      DD_CUDA(ev_after());
+      continue;
+    }
     if (!plan->ws || plan->ws_have < plan->ws_bytes + plan->ws_pair_bytes) return DD_ERR_NOMEM;
-    DD_CUDA(ev_before(0, (int)(&r - plan->ranges.data())));
+    DD_CUDA(ev_before(0, ri));
     DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
     DD_CUDA(ev_after());
     if (dd::use_pairs(plan, r)) {  // DD_KERNEL_SUBBAND: pre-sum the packed rows into the pair rows
-      DD_CUDA(ev_before(3, (int)(&r - plan->ranges.data())));
+      DD_CUDA(ev_before(3, ri));
       DD_CUDA(dd::launch_pairs(plan, r, stream));
       DD_CUDA(ev_after());
     }
-  }
-  for (const auto& r : plan->ranges) {
-    if (all_direct || !r.tiled_ok) {
-      if (!r.d_delays) return DD_ERR_INVALID;  // uploaded by dd_plan_create / dd_plan_set_kernel
-      DD_CUDA(ev_before(2, (int)(&r - plan->ranges.data())));
-      DD_CUDA(dd::launch_direct(plan, r, in_dev, out_dev, stream));
-      DD_CUDA(ev_after());
-    } else {
-      DD_CUDA(ev_before(1, (int)(&r - plan->ranges.data())));
-      DD_CUDA(dd::launch_tiled(plan, r, out_dev, stream));
-      DD_CUDA(ev_after());
-    }
+    DD_CUDA(ev_before(1, ri));
+    DD_CUDA(dd::launch_tiled(plan, r, out_dev, stream));
+    DD_CUDA(ev_after());
   }
   return DD_OK;
 }
@@ -836,23 +836,15 @@ static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out
   DD_CUDA(cudaMemcpyAsync(in_dev, in_host, in_bytes, cudaMemcpyHostToDevice, plan->h2d_stream));
   DD_CUDA(cudaEventRecord(plan->ev_in_ready[slot], plan->h2d_stream));
   DD_CUDA(cudaStreamWaitEvent(stream, plan->ev_in_ready[slot], 0));
-  bool reads_input_late = all_direct;  // the direct kernel reads the input itself
-  for (const auto& r : plan->ranges) {
-    if (all_direct || !r.tiled_ok) {
-      reads_input_late = true;
-      continue;
-    }
-    DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
-    if (dd::use_pairs(plan, r)) DD_CUDA(dd::launch_pairs(plan, r, stream));
-  }
-  if (!reads_input_late) DD_CUDA(cudaEventRecord(plan->ev_in_free[slot], stream));
   DD_CUDA(cudaStreamWaitEvent(stream, plan->ev_out_free[slot], 0));
-  for (const auto& r : plan->ranges) {
+  for (const auto& r : plan->ranges) {  // range by range, as dd_execute: the packed copies share one scratch
     if (all_direct || !r.tiled_ok) {
       DD_CUDA(dd::launch_direct(plan, r, in_dev, out_dev, stream));
       DD_CUDA(copy_rows(r, 0, r.ndm));
       continue;
     }
+    DD_CUDA(dd::launch_pack(plan, r, in_dev, stream));
+    if (dd::use_pairs(plan, r)) DD_CUDA(dd::launch_pairs(plan, r, stream));
     const int per = std::max(1, (r.nblocks + kPieces - 1) / kPieces);
     for (int b0 = 0; b0 < r.nblocks; b0 += per) {
       const int nb = std::min(per, r.nblocks - b0);
@@ -860,7 +852,7 @@ static int execute_host_enqueue(dd_plan_t* plan, const void* in_host, float* out
       DD_CUDA(copy_rows(r, b0 * r.Dcta, std::min(r.ndm, (b0 + nb) * r.Dcta)));
     }
   }
-  if (reads_input_late) DD_CUDA(cudaEventRecord(plan->ev_in_free[slot], stream));
+  DD_CUDA(cudaEventRecord(plan->ev_in_free[slot], stream));  // the last range's pack / direct kernel has read the input
   DD_CUDA(cudaEventRecord(plan->ev_out_free[slot], plan->copy_stream));
   return DD_OK;
 }
@@ -1066,14 +1058,14 @@ int dd_plan_set_kernel(dd_plan_t* p, int32_t variant) {
   if (variant == DD_KERNEL_SUBBAND && p->ws_pair_bytes == 0) {
     // first use: pair tables of every range that qualifies, their device copies, and room for the pair arrays
     try {
-      int64_t off = p->ws_bytes;
+      int64_t pair_bytes = 0;
       for (auto& r : p->ranges) {
         build_pair_tables(*p, r);
         if (!r.pair_ok) continue;
-        r.ws2_offset = off;
-        off += r.ws2_bytes;
+        r.ws2_offset = p->ws_bytes;  // behind the packed copy; shared by the ranges like the packed copy itself
+        pair_bytes = std::max(pair_bytes, r.ws2_bytes);
       }
-      p->ws_pair_bytes = off - p->ws_bytes;
+      p->ws_pair_bytes = pair_bytes;
     } catch (const std::bad_alloc&) {
       return DD_ERR_NOMEM;
     }
