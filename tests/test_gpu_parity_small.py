@@ -510,7 +510,8 @@ def test_subband_host_path_and_two_beams():
 
 def test_random_plans_every_element():
     """Seeded random small plans -- fine, borderline (hybrid) and coarse DM grids, all decimations, both input widths,
-    one or two beams, two ranges each -- through the automatic kernel choice, every output element against the oracle.
+    one or two beams, both input layouts and band orders, two ranges each -- through the automatic kernel choice, every
+    output element against the oracle.
     Covers the table forms and lane widths in combinations no hand-written case names."""
     rng = np.random.default_rng(20261105)
     seen = set()
@@ -536,7 +537,7 @@ def test_random_plans_every_element():
         w = W.Workload("rand%d" % i, f_top, cw, nch, tsamp, ns, nbeams, bits, tuple(ranges), 1, 0, 0)
         x = rng.integers(0, 2 ** bits, size=(nbeams, nch, ns), dtype=np.uint8 if bits == 8 else np.uint16)
         x[0, nch // 3, : ns // 2] = 2 ** bits - 1
-        plan, flat = gpu_run(w, x, TILED)
+        plan, flat = gpu_run(w, x, TILED, in_layout=(i // 4) % 2, ascending=bool((i // 8) % 2))   # all four input conventions
         check_full(w, x, plan, flat)
         seen |= {(plan.tile_info(r)["lanes"], plan.tile_info(r)["mode"]) for r in range(2)}
     assert {(8, 2), (16, 0), (8, 5), (8, 6)} <= seen, seen   # delta, 8-bit lanes, uint16 lanes and hybrid all occurred
