@@ -154,6 +154,7 @@ struct dd_plan {
   unsigned long long* row_stats = nullptr;
   int device = 0;
   int variant = DD_KERNEL_AUTO;
+  int sps_warp_kernel = 1;  // single-pulse search: the barrier-free kernel where it applies (experiment switch)
   // workspace
   int64_t ws_bytes = 0;      // packed copies of every range
   int64_t ws_pair_bytes = 0; // + the pair arrays of DD_KERNEL_SUBBAND (0 until that variant is selected)

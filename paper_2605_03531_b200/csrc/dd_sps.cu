@@ -398,6 +398,224 @@ __global__ void __launch_bounds__(kSpsThreads, WIDE ? 2 : (K <= 8 ? 4 : 3)) dd_s
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// dd_sps_warp_kernel: the search for K <= 9 widths and 32-bit sums, WITHOUT block barriers in the tile loop.  One CTA
+// per row as above, but every warp works on tiles of its own (tile t of kSpsWarpTile samples goes to warp t mod 8): its
+// raw samples arrive by bulk copies into one of the warp's two buffers, the warp turns them into the prefix sum IN PLACE
+// (lane l owns PER consecutive samples, PER odd: conflict-free; a warp scan joins the lanes) and filters it; only
+// __syncwarp orders the phases.  (ncu on the block-wide kernel: 3.1 barrier stalls per issued instruction, the shared-
+// memory data pipe at 59 %.)  Same arithmetic, same results.
+// ------------------------------------------------------------------------------------------------
+constexpr int kSpsWarpTile = 1024;
+__host__ __device__ constexpr int sps_warp_words(int K) {  // words of one warp buffer: prefix entries 0 .. span, 16-byte multiple
+  return (kSpsWarpTile + (1 << (K - 1)) + 1 + 3) / 4 * 4;
+}
+__host__ __device__ constexpr int sps_warp_per(int K) { return ((kSpsWarpTile + (1 << (K - 1)) + 31) / 32) | 1; }
+
+template <int K>
+__global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsParams p) {
+  using acc_t = uint32_t;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ unsigned long long red[2][kSpsThreads / 32];
+  __shared__ SpsRowConsts s_c;
+  __shared__ __align__(8) unsigned long long s_bar[kSpsThreads / 32][2];
+  __shared__ unsigned long long s_best[kSpsMaxK][kSpsThreads / 32];
+  __shared__ int s_tb[kSpsMaxK][kSpsThreads / 32];
+  __shared__ int s_count[kSpsMaxK];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n = p.n;
+  const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
+  const long long orow = (long long)blockIdx.y * p.rows_per_beam + p.row0 + blockIdx.x;
+
+  if (tid < kSpsMaxK) s_count[tid] = 0;
+  if (p.stats) {
+    if (tid == 0) sps_row_consts(p.stats[2 * orow], p.stats[2 * orow + 1], n, K, p.threshold, s_c);
+  } else {
+    unsigned long long t1, t2;
+    sps_row_sums(x, n, red, t1, t2);
+    if (tid == 0) sps_row_consts(t1, t2, n, K, p.threshold, s_c);
+  }
+  const uint32_t bar0 = smem_u32(&s_bar[warp][0]);
+  if (lane == 0) {
+    mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, 1);
+    fence_barrier_init();
+  }
+  __syncthreads();
+
+  constexpr int halo = 1 << (K - 1);
+  constexpr int span = kSpsWarpTile + halo;
+  constexpr int kWords = sps_warp_words(K);
+  constexpr int PER = sps_warp_per(K);
+  uint32_t* const buf0 = reinterpret_cast<uint32_t*>(smem_raw) + (size_t)warp * 2 * kWords;
+
+  acc_t best1[K], thr[K];
+  int tq[K];
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    best1[k] = 0, tq[k] = -1;
+    thr[k] = s_c.thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_c.thr[k];
+  }
+  auto tile_floats = [&](int tile0) { return min((span + 3) & ~3, ((n + 3) & ~3) - tile0); };
+  auto issue = [&](int tile0, int b) {  // lane 0: bulk copy of the tile's raw samples into buffer b of this warp
+    const uint32_t bytes = (uint32_t)tile_floats(tile0) * 4u;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the buffer was last touched by ordinary loads / stores
+    mbar_arrive_expect_tx(bar0 + 8u * b, bytes);
+    bulk_copy_g2s(smem_u32(buf0 + b * kWords), x + tile0, bytes, bar0 + 8u * b);
+  };
+  const int ntiles = (n + kSpsWarpTile - 1) / kSpsWarpTile;
+  if (lane == 0 && warp < ntiles) issue(warp * kSpsWarpTile, 0);
+  auto boxcars4 = [&](const acc_t* P, int k, int tl, const acc_t (&a)[4], const acc_t (&a4)[4], acc_t (&b)[4]) {
+    if (k == 0) {
+      b[0] = a[1] - a[0], b[1] = a[2] - a[1], b[2] = a[3] - a[2], b[3] = a4[0] - a[3];
+    } else if (k == 1) {
+      b[0] = a[2] - a[0], b[1] = a[3] - a[1], b[2] = a4[0] - a[2], b[3] = a4[1] - a[3];
+    } else if (k == 2) {
+      b[0] = a4[0] - a[0], b[1] = a4[1] - a[1], b[2] = a4[2] - a[2], b[3] = a4[3] - a[3];
+    } else {
+      acc_t c[4];
+      load4(P + tl + (1 << k), c);
+      b[0] = c[0] - a[0], b[1] = c[1] - a[1], b[2] = c[2] - a[2], b[3] = c[3] - a[3];
+    }
+  };
+
+  int it = 0;
+  for (int t = warp; t < ntiles; t += kSpsThreads / 32, ++it) {
+    const int b = it & 1;
+    const int tile0 = t * kSpsWarpTile;
+    if (lane == 0 && t + kSpsThreads / 32 < ntiles) issue((t + kSpsThreads / 32) * kSpsWarpTile, b ^ 1);
+    mbar_wait(bar0 + 8u * b, (uint32_t)(it >> 1) & 1u);
+    uint32_t* const P = buf0 + b * kWords;            // raw floats now, prefix sums after the next block
+    const float* const X = reinterpret_cast<const float*>(P);
+    {
+      const int valid = min(span, n - tile0), i0 = lane * PER;
+      uint32_t v[PER];
+      acc_t loc = 0;
+#pragma unroll
+      for (int i = 0; i < PER; ++i) {
+        v[i] = i0 + i < valid ? (uint32_t)X[i0 + i] : 0u;
+        loc += v[i];
+      }
+      acc_t inc = loc;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const acc_t u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
+      }
+      acc_t base = inc - loc;
+      __syncwarp();  // every lane has read its samples: the prefix may overwrite them
+      if (lane == 0) P[0] = 0;
+#pragma unroll
+      for (int i = 0; i < PER; ++i) {
+        base += v[i];
+        if (i0 + i < span) P[i0 + i + 1] = base;
+      }
+      __syncwarp();
+    }
+    const int nfast = min(kSpsWarpTile, max(0, n - halo - 3 - tile0 + 1)) / 4;
+    {
+      uint32_t hits = 0;
+      for (int q = lane; q < nfast; q += 32) {
+        const int tl = 4 * q;
+        acc_t a[4], a4[4];
+        load4(P + tl, a);
+        load4(P + tl + 4, a4);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          acc_t bx[4];
+          boxcars4(P, k, tl, a, a4, bx);
+          const acc_t m01 = bx[0] > bx[1] ? bx[0] : bx[1], m23 = bx[2] > bx[3] ? bx[2] : bx[3], m = m01 > m23 ? m01 : m23;
+          if (m >= thr[k]) hits |= 1u << k;
+          if (m >= best1[k]) {
+            best1[k] = m + 1;
+            tq[k] = tile0 + tl;
+          }
+        }
+      }
+      if (hits) {
+        for (int q = lane; q < nfast; q += 32) {
+          const int tl = 4 * q;
+          acc_t a[4], a4[4];
+          load4(P + tl, a);
+          load4(P + tl + 4, a4);
+#pragma unroll
+          for (int k = 0; k < K; ++k) {
+            if (!(hits & (1u << k))) continue;
+            acc_t bx[4];
+            boxcars4(P, k, tl, a, a4, bx);
+            const int c = (bx[0] >= thr[k]) + (bx[1] >= thr[k]) + (bx[2] >= thr[k]) + (bx[3] >= thr[k]);
+            if (c) atomicAdd(&s_count[k], c);
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < K; ++k) {
+        if (tq[k] >= 0) {
+          const int tl = tq[k] - tile0;
+          acc_t a[4], a4[4], bx[4];
+          load4(P + tl, a);
+          load4(P + tl + 4, a4);
+          boxcars4(P, k, tl, a, a4, bx);
+          const acc_t m = best1[k] - 1;
+          tq[k] = -(tq[k] + (bx[0] == m ? 0 : bx[1] == m ? 1 : bx[2] == m ? 2 : 3) + 2);
+        }
+      }
+    }
+    if (4 * nfast < kSpsWarpTile) {  // the end of the row: windows checked one by one
+      for (int tl = 4 * nfast + lane; tl < kSpsWarpTile; tl += 32) {
+        const int tt = tile0 + tl;
+        if (tt >= n) break;
+        const acc_t p0 = P[tl];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          const int w = 1 << k;
+          if (tt + w <= n) {
+            const acc_t bb = P[tl + w] - p0;
+            if (bb >= best1[k]) best1[k] = bb + 1, tq[k] = -(tt + 2);
+            if (bb >= thr[k]) atomicAdd(&s_count[k], 1);
+          }
+        }
+      }
+    }
+    __syncwarp();  // all lanes are done with this buffer before lane 0 refills it two tiles later
+  }
+
+  // ---------------- reduce over the block: larger sum wins, ties go to the smaller t ----------------------
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    unsigned long long bb = best1[k];
+    int t = best1[k] ? -(tq[k] + 2) : 0x7fffffff;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const unsigned long long ob = shfl_down_u64(bb, o);
+      const int ot = __shfl_down_sync(0xffffffffu, t, o);
+      if (ob > bb || (ob == bb && ot < t)) bb = ob, t = ot;
+    }
+    if (lane == 0) s_best[k][warp] = bb, s_tb[k][warp] = t;
+  }
+  __syncthreads();
+  if (tid < K) {
+    const int k = tid;
+    unsigned long long bb = 0;
+    int t = 0x7fffffff;
+    const int c = s_count[k];
+    for (int i = 0; i < kSpsThreads / 32; ++i) {
+      const unsigned long long ob = s_best[k][i];
+      const int ot = s_tb[k][i];
+      if (ob > bb || (ob == bb && ot < t)) bb = ob, t = ot;
+    }
+    const long long o = orow * K + k;
+    if (bb == 0) {
+      p.snr[o] = 0.0f, p.tmax[o] = -1, p.count[o] = 0;
+    } else {
+      p.snr[o] = sps_snr(bb - 1, s_c, k);
+      p.tmax[o] = t;
+      p.count[o] = c;
+    }
+  }
+}
+
 // Exclusive scan of count[0..m) into offsets[0..m] (int64), one CTA: the list positions of every (row, width).
 __global__ void __launch_bounds__(1024) dd_sps_scan_kernel(const int32_t* __restrict__ count, long long m,
                                                            long long* __restrict__ offsets) {
@@ -509,6 +727,17 @@ static cudaError_t launch_sps(const SpsParams& sp, dim3 grid, size_t smem, cudaS
   return cudaGetLastError();
 }
 
+template <int K>
+static cudaError_t launch_sps_warp(const SpsParams& sp, dim3 grid, cudaStream_t stream) {
+  const size_t smem = (size_t)(kSpsThreads / 32) * 2 * sps_warp_words(K) * 4;
+  cudaError_t e = cudaFuncSetAttribute(dd_sps_warp_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(dd_sps_warp_kernel<K>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  if (e != cudaSuccess) return e;
+  dd_sps_warp_kernel<K><<<grid, kSpsThreads, smem, stream>>>(sp);
+  return cudaGetLastError();
+}
+
 }  // namespace dd
 
 namespace {
@@ -585,6 +814,14 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
     const size_t smem = sps_smem(wide, nwidths);
     const dim3 grid((unsigned)r.ndm, (unsigned)p->nbeams);
     cudaError_t e = cudaErrorInvalidValue;
+    if (!wide && nwidths <= 9 && p->sps_warp_kernel) {  // the barrier-free form
+#define DD_SPSW(K_) case K_: e = dd::launch_sps_warp<K_>(sp, grid, stream); break;
+      switch (nwidths) { DD_SPSW(1) DD_SPSW(2) DD_SPSW(3) DD_SPSW(4) DD_SPSW(5) DD_SPSW(6) DD_SPSW(7) DD_SPSW(8) DD_SPSW(9) }
+#undef DD_SPSW
+      if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_warp_kernel launch");
+      row0 += r.ndm;
+      continue;
+    }
 #define DD_SPS(K_)                                                                                                  \
   case K_:                                                                                                          \
     e = wide ? dd::launch_sps<K_, true>(sp, grid, smem, stream) : dd::launch_sps<K_, false>(sp, grid, smem, stream); \
