@@ -422,13 +422,15 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
   __shared__ unsigned long long s_best[kSpsMaxK][kSpsThreads / 32];
   __shared__ int s_tb[kSpsMaxK][kSpsThreads / 32];
   __shared__ int s_count[kSpsMaxK];
+  __shared__ unsigned int s_blk[kSpsMaxK];  // (largest boxcar any warp has published so far) + 1, 0 = none
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n = p.n;
   const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
   const long long orow = (long long)blockIdx.y * p.rows_per_beam + p.row0 + blockIdx.x;
 
-  if (tid < kSpsMaxK) s_count[tid] = 0;
+  if (tid < kSpsMaxK) s_count[tid] = 0, s_blk[tid] = 0;
+  if (lane < kSpsMaxK) s_best[lane][warp] = 0, s_tb[lane][warp] = 0x7fffffff;  // this warp's record per width
   if (p.stats) {
     if (tid == 0) sps_row_consts(p.stats[2 * orow], p.stats[2 * orow + 1], n, K, p.threshold, s_c);
   } else {
@@ -450,13 +452,25 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
   constexpr int PER = sps_warp_per(K);
   uint32_t* const buf0 = reinterpret_cast<uint32_t*>(smem_raw) + (size_t)warp * 2 * kWords;
 
-  acc_t best1[K], thr[K];
-  int tq[K];
+  // Records live in shared memory, one per warp and width: s_best = (largest boxcar among the warp's windows) + 1 and
+  // s_tb = where it was first seen; they change a few times per row, so the filter loop carries no position.  seen[k]
+  // (the same in every lane) = the largest (boxcar + 1) this warp has recorded or has seen published by another warp:
+  // a tile whose maximum does not beat it cannot hold the first occurrence of the row's maximum.
+  acc_t seen[K], thr[K];
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    best1[k] = 0, tq[k] = -1;
+    seen[k] = 0;
     thr[k] = s_c.thr[k] > 0xffffffffull ? (acc_t)0xffffffffu : (acc_t)s_c.thr[k];
   }
+  // publish (boxcar + 1) of a candidate record; true if no warp has published a larger one (equal ones are both kept:
+  // the final reduction takes the smaller position)
+  auto publish = [&](int k, acc_t w1) -> bool {
+    unsigned int old = 0;
+    if (lane == 0) old = atomicMax(&s_blk[k], w1);
+    old = __shfl_sync(0xffffffffu, old, 0);
+    seen[k] = old > w1 ? old : w1;
+    return w1 >= old;
+  };
   auto tile_floats = [&](int tile0) { return min((span + 3) & ~3, ((n + 3) & ~3) - tile0); };
   auto issue = [&](int tile0, int b) {  // lane 0: bulk copy of the tile's raw samples into buffer b of this warp
     const uint32_t bytes = (uint32_t)tile_floats(tile0) * 4u;
@@ -514,8 +528,14 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
       __syncwarp();
     }
     const int nfast = min(kSpsWarpTile, max(0, n - halo - 3 - tile0 + 1)) / 4;
-    {
-      uint32_t hits = 0;
+    if (nfast > 0) {
+      // Four consecutive samples per lane and step; the loop only keeps, per width, the largest boxcar the lane has seen
+      // in this tile (a fused subtract-max and a three-way max per pair).  Per tile and width the warp's maximum (REDUX)
+      // then decides, uniformly, whether the lanes count windows at or above the threshold (rare) or look up the
+      // position of a new record (a few times per row).
+      acc_t tmax[K];
+#pragma unroll
+      for (int k = 0; k < K; ++k) tmax[k] = 0;
       for (int q = lane; q < nfast; q += 32) {
         const int tl = 4 * q;
         acc_t a[4], a4[4];
@@ -526,55 +546,62 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
           acc_t bx[4];
           boxcars4(P, k, tl, a, a4, bx);
           const acc_t m01 = bx[0] > bx[1] ? bx[0] : bx[1], m23 = bx[2] > bx[3] ? bx[2] : bx[3], m = m01 > m23 ? m01 : m23;
-          if (m >= thr[k]) hits |= 1u << k;
-          if (m >= best1[k]) {
-            best1[k] = m + 1;
-            tq[k] = tile0 + tl;
-          }
+          tmax[k] = m > tmax[k] ? m : tmax[k];
         }
       }
-      if (hits) {
+#pragma unroll
+      for (int k = 0; k < K; ++k) {
+        const acc_t wmax = __reduce_max_sync(0xffffffffu, tmax[k]);
+        const bool hit = wmax >= thr[k];
+        bool better = false;
+        if (wmax + 1 > seen[k]) better = publish(k, wmax + 1);
+        if (!(hit || better)) continue;
+        int c = 0, first = 0x7fffffff;
         for (int q = lane; q < nfast; q += 32) {
           const int tl = 4 * q;
-          acc_t a[4], a4[4];
+          acc_t a[4], a4[4], bx[4];
           load4(P + tl, a);
           load4(P + tl + 4, a4);
+          boxcars4(P, k, tl, a, a4, bx);
+          c += (bx[0] >= thr[k]) + (bx[1] >= thr[k]) + (bx[2] >= thr[k]) + (bx[3] >= thr[k]);
+          if (first == 0x7fffffff && (bx[0] == wmax || bx[1] == wmax || bx[2] == wmax || bx[3] == wmax))
+            first = tile0 + tl + (bx[0] == wmax ? 0 : bx[1] == wmax ? 1 : bx[2] == wmax ? 2 : 3);
+        }
+        if (hit && c) atomicAdd(&s_count[k], c);
+        if (better) {
+          first = __reduce_min_sync(0xffffffffu, first);
+          if (lane == 0) s_best[k][warp] = (unsigned long long)wmax + 1ull, s_tb[k][warp] = first;
+          __syncwarp();
+        }
+      }
+    }
+    if (4 * nfast < kSpsWarpTile) {  // the end of the row: windows checked one by one, then merged into the warp's record
+      acc_t tb1[K];  // this lane's (largest boxcar) + 1 among them, first position
+      int tt[K];
 #pragma unroll
-          for (int k = 0; k < K; ++k) {
-            if (!(hits & (1u << k))) continue;
-            acc_t bx[4];
-            boxcars4(P, k, tl, a, a4, bx);
-            const int c = (bx[0] >= thr[k]) + (bx[1] >= thr[k]) + (bx[2] >= thr[k]) + (bx[3] >= thr[k]);
-            if (c) atomicAdd(&s_count[k], c);
+      for (int k = 0; k < K; ++k) tb1[k] = 0, tt[k] = 0x7fffffff;
+      for (int tl = 4 * nfast + lane; tl < kSpsWarpTile; tl += 32) {
+        const int t1 = tile0 + tl;
+        if (t1 >= n) break;
+        const acc_t p0 = P[tl];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          const int w = 1 << k;
+          if (t1 + w <= n) {
+            const acc_t bb = P[tl + w] - p0;
+            if (bb >= tb1[k]) tb1[k] = bb + 1, tt[k] = t1;
+            if (bb >= thr[k]) atomicAdd(&s_count[k], 1);
           }
         }
       }
 #pragma unroll
       for (int k = 0; k < K; ++k) {
-        if (tq[k] >= 0) {
-          const int tl = tq[k] - tile0;
-          acc_t a[4], a4[4], bx[4];
-          load4(P + tl, a);
-          load4(P + tl + 4, a4);
-          boxcars4(P, k, tl, a, a4, bx);
-          const acc_t m = best1[k] - 1;
-          tq[k] = -(tq[k] + (bx[0] == m ? 0 : bx[1] == m ? 1 : bx[2] == m ? 2 : 3) + 2);
-        }
-      }
-    }
-    if (4 * nfast < kSpsWarpTile) {  // the end of the row: windows checked one by one
-      for (int tl = 4 * nfast + lane; tl < kSpsWarpTile; tl += 32) {
-        const int tt = tile0 + tl;
-        if (tt >= n) break;
-        const acc_t p0 = P[tl];
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-          const int w = 1 << k;
-          if (tt + w <= n) {
-            const acc_t bb = P[tl + w] - p0;
-            if (bb >= best1[k]) best1[k] = bb + 1, tq[k] = -(tt + 2);
-            if (bb >= thr[k]) atomicAdd(&s_count[k], 1);
-          }
+        const acc_t wb1 = __reduce_max_sync(0xffffffffu, tb1[k]);
+        // these windows lie behind every window the warp has looked at so far: only a strictly larger sum is a record
+        if (wb1 > seen[k] && publish(k, wb1)) {
+          const int first = __reduce_min_sync(0xffffffffu, tb1[k] == wb1 ? tt[k] : 0x7fffffff);
+          if (lane == 0) s_best[k][warp] = wb1, s_tb[k][warp] = first;
+          __syncwarp();
         }
       }
     }
@@ -582,18 +609,6 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
   }
 
   // ---------------- reduce over the block: larger sum wins, ties go to the smaller t ----------------------
-#pragma unroll
-  for (int k = 0; k < K; ++k) {
-    unsigned long long bb = best1[k];
-    int t = best1[k] ? -(tq[k] + 2) : 0x7fffffff;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      const unsigned long long ob = shfl_down_u64(bb, o);
-      const int ot = __shfl_down_sync(0xffffffffu, t, o);
-      if (ob > bb || (ob == bb && ot < t)) bb = ob, t = ot;
-    }
-    if (lane == 0) s_best[k][warp] = bb, s_tb[k][warp] = t;
-  }
   __syncthreads();
   if (tid < K) {
     const int k = tid;
