@@ -536,6 +536,7 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
       acc_t tmax[K];
 #pragma unroll
       for (int k = 0; k < K; ++k) tmax[k] = 0;
+#pragma unroll 4  // (independent groups in flight: 8 widths 1.28 -> 1.22 ms)
       for (int q = lane; q < nfast; q += 32) {
         const int tl = 4 * q;
         acc_t a[4], a4[4];
