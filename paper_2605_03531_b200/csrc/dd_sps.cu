@@ -20,7 +20,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <type_traits>
+#include <vector>
 
 #include "dd_internal.h"
 #include "dd_ptx.cuh"
@@ -30,6 +32,7 @@ namespace dd {
 constexpr int kSpsThreads = 256;
 constexpr int kSpsTile = 4096;   // samples per tile
 constexpr int kSpsMaxK = 12;     // widths 1 .. 2048
+constexpr int kSpsMaxRanges = 8;  // ranges one launch of the barrier-free kernel can cover
 
 struct SpsParams {
   const float* plane;  // beam 0 of the range
@@ -41,6 +44,12 @@ struct SpsParams {
   int32_t* count;
   long long row0, rows_per_beam;  // output row = beam*rows_per_beam + row0 + trial
   const unsigned long long* stats;  // [rows][2] = S1, S2 per output row, or nullptr (phase A computes them)
+  // dd_sps_warp_kernel: several ranges in one launch, longest rows first (blockIdx.x runs over the rows of rg[0], rg[1], ...)
+  int nr;
+  struct Range {
+    long long plane_off, pitch, row0;  // floats from `plane` to the range's first row; row pitch; first output row
+    int n, ndm;
+  } rg[kSpsMaxRanges];
   // candidate list (dd_sps_fill_kernel)
   const long long* offsets;  // [rows*K + 1] exclusive scan of count
   dd_sps_cand_t* cand;
@@ -425,9 +434,13 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
   __shared__ unsigned int s_blk[kSpsMaxK];  // (largest boxcar any warp has published so far) + 1, 0 = none
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n = p.n;
-  const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + (long long)blockIdx.x * p.pitch;
-  const long long orow = (long long)blockIdx.y * p.rows_per_beam + p.row0 + blockIdx.x;
+  // which range this row belongs to: the ranges are listed longest rows first, and CTAs start in blockIdx order, so the
+  // short rows fill the end of the launch (one launch per range ends in a partial wave of CTAs each time: 10 % on config 3)
+  int rr = 0, row = (int)blockIdx.x;
+  while (rr + 1 < p.nr && row >= p.rg[rr].ndm) row -= p.rg[rr].ndm, ++rr;
+  const int n = p.rg[rr].n;
+  const float* x = p.plane + (long long)blockIdx.y * p.beam_stride + p.rg[rr].plane_off + (long long)row * p.rg[rr].pitch;
+  const long long orow = (long long)blockIdx.y * p.rows_per_beam + p.rg[rr].row0 + row;
 
   if (tid < kSpsMaxK) s_count[tid] = 0, s_blk[tid] = 0;
   if (lane < kSpsMaxK) s_best[lane][warp] = 0, s_tb[lane][warp] = 0x7fffffff;  // this warp's record per width
@@ -811,8 +824,47 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
   int rc = sps_check(p, plane_dev, nwidths, threshold, &rows_per_beam);
   if (rc != DD_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  // The barrier-free kernel (32-bit sums, up to 9 widths) takes all the ranges it applies to in ONE launch, longest rows
+  // first; the other ranges (and everything else) go range by range to the block-wide kernel below.
+  std::vector<char> merged(p->ranges.size(), 0);
+  if (nwidths <= 9 && p->sps_warp_kernel) {
+    std::vector<int> idx;
+    for (size_t i = 0; i < p->ranges.size(); ++i)
+      if (!sps_wide(p, p->ranges[i], nwidths)) idx.push_back((int)i);
+    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return p->ranges[a].nout > p->ranges[b].nout; });
+    for (size_t first = 0; first < idx.size(); first += dd::kSpsMaxRanges) {
+      dd::SpsParams sp = {};
+      sp.plane = plane_dev;
+      sp.beam_stride = p->beam_stride;
+      sp.K = nwidths;
+      sp.threshold = threshold;
+      sp.snr = snr_dev;
+      sp.tmax = tmax_dev;
+      sp.count = count_dev;
+      sp.rows_per_beam = rows_per_beam;
+      sp.stats = p->row_stats;
+      long long rows = 0;
+      for (size_t k = first; k < idx.size() && k < first + dd::kSpsMaxRanges; ++k) {
+        const auto& r = p->ranges[idx[k]];
+        auto& g = sp.rg[sp.nr++];
+        g.plane_off = r.offset, g.pitch = r.pitch, g.row0 = r.row0, g.n = (int)r.nout, g.ndm = r.ndm;
+        rows += r.ndm;
+        merged[idx[k]] = 1;
+      }
+      const dim3 grid((unsigned)rows, (unsigned)p->nbeams);
+      cudaError_t e = cudaErrorInvalidValue;
+#define DD_SPSW(K_) case K_: e = dd::launch_sps_warp<K_>(sp, grid, stream); break;
+      switch (nwidths) { DD_SPSW(1) DD_SPSW(2) DD_SPSW(3) DD_SPSW(4) DD_SPSW(5) DD_SPSW(6) DD_SPSW(7) DD_SPSW(8) DD_SPSW(9) }
+#undef DD_SPSW
+      if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_warp_kernel launch");
+    }
+  }
   int64_t row0 = 0;
   for (const auto& r : p->ranges) {
+    if (merged[&r - p->ranges.data()]) {
+      row0 += r.ndm;
+      continue;
+    }
     dd::SpsParams sp = {};
     sp.plane = plane_dev + r.offset;
     sp.beam_stride = p->beam_stride;
@@ -830,14 +882,6 @@ int dd_sps_execute(const dd_plan_t* p, const float* plane_dev, int32_t nwidths, 
     const size_t smem = sps_smem(wide, nwidths);
     const dim3 grid((unsigned)r.ndm, (unsigned)p->nbeams);
     cudaError_t e = cudaErrorInvalidValue;
-    if (!wide && nwidths <= 9 && p->sps_warp_kernel) {  // the barrier-free form
-#define DD_SPSW(K_) case K_: e = dd::launch_sps_warp<K_>(sp, grid, stream); break;
-      switch (nwidths) { DD_SPSW(1) DD_SPSW(2) DD_SPSW(3) DD_SPSW(4) DD_SPSW(5) DD_SPSW(6) DD_SPSW(7) DD_SPSW(8) DD_SPSW(9) }
-#undef DD_SPSW
-      if (e != cudaSuccess) return dd::cuda_fail(e, "dd_sps_warp_kernel launch");
-      row0 += r.ndm;
-      continue;
-    }
 #define DD_SPS(K_)                                                                                                  \
   case K_:                                                                                                          \
     e = wide ? dd::launch_sps<K_, true>(sp, grid, smem, stream) : dd::launch_sps<K_, false>(sp, grid, smem, stream); \
