@@ -421,7 +421,7 @@ def run_ours(args, w):
         plan.set_row_stats(None)
         plane_bytes = plan.out_elems() * 4
         hbm = float(peaks.get("hbm_gbs", 6650.0))
-        sps = {"kernel": "dd_sps_kernel", "widths": K, "threshold": thr, "ms": sps_ms, "rows": rows,
+        sps = {"kernel": "dd_sps_warp_kernel (one launch for all ranges)", "widths": K, "threshold": thr, "ms": sps_ms, "rows": rows,
                "row_statistics": "from the dedispersion epilogue (dd_plan_set_row_stats): one pass over the plane",
                "ms_two_pass_without_epilogue_statistics": two_pass_ms, "ms_dd_execute_with_statistics": exec_stats_ms,
                "ms_candidate_list": cand_ms, "candidates_above_threshold": int(offs[-1].item()),
