@@ -353,3 +353,24 @@ def test_pair_tables_reproduce_the_delay_table(cfg, nchans):
     plan.set_kernel(B.DD_KERNEL_TILED)
     assert plan.executed_adds() == brute
     plan.destroy()
+
+
+def test_workspace_is_the_largest_packed_copy_not_their_sum():
+    """The ranges are packed and dedispersed one after the other into one scratch (dd_execute), so the workspace is the
+    largest packed copy: [nbeams][Cpad][Wp] superwords of 16 bytes, Wp = time tiles x tile + largest delay + 8, rounded
+    to 8.  Config 3: 2.2 GB, not the 4.0 GB of three copies side by side; the sub-band variant adds one pair array."""
+    w = W.CONFIGS[3]
+    plan = _host_plan(w)
+    sizes = []
+    for r in range(len(w.ranges)):
+        info, shape, ri = plan.tile_info(r), plan.tile_shape(r), plan.range_info(r)
+        lanes, t = info["lanes"], info["words_per_cta"]
+        h = -(-(-(-ri["nout"] // lanes)) // 16) * 16                    # lane segment, multiple of 16 superwords
+        ntau = -(-h // t)
+        wp = -(-(ntau * t + ri["maxd"] + 8) // 8) * 8
+        sizes.append(-(-(shape["cpad"] * wp * 16) // 256) * 256)
+    assert plan.workspace_bytes() == max(sizes) and plan.workspace_bytes() < 0.6 * sum(sizes)
+    assert 2.0e9 < plan.workspace_bytes() < 2.4e9
+    plan.set_kernel(B.DD_KERNEL_SUBBAND)
+    assert plan.workspace_bytes() == 2 * max(sizes)                     # + the pair rows of the largest range
+    plan.destroy()
