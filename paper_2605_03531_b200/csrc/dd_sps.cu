@@ -467,8 +467,11 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
 
   // Records live in shared memory, one per warp and width: s_best = (largest boxcar among the warp's windows) + 1 and
   // s_tb = where it was first seen; they change a few times per row, so the filter loop carries no position.  seen[k]
-  // (the same in every lane) = the largest (boxcar + 1) this warp has recorded or has seen published by another warp:
-  // a tile whose maximum does not beat it cannot hold the first occurrence of the row's maximum.
+  // (the same in every lane) is what a later tile of this warp has to BEAT to matter: the warp's own record (a tie with
+  // it lies later in the row), or one less than the largest value it has seen published by another warp -- a tie with
+  // another warp's record must still be recorded, because that warp's window may lie later in the row (warps run their
+  // tiles at their own pace: a warp can be told of a record from a tile behind the one it filters next).  A stale
+  // value is only smaller, i.e. costs a lookup, never a result.
   acc_t seen[K], thr[K];
 #pragma unroll
   for (int k = 0; k < K; ++k) {
@@ -481,7 +484,7 @@ __global__ void __launch_bounds__(kSpsThreads, 3) dd_sps_warp_kernel(const SpsPa
     unsigned int old = 0;
     if (lane == 0) old = atomicMax(&s_blk[k], w1);
     old = __shfl_sync(0xffffffffu, old, 0);
-    seen[k] = old > w1 ? old : w1;
+    seen[k] = old > w1 ? old - 1 : w1;
     return w1 >= old;
   };
   auto tile_floats = [&](int tile0) { return min((span + 3) & ~3, ((n + 3) & ~3) - tile0); };
