@@ -98,53 +98,6 @@ def test_sps_all_zero_rows_and_long_rows():
     assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
 
 
-def _check_all(got, ref):
-    for k in ("tmax", "count"):
-        assert np.array_equal(got[k], ref[k]), k
-    assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
-
-
-@pytest.mark.parametrize("K", [1, 4, 8, 9])
-def test_sps_barrier_free_kernel_edge_cases(K):
-    """Up to 9 widths and 32-bit sums run in dd_sps_warp_kernel (every warp filters tiles of its own; records per warp and
-    tile; all ranges in one launch): rows shorter than one warp tile and than the widest filter, constant and all-zero rows
-    (every window ties: the first one wins, across warps and tiles), equal maxima far apart, a late narrow peak in a long
-    row, a threshold below everything (every window counted), two beams, and more ranges than one launch takes."""
-    nch = 8
-    # short rows, constant plane (sigma = 0), then random data with a threshold that counts every window
-    w = W.Workload("spsw_short", 500.0, -200.0 / nch, nch, 1.024e-3, 700, 2, 8,
-                   (W.DMRange(0.0, 1.0, 5, 1), W.DMRange(0.0, 1.0, 3, 4)), 1, 0, 0)
-    x = np.full((2, nch, 700), 100, dtype=np.uint8)
-    plan, got, ref = _sps_both(w, x, K, 1.0)
-    _check_all(got, ref)
-    assert (got["snr"] == 0).all()
-    x = np.random.default_rng(30 + K).integers(0, 256, size=(2, nch, 700), dtype=np.uint8)
-    plan, got, ref = _sps_both(w, x, K, -50.0)
-    _check_all(got, ref)
-    # long rows (40 warp tiles): all zero; then equal maxima in different tiles and warps plus a late narrow peak
-    nch = 4
-    w = W.Workload("spsw_long", 500.0, -200.0 / nch, nch, 1.024e-3, 41000, 1, 8, (W.DMRange(0.0, 1.0, 3, 1),), 1, 0, 0)
-    x = np.zeros((1, nch, 41000), dtype=np.uint8)
-    plan, got, ref = _sps_both(w, x, K, 2.0)
-    _check_all(got, ref)
-    assert (got["tmax"] == 0).all() and (got["snr"] == 0).all()
-    for t0 in (5000, 1030, 20500, 33333):            # the same pulse four times: the earliest position is reported
-        x[0, :, t0:t0 + 3] = 90
-    plan, got, ref = _sps_both(w, x, K, 2.0)
-    _check_all(got, ref)
-    x[0, :, 40960:40962] = 250                        # a stronger one a few samples before the end of the row (its tail loop)
-    x[0, 0, 100] = 1
-    plan, got, ref = _sps_both(w, x, K, 2.0)
-    _check_all(got, ref)
-    # eleven ranges of different row lengths (two launches of the merged kernel), noise with pulses
-    rgs = tuple(W.DMRange(10.0 * i, 1.0 + 0.3 * i, 3 + i % 4, (1, 2, 4, 8)[i % 4]) for i in range(11))
-    w = W.Workload("spsw_many", 700.0, -300.0 / 16, 16, 1.024e-3, 9000, 1, 8, rgs, 1, 0, 0)
-    x = np.random.default_rng(77).integers(100, 140, size=(1, 16, 9000), dtype=np.uint8)
-    x[0, :, 4000:4006] += 60
-    plan, got, ref = _sps_both(w, x, K, 4.0)
-    _check_all(got, ref)
-
-
 # ---- the candidate list (dd_sps_candidates) and the row statistics of the dedispersion epilogue -------------------------
 def _candidates_gpu(plan, plane, K, thr, cnt, max_cands):
     import torch
@@ -251,3 +204,51 @@ def test_row_stats_with_the_direct_kernel_and_subband_variant():
     p16 = B.Plan(500.0, -1.0, 16, 1e-3, 4096, [(0.0, 1.0, 2, 1)], in_bits=16)
     with pytest.raises(B.DDError):
         p16.set_row_stats(st)
+
+
+# ---- last on purpose: written after GPU access had closed, so a failure here hides no other test ----
+def _check_all(got, ref):
+    for k in ("tmax", "count"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert np.array_equal(got["snr"].view(np.uint32), ref["snr"].view(np.uint32))
+
+
+@pytest.mark.parametrize("K", [1, 4, 8, 9])
+def test_sps_barrier_free_kernel_edge_cases(K):
+    """Up to 9 widths and 32-bit sums run in dd_sps_warp_kernel (every warp filters tiles of its own; records per warp and
+    tile; all ranges in one launch): rows shorter than one warp tile and than the widest filter, constant and all-zero rows
+    (every window ties: the first one wins, across warps and tiles), equal maxima far apart, a late narrow peak in a long
+    row, a threshold below everything (every window counted), two beams, and more ranges than one launch takes."""
+    nch = 8
+    # short rows, constant plane (sigma = 0), then random data with a threshold that counts every window
+    w = W.Workload("spsw_short", 500.0, -200.0 / nch, nch, 1.024e-3, 700, 2, 8,
+                   (W.DMRange(0.0, 1.0, 5, 1), W.DMRange(0.0, 1.0, 3, 4)), 1, 0, 0)
+    x = np.full((2, nch, 700), 100, dtype=np.uint8)
+    plan, got, ref = _sps_both(w, x, K, 1.0)
+    _check_all(got, ref)
+    assert (got["snr"] == 0).all()
+    x = np.random.default_rng(30 + K).integers(0, 256, size=(2, nch, 700), dtype=np.uint8)
+    plan, got, ref = _sps_both(w, x, K, -50.0)
+    _check_all(got, ref)
+    # long rows (40 warp tiles): all zero; then equal maxima in different tiles and warps plus a late narrow peak
+    nch = 4
+    w = W.Workload("spsw_long", 500.0, -200.0 / nch, nch, 1.024e-3, 41000, 1, 8, (W.DMRange(0.0, 1.0, 3, 1),), 1, 0, 0)
+    x = np.zeros((1, nch, 41000), dtype=np.uint8)
+    plan, got, ref = _sps_both(w, x, K, 2.0)
+    _check_all(got, ref)
+    assert (got["tmax"] == 0).all() and (got["snr"] == 0).all()
+    for t0 in (5000, 1030, 20500, 33333):            # the same pulse four times: the earliest position is reported
+        x[0, :, t0:t0 + 3] = 90
+    plan, got, ref = _sps_both(w, x, K, 2.0)
+    _check_all(got, ref)
+    x[0, :, 40960:40962] = 250                        # a stronger one a few samples before the end of the row (its tail loop)
+    x[0, 0, 100] = 1
+    plan, got, ref = _sps_both(w, x, K, 2.0)
+    _check_all(got, ref)
+    # eleven ranges of different row lengths (two launches of the merged kernel), noise with pulses
+    rgs = tuple(W.DMRange(10.0 * i, 1.0 + 0.3 * i, 3 + i % 4, (1, 2, 4, 8)[i % 4]) for i in range(11))
+    w = W.Workload("spsw_many", 700.0, -300.0 / 16, 16, 1.024e-3, 9000, 1, 8, rgs, 1, 0, 0)
+    x = np.random.default_rng(77).integers(100, 140, size=(1, 16, 9000), dtype=np.uint8)
+    x[0, :, 4000:4006] += 60
+    plan, got, ref = _sps_both(w, x, K, 4.0)
+    _check_all(got, ref)
